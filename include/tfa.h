@@ -1,0 +1,152 @@
+/* include/tfa.h — C ABI of libtfa: two-fluid finite-volume assembly on one B200 (sm_100a).
+ *
+ * What it computes: one Newton-step assembly of the implicit ideal two-fluid (ion + electron +
+ * full Maxwell with hyperbolic divergence cleaning) finite-volume method of arXiv 1809.02532 on
+ * an unstructured 2-D triangle mesh with 18 FP64 unknowns per cell: the pseudo-steady residual
+ * R~ (Eq. 13) and its block Jacobian dR~/dP (Eq. 14; computed numerically,
+ * L130, by the perturbation loop of Algorithm 1) in 18x18 BSR form, ready for an
+ * external Krylov solver.  "L<n>" cites a line of the paper text; "S<n>" a reading in DESIGN.md.
+ *
+ * Conventions
+ *   NEQ = 18.  Variable (column) order: 0..2 B, 3..5 E, 6 Psi, 7 Phi, 8 rho_i, 9 rho_e,
+ *   10..12 u_i, 13..15 u_e, 16 T_i, 17 T_e  (update variables "RhoiViTi", L181).  Equation (row)
+ *   order is the same with rho -> mass, u -> momentum, T -> total energy (Eq. 3-6).
+ *   Normalisation: mu0 = 1, eps0 = 1/c^2, k_B = 1, m_i = 1, m_e = 1/mass_ratio, q_i = +1, q_e = -1.
+ *   States are array-of-structs [n_cells][18] FP64.  All cell ids are POST-reorder ids.
+ *
+ * Pointers: every `const double* state...`, `double* rhs`, `double* bsr_vals`, `grad`, `phi` of
+ * the device entry points is a DEVICE pointer owned by the caller (e.g. a torch tensor's
+ * data_ptr()); the library neither frees nor retains them.  Mesh inputs of tfa_mesh_create are
+ * HOST pointers and are copied.  `tfa_mesh_get` writes to HOST memory.  Entry points ending in
+ * `_host` take HOST pointers and do the copies themselves.
+ *
+ * Streams: `stream` is a cudaStream_t passed as void* (NULL = default stream).  Device entry
+ * points are asynchronous on it and never synchronise; `_host` entry points and the mesh
+ * builders synchronise the stream before returning.
+ *
+ * Errors: every int-returning function gives 0 on success or a negative TFA_E* code; no C++
+ * exception crosses the ABI; tfa_last_error() returns a thread-local message for the last
+ * failure.  Non-physical face states (rho <= 0 or T <= 0) are counted on the device and
+ * reported lazily by tfa_check().
+ */
+#ifndef TFA_H
+#define TFA_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TFA_NEQ 18
+#define TFA_BLOCK (TFA_NEQ * TFA_NEQ)
+
+enum { TFA_OK = 0, TFA_EINVAL = -1, TFA_EMESH = -2, TFA_ENOMEM = -3, TFA_ECUDA = -4, TFA_ENONPHYS = -5 };
+
+/* Physical constants of the model (the paper's "dco" of EulerMFMHDTerm, L177). */
+typedef struct tfa_physics {
+  double gamma_gas;     /* specific-heat ratio of both fluids (L555); default 5/3 */
+  double mass_ratio;    /* m_i/m_e (L555); default 25 */
+  double c;             /* speed of light in normalised units (L431); default 20 */
+  double gamma_psi;     /* B-cleaning speed factor: flux term gamma^2 Psi (Eq. 2; S1); default 1 */
+  double chi_phi;       /* E-cleaning speed factor: flux term (chi c)^2 Phi (Eq. 2); default 1 */
+  double rusanov_alpha; /* scale of the Rusanov dissipation |A_n| (Eq. 9; S3); default 1 */
+} tfa_physics;
+
+/* Constants of the numerical methods (the "dco"s of the flux, limiter and Jacobian, L195). */
+typedef struct tfa_numerics {
+  double fd_delta;              /* relative perturbation of the numerical Jacobian (L130; S7); 1e-6 */
+  double fd_ref[TFA_NEQ];       /* eps_k = fd_delta * max(|P_k|, fd_ref[k]); 1, except rho_e: 1/mass_ratio */
+  double venkat_K;              /* Venkatakrishnan K, eps^2 = (K sqrt(Omega))^3 (L208; S13); 1 */
+  double lsq_weight_power;      /* least-squares weight w = |d|^-p (L74; S12); 2 */
+  double ausm_Kp, ausm_Ku, ausm_sigma, ausm_beta;  /* AUSM+-up constants (L95-99; S4): 1/4, 3/4, 1, 1/8 */
+  double ausm_Minf[2];          /* cut-off Mach number per species (S4); 0.1 */
+  int32_t term_mask;            /* bit0 convective flux, bit1 source, bit2 BDF2 time term; 7 */
+  int32_t pad_;
+} tfa_numerics;
+
+typedef struct tfa_mesh tfa_mesh;
+typedef struct tfa_ctx tfa_ctx;
+
+/* items for tfa_mesh_get / tfa_mesh_device_ptr */
+enum {
+  TFA_FACE_CELLS = 0,      /* int32 [n_faces][2]: (L, R) with L < R, R = -1 on the boundary (S10) */
+  TFA_CELL_FACES = 1,      /* int32 [n_cells][3]: face of local edge k = (node k -> node k+1) */
+  TFA_STENCIL_PTR = 2,     /* int32 [n_cells+1]: CSR of the face-vertex neighbour stencil (L74) */
+  TFA_STENCIL_IDX = 3,     /* int32 [n_stencil]: ascending, unique, without the cell itself */
+  TFA_BSR_ROWPTR = 4,      /* int32 [n_cells+1] */
+  TFA_BSR_COL = 5,         /* int32 [nnzb]: self + face neighbours, ascending (cuSPARSE bsr layout) */
+  TFA_PERM = 6,            /* int32 [n_cells]: new cell id -> cell id in the arrays given to mesh_create */
+  TFA_VOLUME = 7,          /* f64 [n_cells]: cell area Omega_i */
+  TFA_FACE_NORMAL_LEN = 8, /* f64 [n_faces][3]: unit normal (L -> R) and length Sigma_f */
+  TFA_CENTROID = 9,        /* f64 [n_cells][2] (in the cell's own, unwrapped frame) */
+  TFA_FACE_NODES = 10,     /* int32 [n_faces][2]: (lo, hi) node ids; faces are sorted by this key */
+  TFA_CELL_NBR = 11        /* int32 [n_cells][3]: neighbour across local edge k, -1 on the boundary */
+};
+
+/* ---- step a1: connectivity, geometry, stencil, BSR pattern (L74, L230, L276-319 Listing 1) ----
+ * node_xy [n_nodes][2] f64, cell_nodes [n_cells][3] int32 counter-clockwise, cell_xy
+ * [n_cells][3][2] f64 per-cell corner coordinates (needed for periodic meshes, where node ids are
+ * identified topologically; NULL = gather from node_xy).  HOST pointers, copied.  All derived
+ * arrays are built by CUDA kernels on `stream` and owned by the mesh.
+ * TFA_EMESH: clockwise/degenerate cell, node pair shared by > 2 cells, a cell that neighbours
+ * itself or reaches one neighbour through two faces (periodic direction narrower than 3 cells). */
+int tfa_mesh_create(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                    const int32_t* cell_nodes, const double* cell_xy, void* stream);
+/* Renumber the cells for locality and rebuild every derived array under the same rules.
+ * kind 0: none; 1: reverse Cuthill-McKee on the face-neighbour graph, computed on the device
+ * (S11: start = unvisited cell of minimum (degree, id); neighbours appended by (degree, id));
+ * 2: user_perm[new] = old (HOST pointer, must be a bijection).  Permutations compose into PERM. */
+int tfa_mesh_reorder(tfa_mesh* m, int kind, const int32_t* user_perm, void* stream);
+int tfa_mesh_sizes(const tfa_mesh* m, int64_t* n_cells, int64_t* n_faces, int64_t* nnzb,
+                   int64_t* n_stencil);
+/* Copy one item to host memory; `bytes` must equal the item's size. */
+int tfa_mesh_get(const tfa_mesh* m, int which, void* host_dst, int64_t bytes);
+/* Device pointer of an int32 pattern item (TFA_BSR_ROWPTR, TFA_BSR_COL, TFA_PERM, ...) for the
+ * solver hand-over (zero copy, as Listing 3); valid until destroy/reorder. */
+const void* tfa_mesh_device_ptr(const tfa_mesh* m, int which);
+void tfa_mesh_destroy(tfa_mesh* m);
+
+/* ---- constants and workspace ---- */
+void tfa_default_physics(tfa_physics* p);
+void tfa_default_numerics(tfa_numerics* n, const tfa_physics* p);
+int  tfa_ctx_create(tfa_ctx** out);
+int  tfa_set_physics(tfa_ctx* ctx, const tfa_physics* p);
+int  tfa_set_numerics(tfa_ctx* ctx, const tfa_numerics* n);
+void tfa_ctx_destroy(tfa_ctx* ctx);
+
+/* ---- step a2 (test hook): least-squares gradient (L74) and Venkatakrishnan limiter (L208) ----
+ * grad [n_cells][18][2], phi [n_cells][18]: DEVICE pointers. */
+int tfa_gradients(tfa_ctx* ctx, const tfa_mesh* m, const double* state, double* grad, double* phi,
+                  void* stream);
+
+/* ---- steps a2..a7: residual + BSR Jacobian (Alg. 1; Eq. 8-14) ----
+ * rhs [n_cells][18] = -R~(P);  bsr_vals [nnzb][18][18] row-major blocks of dR~/dP in the
+ * mesh's BSR pattern (64-bit offsets inside).  Every entry of both is overwritten (no memset
+ * needed, unlike Listing 4); bsr_vals may be NULL for a residual-only evaluation.
+ * state_n / state_nm1 are P^n and P^{n-1} of the BDF2 term (Eq. 13).  Deterministic: two calls
+ * on the same inputs give bit-identical outputs (no atomics on the data path). */
+int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                 const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream);
+/* Same with HOST buffers: copies the three states in, assembles, copies rhs and bsr_vals out,
+ * synchronises.  Pinned host memory makes the copies asynchronous DMA; pageable memory works. */
+int tfa_assemble_host(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                      const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream);
+/* Synchronise and report: 0, or TFA_ENONPHYS if any assembly since the last check met a face
+ * state with rho <= 0 or T <= 0 (S16), or TFA_ECUDA for a sticky CUDA error. */
+int tfa_check(tfa_ctx* ctx, void* stream);
+
+/* ---- measurement probes (roofline denominators measured in the same run) ----
+ * tfa_probe_dfma: `grid` CTAs x 256 threads each run `iters` x 8 independent FP64 FMAs per
+ * thread (2 flops each) -> flops = grid*256*iters*8*2.  tfa_probe_copy: dst[i] = src[i] for n
+ * doubles with 16-byte vector accesses -> bytes = 16*n.  Both asynchronous on `stream`. */
+int tfa_probe_dfma(int grid, int iters, double* sink, void* stream);
+int tfa_probe_copy(const double* src, double* dst, int64_t n, void* stream);
+
+/* Number of kernels the last tfa_assemble launched (for bench.py's gpu_launches). */
+int tfa_launches_per_assemble(const tfa_ctx* ctx);
+const char* tfa_last_error(void);
+const char* tfa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,224 @@
+"""Thin Python binding of include/tfa.h — argument marshalling only.
+
+Same names as the C entry points (``mesh_create``, ``mesh_reorder``, ``set_physics``,
+``assemble``, ...).  PyTorch supplies device memory and the stream; every step of the path runs
+in libtfa's CUDA kernels.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+import torch
+
+from . import _lib
+from ._lib import NEQ, BLOCK, Physics, Numerics, TfaError  # noqa: F401
+
+MESH_ITEMS = dict(face_cells=(0, np.int32), cell_faces=(1, np.int32), stencil_ptr=(2, np.int32),
+                  stencil_idx=(3, np.int32), bsr_rowptr=(4, np.int32), bsr_col=(5, np.int32),
+                  perm=(6, np.int32), volume=(7, np.float64), face_normal_len=(8, np.float64),
+                  centroid=(9, np.float64), face_nodes=(10, np.int32), cell_nbr=(11, np.int32))
+_REORDER = {"none": 0, "rcm": 1, "user": 2}
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _hp(a: np.ndarray | None):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _dp(t: torch.Tensor | None):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise ValueError("expected a contiguous float64 CUDA tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+def default_physics(src=None) -> Physics:
+    p = Physics()
+    _lib.load().tfa_default_physics(C.byref(p))
+    if src is not None:
+        for name, _ in Physics._fields_:
+            setattr(p, name, float(getattr(src, name)))
+    return p
+
+
+def default_numerics(ph: Physics | None = None, **over) -> Numerics:
+    ph = ph or default_physics()
+    n = Numerics()
+    _lib.load().tfa_default_numerics(C.byref(n), C.byref(ph))
+    for k, v in over.items():
+        if k in ("fd_ref", "ausm_Minf"):
+            arr = getattr(n, k)
+            for i, x in enumerate(v):
+                arr[i] = float(x)
+        else:
+            setattr(n, k, v)
+    return n
+
+
+class Mesh:
+    """Owner of a ``tfa_mesh*`` (tfa_mesh_create / tfa_mesh_destroy)."""
+
+    def __init__(self, node_xy, cell_nodes, cell_xy=None):
+        lib = _lib.load()
+        self._h = C.c_void_p()
+        node_xy = np.ascontiguousarray(node_xy, dtype=np.float64)
+        cell_nodes = np.ascontiguousarray(cell_nodes, dtype=np.int32)
+        cxy = None if cell_xy is None else np.ascontiguousarray(cell_xy, dtype=np.float64)
+        _lib.check(lib.tfa_mesh_create(C.byref(self._h), node_xy.shape[0], _hp(node_xy), cell_nodes.shape[0],
+                                       _hp(cell_nodes), _hp(cxy), _stream()))
+        self._sizes()
+
+    @classmethod
+    def from_input(cls, mi) -> "Mesh":
+        return cls(mi.node_xy, mi.cell_nodes, mi.cell_xy)
+
+    def _sizes(self):
+        v = [C.c_int64() for _ in range(4)]
+        _lib.check(_lib.load().tfa_mesh_sizes(self._h, *[C.byref(x) for x in v]))
+        self.n_cells, self.n_faces, self.nnzb, self.n_stencil = [int(x.value) for x in v]
+
+    def reorder(self, kind: str = "rcm", perm=None):
+        pp = None if perm is None else np.ascontiguousarray(perm, dtype=np.int32)
+        _lib.check(_lib.load().tfa_mesh_reorder(self._h, _REORDER[kind], _hp(pp), _stream()))
+        self._sizes()
+
+    def get(self, name: str) -> np.ndarray:
+        which, dt = MESH_ITEMS[name]
+        n = dict(face_cells=2 * self.n_faces, face_nodes=2 * self.n_faces, cell_faces=3 * self.n_cells,
+                 cell_nbr=3 * self.n_cells, stencil_ptr=self.n_cells + 1, stencil_idx=self.n_stencil,
+                 bsr_rowptr=self.n_cells + 1, bsr_col=self.nnzb, perm=self.n_cells, volume=self.n_cells,
+                 face_normal_len=3 * self.n_faces, centroid=2 * self.n_cells)[name]
+        out = np.empty(n, dtype=dt)
+        _lib.check(_lib.load().tfa_mesh_get(self._h, which, _hp(out), out.nbytes))
+        shape = dict(face_cells=(-1, 2), face_nodes=(-1, 2), cell_faces=(-1, 3), cell_nbr=(-1, 3),
+                     face_normal_len=(-1, 3), centroid=(-1, 2)).get(name)
+        return out.reshape(shape) if shape else out
+
+    def device_ptr(self, name: str) -> int:
+        return int(_lib.load().tfa_mesh_device_ptr(self._h, MESH_ITEMS[name][0]) or 0)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.load().tfa_mesh_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Context:
+    """Owner of a ``tfa_ctx*``: physics + numerics constants and the per-mesh workspace."""
+
+    def __init__(self, physics=None, numerics: Numerics | None = None):
+        self._h = C.c_void_p()
+        _lib.check(_lib.load().tfa_ctx_create(C.byref(self._h)))
+        self.physics = physics if isinstance(physics, Physics) else default_physics(physics)
+        self.set_physics(self.physics)
+        self.set_numerics(numerics or default_numerics(self.physics))
+
+    def set_physics(self, p: Physics):
+        _lib.check(_lib.load().tfa_set_physics(self._h, C.byref(p)))
+        self.physics = p
+
+    def set_numerics(self, n: Numerics):
+        _lib.check(_lib.load().tfa_set_numerics(self._h, C.byref(n)))
+        self.numerics = n
+
+    def gradients(self, mesh: Mesh, state: torch.Tensor):
+        grad = torch.empty((mesh.n_cells, NEQ, 2), dtype=torch.float64, device=state.device)
+        phi = torch.empty((mesh.n_cells, NEQ), dtype=torch.float64, device=state.device)
+        _lib.check(_lib.load().tfa_gradients(self._h, mesh._h, _dp(state), _dp(grad), _dp(phi), _stream()))
+        return grad, phi
+
+    def assemble(self, mesh: Mesh, state, state_n=None, state_nm1=None, dt=1e-3, rhs=None, vals=None,
+                 jacobian=True):
+        """tfa_assemble on device tensors.  Returns (rhs, vals); asynchronous on the current stream."""
+        state_n = state if state_n is None else state_n
+        state_nm1 = state if state_nm1 is None else state_nm1
+        if rhs is None:
+            rhs = torch.empty((mesh.n_cells, NEQ), dtype=torch.float64, device=state.device)
+        if vals is None and jacobian:
+            vals = torch.empty((mesh.nnzb, NEQ, NEQ), dtype=torch.float64, device=state.device)
+        _lib.check(_lib.load().tfa_assemble(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
+                                            _dp(rhs), _dp(vals) if jacobian else None, _stream()))
+        return rhs, vals
+
+    def assemble_host(self, mesh: Mesh, state, state_n, state_nm1, dt, rhs, vals):
+        """tfa_assemble_host on HOST buffers (numpy arrays or CPU tensors, ideally pinned)."""
+        def hp(x):
+            if x is None:
+                return None
+            if isinstance(x, torch.Tensor):
+                assert not x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+                return C.c_void_p(x.data_ptr())
+            assert x.dtype == np.float64 and x.flags.c_contiguous
+            return _hp(x)
+        _lib.check(_lib.load().tfa_assemble_host(self._h, mesh._h, hp(state), hp(state_n), hp(state_nm1), float(dt),
+                                                 hp(rhs), hp(vals), _stream()))
+        return rhs, vals
+
+    def check(self):
+        _lib.check(_lib.load().tfa_check(self._h, _stream()))
+
+    @property
+    def launches_per_assemble(self) -> int:
+        return int(_lib.load().tfa_launches_per_assemble(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.load().tfa_ctx_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def probe_dfma(grid: int, iters: int, sink: torch.Tensor):
+    _lib.check(_lib.load().tfa_probe_dfma(int(grid), int(iters), _dp(sink), _stream()))
+    return grid * 256 * iters * 8 * 2   # flops
+
+
+def probe_copy(src: torch.Tensor, dst: torch.Tensor):
+    n = src.numel()
+    _lib.check(_lib.load().tfa_probe_copy(_dp(src), _dp(dst), n, _stream()))
+    return 16 * n                       # bytes read + written
+
+
+# C-style aliases, same names as the ABI
+def mesh_create(node_xy, cell_nodes, cell_xy=None) -> Mesh:
+    return Mesh(node_xy, cell_nodes, cell_xy)
+
+
+def mesh_reorder(mesh: Mesh, kind="rcm", perm=None):
+    mesh.reorder(kind, perm)
+
+
+def ctx_create(physics=None, numerics=None) -> Context:
+    return Context(physics, numerics)
+
+
+def set_physics(ctx: Context, p: Physics):
+    ctx.set_physics(p)
+
+
+def set_numerics(ctx: Context, n: Numerics):
+    ctx.set_numerics(n)
+
+
+def assemble(ctx: Context, mesh: Mesh, state, state_n=None, state_nm1=None, dt=1e-3, **kw):
+    return ctx.assemble(mesh, state, state_n, state_nm1, dt, **kw)
+
+
+def destroy(obj):
+    obj.close()

@@ -1,0 +1,100 @@
+// tfa_common.cuh — internal types shared by the translation units of libtfa (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/tfa.h"
+
+#define NEQ TFA_NEQ
+#define BLK TFA_BLOCK
+
+namespace tfa {
+
+int set_error(int code, const std::string& msg);
+
+#define TFA_CUDA(expr)                                                                          \
+  do {                                                                                          \
+    cudaError_t e__ = (expr);                                                                   \
+    if (e__ != cudaSuccess)                                                                     \
+      return tfa::set_error(e__ == cudaErrorMemoryAllocation ? TFA_ENOMEM : TFA_ECUDA,          \
+                            std::string(#expr) + ": " + cudaGetErrorString(e__));               \
+  } while (0)
+
+#define TFA_TRY(expr)          \
+  do {                         \
+    int rc__ = (expr);         \
+    if (rc__ != 0) return rc__; \
+  } while (0)
+
+inline unsigned cdiv(int64_t a, int64_t b) { return (unsigned)((a + b - 1) / b); }
+
+// Per-cell geometry record, 24 doubles = 192 B:
+//   for local face k = 0..2 at [8k .. 8k+7]:
+//     0 nx, 1 ny   unit normal in CANONICAL orientation (from the face's L cell towards R)
+//     2 len        face length Sigma_f
+//     3 dxo, 4 dyo face midpoint minus OWN centroid (own corner coordinates)
+//     5 dxn, 6 dyn face midpoint minus NEIGHBOUR centroid (neighbour's corner coordinates)
+//     7 extra      k=0: volume Omega_i;  k=1: sqrt(Omega_i);  k=2: unused (0)
+constexpr int CGEO = 24;
+
+template <class T>
+struct DevBuf {
+  T* p = nullptr;
+  int64_t n = 0;
+  DevBuf() = default;
+  DevBuf(const DevBuf&) = delete;
+  DevBuf& operator=(const DevBuf&) = delete;
+  ~DevBuf() { release(); }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    n = 0;
+  }
+  cudaError_t alloc(int64_t count) {
+    release();
+    if (count <= 0) count = 1;
+    cudaError_t e = cudaMalloc((void**)&p, (size_t)count * sizeof(T));
+    if (e == cudaSuccess) n = count;
+    return e;
+  }
+  void swap(DevBuf& o) {
+    T* tp = p; p = o.p; o.p = tp;
+    int64_t tn = n; n = o.n; o.n = tn;
+  }
+};
+
+}  // namespace tfa
+
+struct tfa_mesh {
+  int64_t nn = 0, nc = 0, nf = 0, nnzb = 0, nst = 0;
+  uint64_t generation = 0;   // bumped by every (re)build; ctx workspaces key on it
+  tfa::DevBuf<double> node_xy;     // [nn][2]
+  tfa::DevBuf<int32_t> cell_nodes; // [nc][3]
+  tfa::DevBuf<double> cell_xy;     // [nc][3][2]
+  tfa::DevBuf<int32_t> perm;       // [nc] new -> original
+  // derived
+  tfa::DevBuf<int32_t> face_nodes, face_cells;  // [nf][2]
+  tfa::DevBuf<int32_t> cell_faces, cell_nbr;    // [nc][3]
+  tfa::DevBuf<int32_t> st_ptr, st_idx;          // CSR stencil
+  tfa::DevBuf<double> st_d;                     // [nst][2] centroid displacement (S9)
+  tfa::DevBuf<int32_t> bsr_rowptr, bsr_col;
+  tfa::DevBuf<double> cen;                      // [nc][2]
+  tfa::DevBuf<double> cgeo;                     // [nc][24]
+};
+
+struct tfa_ctx {
+  tfa_physics ph;
+  tfa_numerics nu;
+  // workspace, keyed on (mesh, generation, lsq_weight_power)
+  const tfa_mesh* ws_mesh = nullptr;
+  uint64_t ws_generation = 0;
+  double ws_power = -1.0;
+  tfa::DevBuf<double> lsq_coef;   // [nst][2]
+  tfa::DevBuf<double> lgrad;      // [nc][18][2] limited gradient phi*grad
+  tfa::DevBuf<int32_t> flags;     // [4] device counters: 0 = non-physical states
+  // staging for tfa_assemble_host
+  tfa::DevBuf<double> h_state[3], h_rhs, h_vals;
+  int launches = 0;
+};

@@ -1,0 +1,708 @@
+// tfa_mesh.cu — step a1: mesh connectivity, geometry, stencil, BSR pattern and cell reordering,
+// built on the device (PAPER.md L74 stencil, L230 cell->faces loop, L276-319 Listing 1 pattern).
+//
+// Everything derived from (cell_nodes, cell_xy) is produced by the kernels below under the
+// canonical rules of DESIGN.md (readings S9-S11), so that the result is bit-exact and independent
+// of thread scheduling: faces are numbered by sorted (lo node, hi node) key, L is the smaller cell
+// id, stencil and BSR columns are ascending.  Sorting and prefix sums use CUB device primitives
+// (library steps); the rest is hand-written.
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
+
+#include <vector>
+
+#include "tfa_common.cuh"
+
+namespace tfa {
+
+thread_local std::string g_last_error;
+int set_error(int code, const std::string& msg) {
+  g_last_error = msg;
+  return code;
+}
+
+namespace {
+
+enum MeshErr : int {
+  ERR_CW = 1,          // non-positive area
+  ERR_REPEAT = 2,      // a cell repeats a node id
+  ERR_RANGE = 4,       // node id out of range
+  ERR_NONMANIFOLD = 8, // node pair shared by > 2 cells
+  ERR_SELFNBR = 16,    // a cell is its own neighbour
+  ERR_DUPNBR = 32,     // two faces of a cell lead to the same neighbour
+  ERR_STENCIL = 64,    // stencil candidate list overflow
+  ERR_PERM = 128       // permutation is not a bijection
+};
+
+constexpr int TPB = 256;
+constexpr int MAXCAND = 192;   // sum of the three node degrees of a cell (Delaunay: ~18, max seen 30)
+
+// ---- geometry of each cell from its own corner coordinates ----
+__global__ void k_cell_geom(int64_t nc, int64_t nn, const int32_t* __restrict__ cell_nodes,
+                            const double* __restrict__ cell_xy, double* __restrict__ cen,
+                            double* __restrict__ vol, double* __restrict__ olen, double* __restrict__ onrm,
+                            double* __restrict__ ooff, int32_t* err) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  const double* X = cell_xy + 6 * i;
+  double x[3] = {X[0], X[2], X[4]}, y[3] = {X[1], X[3], X[5]};
+  double cx = (x[0] + x[1] + x[2]) / 3.0, cy = (y[0] + y[1] + y[2]) / 3.0;
+  double area = 0.5 * ((x[1] - x[0]) * (y[2] - y[0]) - (y[1] - y[0]) * (x[2] - x[0]));
+  if (!(area > 0.0)) { atomicOr(err, ERR_CW); atomicMin(err + 1, (int32_t)i); }
+  cen[2 * i] = cx;
+  cen[2 * i + 1] = cy;
+  vol[i] = area;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    int k1 = (k + 1) % 3;
+    double dx = x[k1] - x[k], dy = y[k1] - y[k];
+    double len = sqrt(dx * dx + dy * dy);
+    olen[3 * i + k] = len;
+    onrm[6 * i + 2 * k] = dy / len;
+    onrm[6 * i + 2 * k + 1] = -dx / len;
+    ooff[6 * i + 2 * k] = 0.5 * (x[k] + x[k1]) - cx;
+    ooff[6 * i + 2 * k + 1] = 0.5 * (y[k] + y[k1]) - cy;
+  }
+  int32_t a = cell_nodes[3 * i], b = cell_nodes[3 * i + 1], c = cell_nodes[3 * i + 2];
+  if (a == b || b == c || a == c) { atomicOr(err, ERR_REPEAT); atomicMin(err + 1, (int32_t)i); }
+  if (a < 0 || b < 0 || c < 0 || a >= nn || b >= nn || c >= nn) atomicOr(err, ERR_RANGE);
+}
+
+__global__ void k_gather_xy(int64_t n3, int64_t nn, const int32_t* __restrict__ cell_nodes,
+                            const double* __restrict__ node_xy, double* __restrict__ cell_xy, int32_t* err) {
+  int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (q >= n3) return;
+  int32_t v = cell_nodes[q];
+  if (v < 0 || v >= nn) { atomicOr(err, ERR_RANGE); v = 0; }
+  cell_xy[2 * q] = node_xy[2 * (int64_t)v];
+  cell_xy[2 * q + 1] = node_xy[2 * (int64_t)v + 1];
+}
+
+// ---- faces: unique (lo, hi) node pairs, numbered in sorted key order (S10) ----
+__global__ void k_edge_keys(int64_t nc, int64_t nn, const int32_t* __restrict__ cell_nodes,
+                            uint64_t* __restrict__ keys, int32_t* __restrict__ vals) {
+  int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= 3 * nc) return;
+  int64_t c = e / 3;
+  int k = (int)(e % 3);
+  int32_t a = cell_nodes[3 * c + k], b = cell_nodes[3 * c + (k + 1) % 3];
+  uint64_t lo = (uint64_t)min(a, b), hi = (uint64_t)max(a, b);
+  keys[e] = lo * (uint64_t)nn + hi;
+  vals[e] = (int32_t)e;
+}
+
+__global__ void k_face_heads(int64_t ne, const uint64_t* __restrict__ keys, int32_t* __restrict__ head,
+                             int32_t* err) {
+  int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= ne) return;
+  head[e] = (e == 0 || keys[e] != keys[e - 1]) ? 1 : 0;
+  if (e >= 2 && keys[e] == keys[e - 2]) atomicOr(err, ERR_NONMANIFOLD);
+}
+
+__global__ void k_faces(int64_t ne, int64_t nn, const uint64_t* __restrict__ keys,
+                        const int32_t* __restrict__ vals, const int32_t* __restrict__ fid,
+                        int32_t* __restrict__ face_nodes, int32_t* __restrict__ face_cells,
+                        int32_t* __restrict__ cell_faces, int32_t* err) {
+  int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= ne) return;
+  const int32_t f = fid[e] - 1;
+  const uint64_t key = keys[e];
+  const int32_t v = vals[e];
+  const int32_t c = v / 3;
+  cell_faces[v] = f;
+  const bool is_head = (e == 0 || keys[e - 1] != key);
+  if (is_head) {
+    face_nodes[2 * (int64_t)f] = (int32_t)(key / (uint64_t)nn);
+    face_nodes[2 * (int64_t)f + 1] = (int32_t)(key % (uint64_t)nn);
+    face_cells[2 * (int64_t)f] = c;   // stable sort of ascending values: the smaller cell id comes first
+    if (!(e + 1 < ne && keys[e + 1] == key)) face_cells[2 * (int64_t)f + 1] = -1;
+  } else {
+    face_cells[2 * (int64_t)f + 1] = c;
+    if (vals[e - 1] / 3 == c) atomicOr(err, ERR_SELFNBR);
+  }
+}
+
+__global__ void k_cell_nbr(int64_t nc, const int32_t* __restrict__ cell_faces,
+                           const int32_t* __restrict__ face_cells, int32_t* __restrict__ cell_nbr,
+                           int32_t* __restrict__ rowcnt, int32_t* err) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  int32_t nb[3];
+  int cnt = 1;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    int64_t f = cell_faces[3 * i + k];
+    int32_t L = face_cells[2 * f], R = face_cells[2 * f + 1];
+    nb[k] = (L == (int32_t)i) ? R : L;
+    cell_nbr[3 * i + k] = nb[k];
+    cnt += nb[k] >= 0;
+  }
+  if ((nb[0] >= 0 && (nb[0] == nb[1] || nb[0] == nb[2])) || (nb[1] >= 0 && nb[1] == nb[2]))
+    atomicOr(err, ERR_DUPNBR);
+  rowcnt[i] = cnt;
+}
+
+// BSR columns: self + face neighbours, ascending (Listing 1's allNonZero = nbEqs x blocks per row)
+__global__ void k_bsr_cols(int64_t nc, const int32_t* __restrict__ cell_nbr,
+                           const int32_t* __restrict__ rowptr, int32_t* __restrict__ col) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  int32_t c[4] = {(int32_t)i, cell_nbr[3 * i], cell_nbr[3 * i + 1], cell_nbr[3 * i + 2]};
+  const int32_t base = rowptr[i];
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    if (c[a] < 0) continue;
+    int rank = 0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) rank += (c[b] >= 0 && c[b] < c[a]);
+    col[base + rank] = c[a];
+  }
+}
+
+// ---- vertex-neighbour stencil (L74) ----
+__global__ void k_node_pairs(int64_t nc, const int32_t* __restrict__ cell_nodes, uint32_t* __restrict__ keys,
+                             int32_t* __restrict__ vals, int32_t* __restrict__ node_cnt) {
+  int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= 3 * nc) return;
+  int32_t v = cell_nodes[e];
+  keys[e] = (uint32_t)v;
+  vals[e] = (int32_t)(e / 3);
+  atomicAdd(node_cnt + v, 1);   // integer count: the result does not depend on the order
+}
+
+// candidates = union of the cell lists of the three nodes, sorted, unique, without self
+__device__ int stencil_candidates(int64_t i, const int32_t* __restrict__ cell_nodes,
+                                  const int32_t* __restrict__ node_ptr, const int32_t* __restrict__ node_cells,
+                                  int32_t* cand, bool* overflow) {
+  int n = 0;
+  for (int k = 0; k < 3; ++k) {
+    int32_t v = cell_nodes[3 * i + k];
+    for (int32_t q = node_ptr[v]; q < node_ptr[v + 1]; ++q) {
+      int32_t j = node_cells[q];
+      if (j == (int32_t)i) continue;
+      if (n >= MAXCAND) { *overflow = true; return n; }
+      int p = n++;   // insertion sort keeps the list ascending
+      while (p > 0 && cand[p - 1] > j) { cand[p] = cand[p - 1]; --p; }
+      cand[p] = j;
+    }
+  }
+  int u = 0;
+  for (int p = 0; p < n; ++p)
+    if (p == 0 || cand[p] != cand[p - 1]) cand[u++] = cand[p];
+  return u;
+}
+
+__global__ void k_stencil_count(int64_t nc, const int32_t* __restrict__ cell_nodes,
+                                const int32_t* __restrict__ node_ptr, const int32_t* __restrict__ node_cells,
+                                int32_t* __restrict__ cnt, int32_t* err) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  int32_t cand[MAXCAND];
+  bool ovf = false;
+  cnt[i] = stencil_candidates(i, cell_nodes, node_ptr, node_cells, cand, &ovf);
+  if (ovf) atomicOr(err, ERR_STENCIL);
+}
+
+__global__ void k_stencil_fill(int64_t nc, const int32_t* __restrict__ cell_nodes,
+                               const int32_t* __restrict__ node_ptr, const int32_t* __restrict__ node_cells,
+                               const int32_t* __restrict__ st_ptr, const double* __restrict__ cell_xy,
+                               const double* __restrict__ cen, int32_t* __restrict__ st_idx,
+                               double* __restrict__ st_d) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  int32_t cand[MAXCAND];
+  bool ovf = false;
+  const int n = stencil_candidates(i, cell_nodes, node_ptr, node_cells, cand, &ovf);
+  const int32_t base = st_ptr[i];
+  const int32_t ni[3] = {cell_nodes[3 * i], cell_nodes[3 * i + 1], cell_nodes[3 * i + 2]};
+  for (int p = 0; p < n; ++p) {
+    const int64_t j = cand[p];
+    // displacement through the smallest shared node id (S9, S22): periodic-safe, no min-image
+    int32_t v = INT32_MAX;
+    int ai = 0, bj = 0;
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) {
+        int32_t nj = cell_nodes[3 * j + b];
+        if (ni[a] == nj && nj < v) { v = nj; ai = a; bj = b; }
+      }
+    double dx = (cen[2 * j] - cell_xy[6 * j + 2 * bj]) - (cen[2 * i] - cell_xy[6 * i + 2 * ai]);
+    double dy = (cen[2 * j + 1] - cell_xy[6 * j + 2 * bj + 1]) - (cen[2 * i + 1] - cell_xy[6 * i + 2 * ai + 1]);
+    st_idx[base + p] = (int32_t)j;
+    st_d[2 * (int64_t)(base + p)] = dx;
+    st_d[2 * (int64_t)(base + p) + 1] = dy;
+  }
+}
+
+// ---- per-cell geometry record in canonical face orientation (tfa_common.cuh CGEO) ----
+__global__ void k_cgeo(int64_t nc, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ cell_faces,
+                       const double* __restrict__ vol, const double* __restrict__ olen,
+                       const double* __restrict__ onrm, const double* __restrict__ ooff,
+                       double* __restrict__ cgeo) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  double* g = cgeo + CGEO * i;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const int64_t j = cell_nbr[3 * i + k];
+    const int32_t f = cell_faces[3 * i + k];
+    int kj = 0;
+    if (j >= 0)
+      for (int q = 0; q < 3; ++q)
+        if (cell_faces[3 * j + q] == f) kj = q;
+    const bool own_is_L = (j < 0) || (i < j);
+    const int64_t cL = own_is_L ? i : j;
+    const int kL = own_is_L ? k : kj;
+    g[8 * k + 0] = onrm[6 * cL + 2 * kL];
+    g[8 * k + 1] = onrm[6 * cL + 2 * kL + 1];
+    g[8 * k + 2] = olen[3 * cL + kL];
+    g[8 * k + 3] = ooff[6 * i + 2 * k];
+    g[8 * k + 4] = ooff[6 * i + 2 * k + 1];
+    g[8 * k + 5] = j >= 0 ? ooff[6 * j + 2 * kj] : 0.0;
+    g[8 * k + 6] = j >= 0 ? ooff[6 * j + 2 * kj + 1] : 0.0;
+  }
+  g[7] = vol[i];
+  g[15] = sqrt(vol[i]);
+  g[23] = 0.0;
+}
+
+// ---- reverse Cuthill-McKee, one CTA, level-synchronous, deterministic (S11) ----
+// Equivalent to the serial queue algorithm: a cell's parent is the earliest-ordered frontier
+// cell adjacent to it; children of one parent are appended sorted by (degree, id).
+constexpr int RCM_T = 1024;
+__global__ void __launch_bounds__(RCM_T) k_rcm(int32_t nc, const int32_t* __restrict__ nbr,
+                                              int32_t* __restrict__ order, int32_t* __restrict__ pos,
+                                              int32_t* __restrict__ parent) {
+  __shared__ int32_t s_scan[RCM_T];
+  __shared__ unsigned long long s_best;
+  __shared__ int32_t s_lb, s_le, s_total;
+  const int t = threadIdx.x;
+  auto degree = [&](int32_t c) { return (nbr[3 * c] >= 0) + (nbr[3 * c + 1] >= 0) + (nbr[3 * c + 2] >= 0); };
+  for (int32_t c = t; c < nc; c += RCM_T) { pos[c] = -1; parent[c] = INT32_MAX; }
+  if (t == 0) { s_lb = 0; s_le = 0; }
+  __syncthreads();
+  while (true) {
+    int32_t placed = s_le;
+    if (placed >= nc) break;
+    // start of a new component: unvisited cell with minimum (degree, id)
+    if (t == 0) s_best = ~0ull;
+    __syncthreads();
+    unsigned long long best = ~0ull;
+    for (int32_t c = t; c < nc; c += RCM_T)
+      if (pos[c] < 0) {
+        unsigned long long key = ((unsigned long long)degree(c) << 32) | (unsigned)c;
+        best = key < best ? key : best;
+      }
+    atomicMin(&s_best, best);
+    __syncthreads();
+    if (t == 0) {
+      int32_t c = (int32_t)(s_best & 0xffffffffu);
+      order[placed] = c;
+      pos[c] = placed;
+      s_lb = placed;
+      s_le = placed + 1;
+    }
+    __syncthreads();
+    // breadth-first levels
+    while (true) {
+      const int32_t lb = s_lb, le = s_le;
+      if (lb == le) break;
+      // 1. every unvisited neighbour of the frontier records its earliest parent
+      for (int32_t p = lb + t; p < le; p += RCM_T) {
+        const int32_t v = order[p];
+        for (int k = 0; k < 3; ++k) {
+          const int32_t w = nbr[3 * v + k];
+          if (w >= 0 && pos[w] < 0) atomicMin(parent + w, p);
+        }
+      }
+      __syncthreads();
+      // 2. children per frontier cell, exclusive scan over the frontier in chunks of RCM_T
+      int32_t running = 0;
+      for (int32_t p0 = lb; p0 < le; p0 += RCM_T) {
+        const int32_t p = p0 + t;
+        int32_t ch[3];
+        int n = 0;
+        if (p < le) {
+          const int32_t v = order[p];
+          for (int k = 0; k < 3; ++k) {
+            const int32_t w = nbr[3 * v + k];
+            if (w >= 0 && pos[w] < 0 && parent[w] == p) ch[n++] = w;
+          }
+        }
+        s_scan[t] = n;
+        __syncthreads();
+        for (int off = 1; off < RCM_T; off <<= 1) {   // Hillis-Steele inclusive scan
+          int32_t x = t >= off ? s_scan[t - off] : 0;
+          __syncthreads();
+          s_scan[t] += x;
+          __syncthreads();
+        }
+        const int32_t excl = s_scan[t] - n;
+        if (t == RCM_T - 1) s_total = s_scan[t];
+        // sort the <= 3 children by (degree, id) and append
+        for (int a = 1; a < n; ++a) {
+          int32_t w = ch[a];
+          int dw = degree(w);
+          int b = a;
+          while (b > 0 && (degree(ch[b - 1]) > dw || (degree(ch[b - 1]) == dw && ch[b - 1] > w))) {
+            ch[b] = ch[b - 1];
+            --b;
+          }
+          ch[b] = w;
+        }
+        for (int a = 0; a < n; ++a) order[le + running + excl + a] = ch[a];
+        __syncthreads();
+        running += s_total;
+        __syncthreads();
+      }
+      // 3. publish positions of the new level (after all parent tests of this level are done)
+      for (int32_t q = le + t; q < le + running; q += RCM_T) pos[order[q]] = q;
+      __syncthreads();
+      if (t == 0) { s_lb = le; s_le = le + running; }
+      __syncthreads();
+    }
+  }
+}
+
+__global__ void k_reverse(int32_t n, const int32_t* __restrict__ in, int32_t* __restrict__ out) {
+  int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = in[n - 1 - i];
+}
+
+__global__ void k_check_perm(int64_t nc, const int32_t* __restrict__ p, int32_t* __restrict__ hit, int32_t* err) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  int32_t v = p[i];
+  if (v < 0 || v >= nc) { atomicOr(err, ERR_PERM); return; }
+  if (atomicAdd(hit + v, 1) != 0) atomicOr(err, ERR_PERM);
+}
+
+__global__ void k_permute_cells(int64_t nc, const int32_t* __restrict__ p, const int32_t* __restrict__ cn_in,
+                                const double* __restrict__ cx_in, const int32_t* __restrict__ perm_in,
+                                int32_t* __restrict__ cn, double* __restrict__ cx, int32_t* __restrict__ perm) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  const int64_t o = p[i];
+  for (int k = 0; k < 3; ++k) cn[3 * i + k] = cn_in[3 * o + k];
+  for (int k = 0; k < 6; ++k) cx[6 * i + k] = cx_in[6 * o + k];
+  perm[i] = perm_in[o];
+}
+
+__global__ void k_iota(int64_t n, int32_t* p) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) p[i] = (int32_t)i;
+}
+
+__global__ void k_face_geom_out(int64_t nf, const int32_t* __restrict__ face_cells,
+                                const int32_t* __restrict__ cell_faces, const double* __restrict__ cgeo,
+                                double* __restrict__ out) {
+  int64_t f = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (f >= nf) return;
+  const int64_t L = face_cells[2 * f];
+  int k = 0;
+  for (int q = 0; q < 3; ++q)
+    if (cell_faces[3 * L + q] == (int32_t)f) k = q;
+  out[3 * f] = cgeo[CGEO * L + 8 * k];
+  out[3 * f + 1] = cgeo[CGEO * L + 8 * k + 1];
+  out[3 * f + 2] = cgeo[CGEO * L + 8 * k + 2];
+}
+
+__global__ void k_volume_out(int64_t nc, const double* __restrict__ cgeo, double* __restrict__ out) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < nc) out[i] = cgeo[CGEO * i + 7];
+}
+
+std::string describe(int bits, int cell) {
+  std::string s;
+  if (bits & ERR_CW) s += "cell " + std::to_string(cell) + " is not counter-clockwise (area <= 0); ";
+  if (bits & ERR_REPEAT) s += "a cell repeats a node id (periodic direction too narrow); ";
+  if (bits & ERR_RANGE) s += "node id out of range; ";
+  if (bits & ERR_NONMANIFOLD) s += "a node pair is shared by more than 2 cells; ";
+  if (bits & ERR_SELFNBR) s += "a cell is its own neighbour (periodic direction too narrow); ";
+  if (bits & ERR_DUPNBR) s += "two faces of a cell lead to the same neighbour (periodic direction too narrow); ";
+  if (bits & ERR_STENCIL) s += "vertex stencil exceeds the internal candidate limit; ";
+  if (bits & ERR_PERM) s += "permutation is not a bijection; ";
+  return s;
+}
+
+int check_err(DevBuf<int32_t>& err, cudaStream_t st) {
+  int32_t h[2];
+  TFA_CUDA(cudaMemcpyAsync(h, err.p, sizeof(h), cudaMemcpyDeviceToHost, st));
+  TFA_CUDA(cudaStreamSynchronize(st));
+  if (h[0]) return set_error(TFA_EMESH, describe(h[0], h[1]));
+  return 0;
+}
+
+template <class T>
+int exclusive_scan_with_total(const DevBuf<int32_t>& in, int64_t n, DevBuf<T>& out, int64_t* total,
+                              cudaStream_t st) {
+  // out[0..n] : out[i] = sum_{q<i} in[q]; out[n] = total
+  size_t tmp_bytes = 0;
+  cub::DeviceScan::InclusiveSum(nullptr, tmp_bytes, in.p, out.p + 1, (int)n, st);
+  DevBuf<char> tmp;
+  TFA_CUDA(tmp.alloc((int64_t)tmp_bytes));
+  TFA_CUDA(cudaMemsetAsync(out.p, 0, sizeof(T), st));
+  TFA_CUDA(cub::DeviceScan::InclusiveSum(tmp.p, tmp_bytes, in.p, out.p + 1, (int)n, st));
+  T h = 0;
+  TFA_CUDA(cudaMemcpyAsync(&h, out.p + n, sizeof(T), cudaMemcpyDeviceToHost, st));
+  TFA_CUDA(cudaStreamSynchronize(st));
+  *total = (int64_t)h;
+  return 0;
+}
+
+}  // namespace
+
+// Build every derived array of the mesh from (cell_nodes, cell_xy).
+int build_mesh(tfa_mesh& m, cudaStream_t st) {
+  const int64_t nc = m.nc, nn = m.nn, ne = 3 * nc;
+  if (ne >= (int64_t)INT32_MAX) return set_error(TFA_EINVAL, "mesh too large for 32-bit face-edge ids");
+  DevBuf<int32_t> err;
+  TFA_CUDA(err.alloc(2));
+  {
+    int32_t h[2] = {0, INT32_MAX};
+    TFA_CUDA(cudaMemcpyAsync(err.p, h, sizeof(h), cudaMemcpyHostToDevice, st));
+  }
+  DevBuf<double> vol, olen, onrm, ooff;
+  TFA_CUDA(m.cen.alloc(2 * nc));
+  TFA_CUDA(vol.alloc(nc));
+  TFA_CUDA(olen.alloc(3 * nc));
+  TFA_CUDA(onrm.alloc(6 * nc));
+  TFA_CUDA(ooff.alloc(6 * nc));
+  if (nc == 0) {
+    m.nf = m.nnzb = m.nst = 0;
+    TFA_CUDA(m.st_ptr.alloc(1));
+    TFA_CUDA(m.bsr_rowptr.alloc(1));
+    TFA_CUDA(cudaMemsetAsync(m.st_ptr.p, 0, 4, st));
+    TFA_CUDA(cudaMemsetAsync(m.bsr_rowptr.p, 0, 4, st));
+    TFA_CUDA(m.face_nodes.alloc(0)); TFA_CUDA(m.face_cells.alloc(0)); TFA_CUDA(m.cell_faces.alloc(0));
+    TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
+    TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0));
+    ++m.generation;
+    return 0;
+  }
+  k_cell_geom<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, nn, m.cell_nodes.p, m.cell_xy.p, m.cen.p, vol.p, olen.p, onrm.p,
+                                            ooff.p, err.p);
+  TFA_TRY(check_err(err, st));
+
+  // faces
+  DevBuf<uint64_t> keys, keys_s;
+  DevBuf<int32_t> vals, vals_s, head, fid;
+  TFA_CUDA(keys.alloc(ne)); TFA_CUDA(keys_s.alloc(ne));
+  TFA_CUDA(vals.alloc(ne)); TFA_CUDA(vals_s.alloc(ne));
+  TFA_CUDA(head.alloc(ne)); TFA_CUDA(fid.alloc(ne));
+  k_edge_keys<<<cdiv(ne, TPB), TPB, 0, st>>>(nc, nn, m.cell_nodes.p, keys.p, vals.p);
+  {
+    int end_bit = 1;
+    while (end_bit < 64 && ((uint64_t)nn * (uint64_t)nn) >> end_bit) ++end_bit;
+    size_t tmp_bytes = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys.p, keys_s.p, vals.p, vals_s.p, (int)ne, 0, end_bit, st);
+    DevBuf<char> tmp;
+    TFA_CUDA(tmp.alloc((int64_t)tmp_bytes));
+    TFA_CUDA(cub::DeviceRadixSort::SortPairs(tmp.p, tmp_bytes, keys.p, keys_s.p, vals.p, vals_s.p, (int)ne, 0,
+                                             end_bit, st));
+    TFA_CUDA(cudaStreamSynchronize(st));
+  }
+  k_face_heads<<<cdiv(ne, TPB), TPB, 0, st>>>(ne, keys_s.p, head.p, err.p);
+  {
+    size_t tmp_bytes = 0;
+    cub::DeviceScan::InclusiveSum(nullptr, tmp_bytes, head.p, fid.p, (int)ne, st);
+    DevBuf<char> tmp;
+    TFA_CUDA(tmp.alloc((int64_t)tmp_bytes));
+    TFA_CUDA(cub::DeviceScan::InclusiveSum(tmp.p, tmp_bytes, head.p, fid.p, (int)ne, st));
+    int32_t nf = 0;
+    TFA_CUDA(cudaMemcpyAsync(&nf, fid.p + ne - 1, 4, cudaMemcpyDeviceToHost, st));
+    TFA_CUDA(cudaStreamSynchronize(st));
+    m.nf = nf;
+  }
+  TFA_TRY(check_err(err, st));
+  TFA_CUDA(m.face_nodes.alloc(2 * m.nf));
+  TFA_CUDA(m.face_cells.alloc(2 * m.nf));
+  TFA_CUDA(m.cell_faces.alloc(3 * nc));
+  TFA_CUDA(m.cell_nbr.alloc(3 * nc));
+  k_faces<<<cdiv(ne, TPB), TPB, 0, st>>>(ne, nn, keys_s.p, vals_s.p, fid.p, m.face_nodes.p, m.face_cells.p,
+                                        m.cell_faces.p, err.p);
+  DevBuf<int32_t> cnt;
+  TFA_CUDA(cnt.alloc(nc));
+  k_cell_nbr<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_faces.p, m.face_cells.p, m.cell_nbr.p, cnt.p, err.p);
+  TFA_TRY(check_err(err, st));
+
+  // BSR pattern
+  TFA_CUDA(m.bsr_rowptr.alloc(nc + 1));
+  TFA_TRY(exclusive_scan_with_total(cnt, nc, m.bsr_rowptr, &m.nnzb, st));
+  TFA_CUDA(m.bsr_col.alloc(m.nnzb));
+  k_bsr_cols<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.bsr_rowptr.p, m.bsr_col.p);
+
+  // vertex-neighbour stencil
+  {
+    DevBuf<uint32_t> nk, nk_s;
+    DevBuf<int32_t> node_cnt, node_ptr;
+    TFA_CUDA(nk.alloc(ne)); TFA_CUDA(nk_s.alloc(ne));
+    TFA_CUDA(node_cnt.alloc(nn)); TFA_CUDA(node_ptr.alloc(nn + 1));
+    TFA_CUDA(cudaMemsetAsync(node_cnt.p, 0, (size_t)nn * 4, st));
+    k_node_pairs<<<cdiv(ne, TPB), TPB, 0, st>>>(nc, m.cell_nodes.p, nk.p, vals.p, node_cnt.p);
+    int end_bit = 1;
+    while (end_bit < 32 && ((uint64_t)nn >> end_bit)) ++end_bit;
+    size_t tmp_bytes = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, nk.p, nk_s.p, vals.p, vals_s.p, (int)ne, 0, end_bit, st);
+    DevBuf<char> tmp;
+    TFA_CUDA(tmp.alloc((int64_t)tmp_bytes));
+    TFA_CUDA(cub::DeviceRadixSort::SortPairs(tmp.p, tmp_bytes, nk.p, nk_s.p, vals.p, vals_s.p, (int)ne, 0, end_bit,
+                                             st));
+    int64_t tot = 0;
+    TFA_TRY(exclusive_scan_with_total(node_cnt, nn, node_ptr, &tot, st));
+    k_stencil_count<<<cdiv(nc, 128), 128, 0, st>>>(nc, m.cell_nodes.p, node_ptr.p, vals_s.p, cnt.p, err.p);
+    TFA_TRY(check_err(err, st));
+    TFA_CUDA(m.st_ptr.alloc(nc + 1));
+    TFA_TRY(exclusive_scan_with_total(cnt, nc, m.st_ptr, &m.nst, st));
+    TFA_CUDA(m.st_idx.alloc(m.nst));
+    TFA_CUDA(m.st_d.alloc(2 * m.nst));
+    k_stencil_fill<<<cdiv(nc, 128), 128, 0, st>>>(nc, m.cell_nodes.p, node_ptr.p, vals_s.p, m.st_ptr.p, m.cell_xy.p,
+                                                 m.cen.p, m.st_idx.p, m.st_d.p);
+    TFA_CUDA(cudaStreamSynchronize(st));
+  }
+  TFA_CUDA(m.cgeo.alloc(CGEO * nc));
+  k_cgeo<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.cell_faces.p, vol.p, olen.p, onrm.p, ooff.p, m.cgeo.p);
+  TFA_CUDA(cudaGetLastError());
+  TFA_CUDA(cudaStreamSynchronize(st));
+  ++m.generation;
+  return 0;
+}
+
+}  // namespace tfa
+
+using namespace tfa;
+
+extern "C" {
+
+const char* tfa_last_error(void) { return tfa::g_last_error.c_str(); }
+const char* tfa_version(void) { return "tfa 0.1 (sm_100a)"; }
+
+int tfa_mesh_create(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                    const int32_t* cell_nodes, const double* cell_xy, void* stream) {
+  if (!out || n_nodes < 0 || n_cells < 0 || (n_cells > 0 && !cell_nodes) || (!node_xy && !cell_xy && n_cells > 0))
+    return set_error(TFA_EINVAL, "tfa_mesh_create: bad argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  tfa_mesh* m = new (std::nothrow) tfa_mesh;
+  if (!m) return set_error(TFA_ENOMEM, "host allocation failed");
+  m->nn = n_nodes;
+  m->nc = n_cells;
+  auto body = [&]() -> int {
+    TFA_CUDA(m->node_xy.alloc(2 * n_nodes));
+    TFA_CUDA(m->cell_nodes.alloc(3 * n_cells));
+    TFA_CUDA(m->cell_xy.alloc(6 * n_cells));
+    TFA_CUDA(m->perm.alloc(n_cells));
+    if (node_xy && n_nodes)
+      TFA_CUDA(cudaMemcpyAsync(m->node_xy.p, node_xy, (size_t)n_nodes * 16, cudaMemcpyHostToDevice, st));
+    if (n_cells) {
+      TFA_CUDA(cudaMemcpyAsync(m->cell_nodes.p, cell_nodes, (size_t)n_cells * 12, cudaMemcpyHostToDevice, st));
+      if (cell_xy) TFA_CUDA(cudaMemcpyAsync(m->cell_xy.p, cell_xy, (size_t)n_cells * 48, cudaMemcpyHostToDevice, st));
+      else {
+        DevBuf<int32_t> err;
+        TFA_CUDA(err.alloc(2));
+        TFA_CUDA(cudaMemsetAsync(err.p, 0, 8, st));
+        k_gather_xy<<<cdiv(3 * n_cells, TPB), TPB, 0, st>>>(3 * n_cells, n_nodes, m->cell_nodes.p, m->node_xy.p,
+                                                           m->cell_xy.p, err.p);
+        TFA_TRY(check_err(err, st));
+      }
+      k_iota<<<cdiv(n_cells, TPB), TPB, 0, st>>>(n_cells, m->perm.p);
+    }
+    return build_mesh(*m, st);
+  };
+  int rc = body();
+  if (rc) { delete m; return rc; }
+  *out = m;
+  return 0;
+}
+
+int tfa_mesh_reorder(tfa_mesh* m, int kind, const int32_t* user_perm, void* stream) {
+  if (!m) return set_error(TFA_EINVAL, "null mesh");
+  if (kind == 0 || m->nc == 0) return 0;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t nc = m->nc;
+  DevBuf<int32_t> p;
+  TFA_CUDA(p.alloc(nc));
+  if (kind == 1) {
+    DevBuf<int32_t> order, pos, parent;
+    TFA_CUDA(order.alloc(nc)); TFA_CUDA(pos.alloc(nc)); TFA_CUDA(parent.alloc(nc));
+    k_rcm<<<1, RCM_T, 0, st>>>((int32_t)nc, m->cell_nbr.p, order.p, pos.p, parent.p);
+    k_reverse<<<cdiv(nc, TPB), TPB, 0, st>>>((int32_t)nc, order.p, p.p);
+    TFA_CUDA(cudaGetLastError());
+    TFA_CUDA(cudaStreamSynchronize(st));
+  } else if (kind == 2) {
+    if (!user_perm) return set_error(TFA_EINVAL, "user permutation missing");
+    TFA_CUDA(cudaMemcpyAsync(p.p, user_perm, (size_t)nc * 4, cudaMemcpyHostToDevice, st));
+    DevBuf<int32_t> hit, err;
+    TFA_CUDA(hit.alloc(nc)); TFA_CUDA(err.alloc(2));
+    TFA_CUDA(cudaMemsetAsync(hit.p, 0, (size_t)nc * 4, st));
+    TFA_CUDA(cudaMemsetAsync(err.p, 0, 8, st));
+    k_check_perm<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, p.p, hit.p, err.p);
+    int rc = check_err(err, st);
+    if (rc) return set_error(TFA_EINVAL, tfa::g_last_error);
+  } else {
+    return set_error(TFA_EINVAL, "unknown reorder kind");
+  }
+  DevBuf<int32_t> cn, pm;
+  DevBuf<double> cx;
+  TFA_CUDA(cn.alloc(3 * nc)); TFA_CUDA(pm.alloc(nc)); TFA_CUDA(cx.alloc(6 * nc));
+  k_permute_cells<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, p.p, m->cell_nodes.p, m->cell_xy.p, m->perm.p, cn.p, cx.p, pm.p);
+  TFA_CUDA(cudaStreamSynchronize(st));
+  m->cell_nodes.swap(cn);
+  m->cell_xy.swap(cx);
+  m->perm.swap(pm);
+  return build_mesh(*m, st);
+}
+
+int tfa_mesh_sizes(const tfa_mesh* m, int64_t* n_cells, int64_t* n_faces, int64_t* nnzb, int64_t* n_stencil) {
+  if (!m) return set_error(TFA_EINVAL, "null mesh");
+  if (n_cells) *n_cells = m->nc;
+  if (n_faces) *n_faces = m->nf;
+  if (nnzb) *nnzb = m->nnzb;
+  if (n_stencil) *n_stencil = m->nst;
+  return 0;
+}
+
+static const void* item_ptr(const tfa_mesh* m, int which, int64_t* bytes) {
+  switch (which) {
+    case TFA_FACE_CELLS: *bytes = m->nf * 8; return m->face_cells.p;
+    case TFA_FACE_NODES: *bytes = m->nf * 8; return m->face_nodes.p;
+    case TFA_CELL_FACES: *bytes = m->nc * 12; return m->cell_faces.p;
+    case TFA_CELL_NBR: *bytes = m->nc * 12; return m->cell_nbr.p;
+    case TFA_STENCIL_PTR: *bytes = (m->nc + 1) * 4; return m->st_ptr.p;
+    case TFA_STENCIL_IDX: *bytes = m->nst * 4; return m->st_idx.p;
+    case TFA_BSR_ROWPTR: *bytes = (m->nc + 1) * 4; return m->bsr_rowptr.p;
+    case TFA_BSR_COL: *bytes = m->nnzb * 4; return m->bsr_col.p;
+    case TFA_PERM: *bytes = m->nc * 4; return m->perm.p;
+    case TFA_CENTROID: *bytes = m->nc * 16; return m->cen.p;
+    default: return nullptr;
+  }
+}
+
+int tfa_mesh_get(const tfa_mesh* m, int which, void* host_dst, int64_t bytes) {
+  if (!m || !host_dst) return set_error(TFA_EINVAL, "null argument");
+  int64_t need = 0;
+  if (which == TFA_VOLUME || which == TFA_FACE_NORMAL_LEN) {
+    const int64_t n = which == TFA_VOLUME ? m->nc : 3 * m->nf;
+    if (bytes != n * 8) return set_error(TFA_EINVAL, "tfa_mesh_get: size mismatch, need " + std::to_string(n * 8));
+    if (n == 0) return 0;
+    DevBuf<double> tmp;
+    TFA_CUDA(tmp.alloc(n));
+    if (which == TFA_VOLUME) k_volume_out<<<cdiv(m->nc, TPB), TPB>>>(m->nc, m->cgeo.p, tmp.p);
+    else k_face_geom_out<<<cdiv(m->nf, TPB), TPB>>>(m->nf, m->face_cells.p, m->cell_faces.p, m->cgeo.p, tmp.p);
+    TFA_CUDA(cudaMemcpy(host_dst, tmp.p, (size_t)n * 8, cudaMemcpyDeviceToHost));
+    return 0;
+  }
+  const void* src = item_ptr(m, which, &need);
+  if (!src) return set_error(TFA_EINVAL, "tfa_mesh_get: unknown item");
+  if (bytes != need) return set_error(TFA_EINVAL, "tfa_mesh_get: size mismatch, need " + std::to_string(need));
+  if (need) TFA_CUDA(cudaMemcpy(host_dst, src, (size_t)need, cudaMemcpyDeviceToHost));
+  return 0;
+}
+
+const void* tfa_mesh_device_ptr(const tfa_mesh* m, int which) {
+  if (!m) return nullptr;
+  int64_t b = 0;
+  return item_ptr(m, which, &b);
+}
+
+void tfa_mesh_destroy(tfa_mesh* m) { delete m; }
+
+}  // extern "C"

@@ -1,0 +1,325 @@
+"""GPU parity tests: libtfa (through the C ABI binding) against the CPU oracle, element by element.
+
+Tolerances are north_star's, read as in DESIGN.md (S18): residual 1e-12 of the per-variable
+sum-of-|terms| scale; Jacobian 1e-8 of the row-maximum magnitude; connectivity bit-exact.
+"""
+import numpy as np
+import pytest
+
+from conftest import random_state
+from helpers import (RES_TOL, JAC_TOL, residual_error, jacobian_error_rows, bsr_to_rows,
+                     check_connectivity_against_brute)
+
+pytestmark = pytest.mark.gpu
+
+INT_ITEMS = ["face_nodes", "face_cells", "cell_faces", "stencil_ptr", "stencil_idx", "bsr_rowptr", "bsr_col", "perm"]
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_1809_02532_b200 import build, api
+    build.build()
+    return api
+
+
+def dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def small_meshes(W):
+    return {
+        "c1": W.make_workload("c1").mesh,
+        "periodic7x5": W.split_quad_mesh(7, 5),
+        "channel": W.split_quad_mesh(9, 6, *W.GEM_DOMAIN, periodic_x=True, periodic_y=False),
+        "box": W.split_quad_mesh(5, 4, periodic_x=False, periodic_y=False),
+        "delaunay": W.delaunay_mesh(23, 17, *W.GEM_DOMAIN, jitter=0.3, seed=4, shuffle_cells=True),
+    }
+
+
+# ------------------------------------------------------------------------------------------
+# a1: connectivity, geometry, reordering
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c1", "periodic7x5", "channel", "box", "delaunay"])
+def test_connectivity_bit_exact(api, orc, W, name):
+    mi = small_meshes(W)[name]
+    g = api.Mesh.from_input(mi)
+    o = orc.OracleMesh.from_input(mi)
+    assert (g.n_cells, g.n_faces, g.nnzb, g.n_stencil) == (o.n_cells, o.n_faces, o.nnzb, o.n_stencil)
+    for item in INT_ITEMS:
+        np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
+    check_connectivity_against_brute(g.get, (g.n_cells, g.n_faces, g.nnzb, g.n_stencil), mi.cell_nodes)
+    # neighbour table is consistent with the face table
+    nbr, cf, fc = g.get("cell_nbr"), g.get("cell_faces"), g.get("face_cells")
+    for c in range(0, g.n_cells, 5):
+        for k in range(3):
+            L, R = fc[cf[c, k]]
+            assert nbr[c, k] == (R if L == c else L)
+    for item in ("volume", "centroid", "face_normal_len"):
+        np.testing.assert_allclose(g.get(item), o.get(item), rtol=1e-14, atol=1e-15, err_msg=item)
+    assert g.device_ptr("bsr_col") != 0 and g.device_ptr("bsr_rowptr") != 0
+
+
+@pytest.mark.parametrize("name", ["c1", "channel", "delaunay"])
+def test_rcm_bit_exact(api, orc, W, name):
+    mi = small_meshes(W)[name]
+    g = api.Mesh.from_input(mi)
+    o = orc.OracleMesh.from_input(mi)
+    g.reorder("rcm")
+    o.reorder("rcm")
+    for item in INT_ITEMS:
+        np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
+    perm = g.get("perm")
+    assert sorted(perm.tolist()) == list(range(g.n_cells))
+    # a second, user-given permutation composes with the first
+    rng = np.random.default_rng(0)
+    p2 = rng.permutation(g.n_cells).astype(np.int32)
+    g.reorder("user", p2)
+    o.reorder("user", p2)
+    np.testing.assert_array_equal(g.get("perm"), perm[p2])
+    for item in INT_ITEMS:
+        np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
+
+
+def test_rcm_disconnected_components(api, orc, W):
+    """Two meshes glued into one node/cell list: RCM restarts at the min-(degree, id) unvisited cell."""
+    a = W.split_quad_mesh(4, 3, periodic_x=False, periodic_y=False)
+    b = W.delaunay_mesh(6, 5, *W.GEM_DOMAIN, jitter=0.3, seed=9)
+    nodes = np.concatenate([a.node_xy, b.node_xy + 100.0])
+    cells = np.concatenate([a.cell_nodes, b.cell_nodes + a.n_nodes]).astype(np.int32)
+    rng = np.random.default_rng(3)
+    cells = cells[rng.permutation(len(cells))]
+    g = api.Mesh(nodes, cells)
+    o = orc.OracleMesh(nodes, cells)
+    g.reorder("rcm")
+    o.reorder("rcm")
+    for item in INT_ITEMS:
+        np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
+
+
+def test_mesh_errors_and_degenerate_sizes(api, W):
+    mi = W.split_quad_mesh(3, 3, periodic_x=False, periodic_y=False)
+    bad = mi.cell_nodes.copy()
+    bad[4] = bad[4][::-1]
+    with pytest.raises(api.TfaError) as e:
+        api.Mesh(mi.node_xy, bad)
+    assert e.value.code == -2 and "counter-clockwise" in str(e.value)
+    with pytest.raises(api.TfaError) as e:
+        api.Mesh.from_input(W.split_quad_mesh(2, 4))       # periodic direction 2 cells wide
+    assert e.value.code == -2
+    dup = np.concatenate([mi.cell_nodes, mi.cell_nodes[:1]])   # a node pair shared by 3 cells
+    with pytest.raises(api.TfaError):
+        api.Mesh(mi.node_xy, dup)
+    g = api.Mesh.from_input(mi)
+    with pytest.raises(api.TfaError) as e:
+        g.reorder("user", np.zeros(g.n_cells, dtype=np.int32))
+    assert e.value.code == -1
+    # empty mesh and single triangle
+    e0 = api.Mesh(np.zeros((0, 2)), np.zeros((0, 3), dtype=np.int32))
+    assert (e0.n_cells, e0.n_faces, e0.nnzb) == (0, 0, 0)
+    one = api.Mesh(np.array([[0.0, 0], [1, 0], [0, 1]]), np.array([[0, 1, 2]], dtype=np.int32))
+    assert (one.n_cells, one.n_faces, one.nnzb, one.n_stencil) == (1, 3, 1, 0)
+    ctx = api.Context()
+    import torch
+    P = dev(random_state(np.random.default_rng(0), 1))
+    rhs, vals = ctx.assemble(one, P)
+    torch.cuda.synchronize()
+    assert np.isfinite(rhs.cpu().numpy()).all() and vals.shape == (1, 18, 18)
+    rhs0, vals0 = ctx.assemble(e0, dev(np.zeros((0, 18))))
+    assert rhs0.shape == (0, 18)
+
+
+# ------------------------------------------------------------------------------------------
+# a2: gradient + limiter
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c1", "channel", "delaunay"])
+@pytest.mark.parametrize("K,p", [(1.0, 2.0), (0.3, 1.0)])
+def test_gradients_parity(api, orc, W, name, K, p):
+    mi = small_meshes(W)[name]
+    g, o = api.Mesh.from_input(mi), orc.OracleMesh.from_input(mi)
+    rng = np.random.default_rng(5)
+    P = random_state(rng, g.n_cells)
+    ctx = api.Context(numerics=api.default_numerics(venkat_K=K, lsq_weight_power=p))
+    grad, phi = ctx.gradients(g, dev(P))
+    go, po = orc.gradients(o, orc.default_numerics(venkat_K=K, lsq_weight_power=p), P)
+    h = np.sqrt(o.get("volume")).min()
+    np.testing.assert_allclose(grad.cpu().numpy(), go, rtol=0, atol=1e-12 * np.abs(go).max())
+    np.testing.assert_allclose(phi.cpu().numpy(), po, rtol=0, atol=1e-11)
+    assert h > 0
+
+
+# ------------------------------------------------------------------------------------------
+# a3..a7: residual + Jacobian
+# ------------------------------------------------------------------------------------------
+def compare_assembly(api, orc, mi, P, Pn=None, Pnm1=None, dt=1e-3, physics=None, numerics_kw=None,
+                     reorder=None, rows=None):
+    numerics_kw = numerics_kw or {}
+    g, o = api.Mesh.from_input(mi), orc.OracleMesh.from_input(mi)
+    if reorder:
+        g.reorder(reorder)
+        o.reorder(reorder)
+        perm = g.get("perm")
+        np.testing.assert_array_equal(perm, o.get("perm"))
+        P = P[perm]
+        Pn = None if Pn is None else Pn[perm]
+        Pnm1 = None if Pnm1 is None else Pnm1[perm]
+    ph_g = api.default_physics(physics)
+    ctx = api.Context(ph_g, api.default_numerics(ph_g, **numerics_kw))
+    ph_o = orc.physics_c(physics)
+    nu_o = orc.default_numerics(ph_o, **numerics_kw)
+    rhs, vals = ctx.assemble(g, dev(P), None if Pn is None else dev(Pn), None if Pnm1 is None else dev(Pnm1), dt)
+    ctx.check()
+    rhs, vals = rhs.cpu().numpy(), vals.cpu().numpy()
+    rhs_o, scale_o, vals_o = orc.assemble(o, ph_o, nu_o, P, Pn, Pnm1, dt, rows=rows)
+    rp = g.get("bsr_rowptr")
+    if rows is None:
+        er = residual_error(rhs, rhs_o, scale_o)
+        ej = jacobian_error_rows(bsr_to_rows(vals, rp), bsr_to_rows(vals_o, rp))
+    else:
+        # per-variable scale from the sampled rows
+        er = residual_error(rhs[rows], rhs_o, scale_o)
+        ej = jacobian_error_rows(bsr_to_rows(vals, rp, rows), vals_o)
+    return er, ej, (rhs, vals, rhs_o, vals_o)
+
+
+@pytest.mark.parametrize("name", ["c1", "periodic7x5", "channel", "box", "delaunay"])
+def test_assembly_parity_small(api, orc, W, name):
+    mi = small_meshes(W)[name]
+    cen = mi.centroids()
+    if name in ("c1", "periodic7x5"):
+        P = W.wave_state(cen, seed=0)
+    else:
+        P = W.gem_state(cen) + np.random.default_rng(1).uniform(-1e-3, 1e-3, (mi.n_cells, 18))
+    Pn = W.perturb(P, 11, 1e-4)
+    Pnm1 = W.perturb(P, 12, 1e-4)
+    er, ej, _ = compare_assembly(api, orc, mi, P, Pn, Pnm1)
+    assert er < RES_TOL, er
+    assert ej < JAC_TOL, ej
+
+
+def test_config1_exact_recipe(api, orc, W):
+    """BASELINE config 1: 512 cells, seed 0, P^n = P^{n-1} = P, dt = 1e-3, one assembly."""
+    w = W.make_workload("c1")
+    assert w.mesh.n_cells == 512
+    er, ej, (rhs, vals, rhs_o, vals_o) = compare_assembly(api, orc, w.mesh, w.state, dt=w.dt, physics=w.physics)
+    assert er < RES_TOL, er
+    assert ej < JAC_TOL, ej
+    # structural zeros of the off-diagonal blocks are exact zeros on the GPU as well
+    grp = np.array([0] * 8 + [1, 2] + [1] * 3 + [2] * 3 + [1, 2])
+    coupled = grp[:, None] == grp[None, :]
+    g = api.Mesh.from_input(w.mesh)
+    rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
+    rows = np.repeat(np.arange(g.n_cells), np.diff(rp))
+    offd = rows != col
+    assert (vals[offd][:, ~coupled] == 0.0).all() and (vals_o[offd][:, ~coupled] == 0.0).all()
+
+
+@pytest.mark.parametrize("mask", [1, 2, 4, 3, 5, 6])
+def test_term_masks(api, orc, W, mask):
+    mi = small_meshes(W)["delaunay"]
+    P = W.gem_state(mi.centroids()) + np.random.default_rng(2).uniform(-1e-3, 1e-3, (mi.n_cells, 18))
+    er, ej, _ = compare_assembly(api, orc, mi, P, W.perturb(P, 1, 1e-3), W.perturb(P, 2, 1e-3),
+                                 numerics_kw=dict(term_mask=mask))
+    assert er < RES_TOL and ej < JAC_TOL, (er, ej)
+
+
+def test_other_constants(api, orc, W):
+    """Non-default physics and numerics reach the kernels (cleaning speeds, alpha, AUSM constants, delta)."""
+    mi = small_meshes(W)["channel"]
+    P = W.gem_state(mi.centroids()) + np.random.default_rng(3).uniform(-1e-2, 1e-2, (mi.n_cells, 18))
+    ph = W.Physics(gamma_gas=1.4, mass_ratio=100.0, c=10.0, gamma_psi=1.3, chi_phi=0.7, rusanov_alpha=0.4)
+    P[:, 9] = P[:, 8] / 100.0
+    kw = dict(fd_delta=1e-5, venkat_K=0.5, lsq_weight_power=1.0, ausm_Kp=0.3, ausm_Ku=0.6, ausm_sigma=0.9,
+              ausm_beta=0.1, ausm_Minf=[0.2, 0.05])
+    er, ej, _ = compare_assembly(api, orc, mi, P, dt=2e-3, physics=ph, numerics_kw=kw)
+    assert er < RES_TOL and ej < JAC_TOL, (er, ej)
+
+
+def test_supersonic_and_upwind_branches(api, orc, W):
+    """States with |M| > 1 and both flow directions exercise the other branches of the AUSM splits."""
+    mi = small_meshes(W)["periodic7x5"]
+    rng = np.random.default_rng(6)
+    P = random_state(rng, mi.n_cells, vel=2.5)
+    er, ej, _ = compare_assembly(api, orc, mi, P)
+    assert er < RES_TOL and ej < JAC_TOL, (er, ej)
+
+
+def test_reordered_assembly(api, orc, W):
+    mi = small_meshes(W)["delaunay"]
+    P = W.gem_state(mi.centroids()) + np.random.default_rng(4).uniform(-1e-3, 1e-3, (mi.n_cells, 18))
+    er, ej, _ = compare_assembly(api, orc, mi, P, reorder="rcm")
+    assert er < RES_TOL and ej < JAC_TOL, (er, ej)
+
+
+def test_run_to_run_determinism_and_no_memset_needed(api, W):
+    """S21: two assemblies of the same input are bit-identical, whatever the output held before."""
+    import torch
+    mi = small_meshes(W)["delaunay"]
+    g = api.Mesh.from_input(mi)
+    ctx = api.Context()
+    P = dev(W.gem_state(mi.centroids()))
+    rhs1 = torch.full((g.n_cells, 18), float("nan"), dtype=torch.float64, device="cuda")
+    vals1 = torch.full((g.nnzb, 18, 18), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.assemble(g, P, rhs=rhs1, vals=vals1)
+    rhs2 = torch.full((g.n_cells, 18), 7.0, dtype=torch.float64, device="cuda")
+    vals2 = torch.full((g.nnzb, 18, 18), 7.0, dtype=torch.float64, device="cuda")
+    ctx.assemble(g, P, rhs=rhs2, vals=vals2)
+    torch.cuda.synchronize()
+    assert torch.equal(rhs1, rhs2) and torch.equal(vals1, vals2)
+    assert torch.isfinite(vals1).all()
+    # residual-only evaluation gives the same rhs
+    rhs3, none = ctx.assemble(g, P, jacobian=False)
+    assert none is None and torch.equal(rhs1, rhs3)
+    assert ctx.launches_per_assemble == 2
+
+
+def test_host_entry_point_matches_device_entry_point(api, W):
+    import torch
+    mi = small_meshes(W)["channel"]
+    g = api.Mesh.from_input(mi)
+    ctx = api.Context()
+    P = W.gem_state(mi.centroids())
+    Pn = W.perturb(P, 1, 1e-3)
+    rhs_d, vals_d = ctx.assemble(g, dev(P), dev(Pn), dev(Pn), 1e-3)
+    rhs_h = torch.empty((g.n_cells, 18), dtype=torch.float64).pin_memory()
+    vals_h = torch.empty((g.nnzb, 18, 18), dtype=torch.float64).pin_memory()
+    ctx.assemble_host(g, P, Pn, Pn, 1e-3, rhs_h, vals_h)
+    assert torch.equal(rhs_h, rhs_d.cpu()) and torch.equal(vals_h, vals_d.cpu())
+
+
+def test_nonphysical_state_is_reported(api, W):
+    mi = small_meshes(W)["box"]
+    g = api.Mesh.from_input(mi)
+    ctx = api.Context()
+    P = W.gem_state(mi.centroids())
+    P[3, 16] = -1.0
+    ctx.assemble(g, dev(P))
+    with pytest.raises(api.TfaError) as e:
+        ctx.check()
+    assert e.value.code == -5
+    ctx.assemble(g, dev(W.gem_state(mi.centroids())))
+    ctx.check()     # the flag was cleared
+
+
+def test_config2_first_and_last_of_ten_calls(api, orc, W):
+    """BASELINE config 2 at a size the oracle finishes in seconds (64x64 quads = 8192 cells):
+    10 consecutive assemblies with the state perturbed by 1e-6 between calls; parity on 1st and 10th."""
+    w = W.make_workload("c2", scale=0.25)
+    g, o = api.Mesh.from_input(w.mesh), orc.OracleMesh.from_input(w.mesh)
+    ctx = api.Context(w.physics)
+    ph_o = orc.physics_c(w.physics)
+    nu_o = orc.default_numerics(ph_o)
+    rp = g.get("bsr_rowptr")
+    P_prev2 = P_prev = P = w.state
+    for call in range(10):
+        rhs, vals = ctx.assemble(g, dev(P), dev(P_prev), dev(P_prev2), w.dt)
+        if call in (0, 9):
+            rhs_o, sc_o, vals_o = orc.assemble(o, ph_o, nu_o, P, P_prev, P_prev2, w.dt)
+            er = residual_error(rhs.cpu().numpy(), rhs_o, sc_o)
+            ej = jacobian_error_rows(bsr_to_rows(vals.cpu().numpy(), rp), bsr_to_rows(vals_o, rp))
+            assert er < RES_TOL and ej < JAC_TOL, (call, er, ej)
+        P_prev2, P_prev, P = P_prev, P, W.perturb(P, 100 + call, 1e-6)
+    ctx.check()
