@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the residual + BSR-Jacobian assembly (BASELINE.json metric).
+
+    python bench.py --gpus 1 --steps 10 --warmup 3             # this repo's CUDA path
+    python bench.py --impl reference --steps 3 --warmup 1      # the CPU oracle, timed as it stands
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N   # N replicas
+
+A "step" is one whole assembly (gradient + limiter kernel, then the fused flux / Jacobian /
+source / BDF2 / BSR-write kernel) of one synthetic batch.  Default workload: BASELINE config 4,
+run B — GEM Harris sheet on a 1,000,000-cell jittered Delaunay mesh, reverse-Cuthill-McKee order.
+Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "residual+BSR-Jacobian assembly throughput"
+UNIT = "Mcells/s"
+
+
+# --------------------------------------------------------------------------------------------
+def algorithmic_bytes(nc: int, nnzb: int, nst: int):
+    """compulsory HBM bytes per launch of each kernel."""
+    asm = (nnzb * 18 * 18 * 8      # BSR Jacobian blocks written once
+           + nc * 144 * 3          # state, state_n, state_nm1 read
+           + nc * 144              # rhs written
+           + nc * 288              # limited gradient read
+           + nc * 192              # per-cell geometry record
+           + nc * 12 + nc * 4)     # neighbour table, row pointers
+    grad = (nc * 144 + nst * 4 + nst * 16 + nc * 4 + nc * 192 + nc * 288)
+    return asm, grad
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons, pw = [], [], set(), []
+        for t, line in self.rows:
+            if not (t0 - 0.05 <= t <= t1 + 0.15):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:   # region shorter than the sampling period: take everything we saw
+            for _, line in self.rows:
+                f = [x.strip() for x in line.split(",")]
+                try:
+                    sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+                except Exception:
+                    pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (driver-measured copy bandwidth)"
+    return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md; MEASURED_PEAKS.json absent)"
+
+
+def ncu_traffic(workload: str):
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(workload, {}).get("k_assemble_dram_bytes_per_launch")
+    return None
+
+
+# --------------------------------------------------------------------------------------------
+def oracle_sample(wl, n_rows: int, steps: int, warmup: int):
+    """Time the oracle as it stands on a row sample of the workload (host cores of this box)."""
+    import oracle
+    oracle.build()
+    om = oracle.OracleMesh.from_input(wl.mesh)
+    state = wl.state
+    if wl.reorder == "rcm":
+        om.reorder("rcm")
+        state = np.ascontiguousarray(state[om.get("perm")])
+    ph = oracle.physics_c(wl.physics)
+    nu = oracle.default_numerics(ph)
+    rng = np.random.default_rng(12345)
+    n_rows = min(n_rows, om.n_cells)
+    rows = np.sort(rng.choice(om.n_cells, size=n_rows, replace=False)).astype(np.int32)
+    times = []
+    for it in range(warmup + steps):
+        t = time.perf_counter()
+        oracle.assemble(om, ph, nu, state, dt=wl.dt, rows=rows)
+        if it >= warmup:
+            times.append(time.perf_counter() - t)
+    sec = float(np.mean(times))
+    return {"value": n_rows / sec / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{n_rows} random rows of {om.n_cells} (gradients of the rows and their neighbours "
+                      f"included), mean of {steps} runs, {sec:.2f} s each"}, sec
+
+
+def run_reference(args, wl):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb, sec = oracle_sample(wl, args.cpu_rows, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl_description(args.workload, wl), "sample_rows": min(args.cpu_rows, wl.mesh.n_cells)},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def wl_description(name, wl):
+    desc = {"c1": "config 1: wave, 16x16 split quads, periodic",
+            "c2": "config 2: wave, 256x256 split quads, periodic",
+            "c3": "config 3: GEM, 512x256 split quads, periodic-x",
+            "c4a": "config 4 run A: GEM, 1M-cell jittered Delaunay, random cell order",
+            "c4b": "config 4 run B: GEM, 1M-cell jittered Delaunay, reverse Cuthill-McKee order",
+            "c5": "config 5: GEM, 4M-cell jittered Delaunay, RCM order"}[name]
+    return f"{desc} ({wl.mesh.n_cells} cells)"
+
+
+# --------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4b", choices=["c1", "c2", "c3", "c4a", "c4b", "c5"])
+    ap.add_argument("--scale", type=float, default=1.0, help="linear lattice scale (tests only)")
+    ap.add_argument("--cpu-rows", type=int, default=200000, help="rows of the oracle's timed sample")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = max(args.warmup, 1)
+
+    from paper_1809_02532_b200 import workloads as W
+    t_gen = time.time()
+    wl = W.make_workload(args.workload, scale=args.scale)
+    t_gen = time.time() - t_gen
+    if args.impl == "reference":
+        return run_reference(args, wl)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1809_02532_b200 import api, build
+    build.build()
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- setup (step a1; timed separately, once per mesh) ----
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    e0, e1, e2 = ev(), ev(), ev()
+    e0.record()
+    mesh = api.Mesh.from_input(wl.mesh)
+    e1.record()
+    if wl.reorder == "rcm":
+        mesh.reorder("rcm")
+    e2.record()
+    torch.cuda.synchronize()
+    setup_ms = {"mesh_create_ms": e0.elapsed_time(e1), "reorder_ms": e1.elapsed_time(e2), "generate_s": t_gen}
+    perm = mesh.get("perm")
+    state_h = np.ascontiguousarray(wl.state[perm])
+    nc, nnzb, nst = mesh.n_cells, mesh.nnzb, mesh.n_stencil
+    ctx = api.Context(wl.physics)
+    P = torch.from_numpy(state_h).cuda()
+    Pn, Pnm1 = P.clone(), P.clone()
+    rhs = torch.empty((nc, 18), dtype=torch.float64, device="cuda")
+    vals = torch.empty((nnzb, 18, 18), dtype=torch.float64, device="cuda")
+    noise = torch.empty_like(P)
+    gen = torch.Generator(device="cuda").manual_seed(1000 + rank)
+
+    def perturb():   # BASELINE config 2: seeded noise of 1e-6 between calls (outside the timed kernels)
+        noise.uniform_(-1e-6, 1e-6, generator=gen)
+        P.add_(noise)
+
+    # ---- probes: FP64 FMA peak and copy bandwidth in this run ----
+    sink = torch.zeros(8, dtype=torch.float64, device="cuda")
+    flops = api.probe_dfma(148 * 8, 1 << 14, sink)
+    torch.cuda.synchronize()
+    best = 1e9
+    for _ in range(3):
+        a, b = ev(), ev()
+        a.record(); flops = api.probe_dfma(148 * 8, 1 << 14, sink); b.record(); torch.cuda.synchronize()
+        best = min(best, a.elapsed_time(b))
+    fp64_tflops = flops / (best * 1e-3) / 1e12
+    src = torch.empty(1 << 27, dtype=torch.float64, device="cuda").normal_()
+    dst = torch.empty_like(src)
+    best = 1e9
+    for _ in range(4):
+        a, b = ev(), ev()
+        a.record(); nbytes = api.probe_copy(src, dst); b.record(); torch.cuda.synchronize()
+        best = min(best, a.elapsed_time(b))
+    copy_gbs = nbytes / (best * 1e-3) / 1e9
+    del src, dst
+
+    # ---- device-resident timing ----
+    for _ in range(max(args.warmup, 3)):
+        perturb()
+        ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
+    ctx.check()
+    ctx.timing_enable(True)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t0 = time.time()
+    start, end = ev(), ev()
+    start.record()
+    for _ in range(args.steps):
+        ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
+    end.record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    total_ms = start.elapsed_time(end)
+    ms_grad, ms_asm, ncalls = ctx.timing_read()
+    ctx.timing_enable(False)
+    ctx.check()
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * nc * args.steps / (total_ms * 1e-3) / 1e6
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        k_e2e = max(1, min(args.steps, 3))
+        sh = [torch.from_numpy(state_h).pin_memory() for _ in range(3)]
+        rhs_h = torch.empty((nc, 18), dtype=torch.float64).pin_memory()
+        vals_h = torch.empty((nnzb, 18, 18), dtype=torch.float64).pin_memory()
+        ctx.assemble_host(mesh, sh[0], sh[1], sh[2], wl.dt, rhs_h, vals_h)   # warm-up (allocates staging)
+        barrier()
+        tt = time.perf_counter()
+        for _ in range(k_e2e):
+            ctx.assemble_host(mesh, sh[0], sh[1], sh[2], wl.dt, rhs_h, vals_h)
+        torch.cuda.synchronize()
+        sec = (time.perf_counter() - tt)
+        if world > 1:
+            t = torch.tensor([sec], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sec = float(t.item())
+        e2e = {"value": world * nc * k_e2e / sec / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": 3 * nc * 144, "d2h_bytes_per_step": nc * 144 + nnzb * 2592,
+               "steps": k_e2e, "ms_per_step": sec / k_e2e * 1e3,
+               "note": "tfa_assemble_host: pinned host buffers, H2D of 3 states and D2H of rhs + BSR values inside"}
+        del sh, rhs_h, vals_h
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_assemble) ----
+    asm_bytes, grad_bytes = algorithmic_bytes(nc, nnzb, nst)
+    peak, peak_src = measured_peaks()
+    asm_ms = ms_asm / max(ncalls, 1)
+    grad_ms = ms_grad / max(ncalls, 1)
+    achieved = asm_bytes / (asm_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_assemble<true>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": ncu_traffic(args.workload),
+                "algorithmic_bytes_per_launch": asm_bytes, "kernel_ms": asm_ms, "peak_source": peak_src,
+                "kernel_share_of_step": asm_ms / ms_per_step,
+                "copy_probe_gbs_this_run": copy_gbs, "fp64_probe_tflops_this_run": fp64_tflops,
+                "gradient_kernel": {"ms": grad_ms, "algorithmic_bytes_per_launch": grad_bytes,
+                                    "achieved_gbs": grad_bytes / (grad_ms * 1e-3) / 1e9},
+                "step_frac_of_hbm_roofline": ((asm_bytes + grad_bytes) / (ms_per_step * 1e-3) / 1e9) / peak}
+
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        cpu_baseline, _ = oracle_sample(wl, args.cpu_rows, 1, 0)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl_description(args.workload, wl), "n_cells": nc, "nnzb": nnzb,
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs+outputs per step (%.1f GB) exceed the 126 MB L2; no flush needed" %
+                             ((asm_bytes + grad_bytes) / 1e9),
+                       "dt": wl.dt, "reorder": wl.reorder},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": ctx.launches_per_assemble * args.steps,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "setup": setup_ms}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

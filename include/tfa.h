@@ -141,6 +141,15 @@ int tfa_check(tfa_ctx* ctx, void* stream);
 int tfa_probe_dfma(int grid, int iters, double* sink, void* stream);
 int tfa_probe_copy(const double* src, double* dst, int64_t n, void* stream);
 
+/* Per-kernel timing with CUDA events recorded on the launching stream (bench.py's roofline).
+ * tfa_timing_enable(ctx, 1): every later tfa_assemble records events before, between and after
+ * its two kernels and accumulates their durations at the next tfa_timing_read, which
+ * synchronises on the last event, writes the accumulated milliseconds since the previous read
+ * to ms[0] (gradient + limiter kernel) and ms[1] (assembly kernel), the number of assemblies
+ * to *n_calls, and resets the accumulators.  At most 64 assemblies may be outstanding. */
+int tfa_timing_enable(tfa_ctx* ctx, int on);
+int tfa_timing_read(tfa_ctx* ctx, double* ms /*[2]*/, int* n_calls);
+
 /* Number of kernels the last tfa_assemble launched (for bench.py's gpu_launches). */
 int tfa_launches_per_assemble(const tfa_ctx* ctx);
 const char* tfa_last_error(void);

@@ -168,6 +168,16 @@ class Context:
     def check(self):
         _lib.check(_lib.load().tfa_check(self._h, _stream()))
 
+    def timing_enable(self, on: bool = True):
+        _lib.check(_lib.load().tfa_timing_enable(self._h, int(on)))
+
+    def timing_read(self):
+        """(ms_gradient_kernel, ms_assembly_kernel, n_calls) accumulated since the last read."""
+        ms = (C.c_double * 2)()
+        n = C.c_int()
+        _lib.check(_lib.load().tfa_timing_read(self._h, ms, C.byref(n)))
+        return float(ms[0]), float(ms[1]), int(n.value)
+
     @property
     def launches_per_assemble(self) -> int:
         return int(_lib.load().tfa_launches_per_assemble(self._h))

@@ -115,9 +115,22 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
   cudaStream_t st = (cudaStream_t)stream;
   TFA_TRY(prepare(ctx, m, st));
   const Consts K = make_consts(ctx->ph, ctx->nu);
+  cudaEvent_t* ev = nullptr;
+  if (ctx->timing) {
+    if (ctx->timed >= tfa_ctx::kMaxTimed) return set_error(TFA_EINVAL, "tfa_timing_read must be called every 64 assemblies");
+    ev = ctx->ev[ctx->timed];
+    for (int q = 0; q < 3; ++q)
+      if (!ev[q]) TFA_CUDA(cudaEventCreate(&ev[q]));
+    TFA_CUDA(cudaEventRecord(ev[0], st));
+  }
   TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->lgrad.p, nullptr, nullptr, st));
+  if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
   TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->lgrad.p, rhs, bsr_vals, ctx->flags.p, st));
-  ctx->launches = m->nc ? 2 : 0;
+  if (ev) {
+    TFA_CUDA(cudaEventRecord(ev[2], st));
+    ++ctx->timed;
+  }
+  ctx->launches = 2;
   return 0;
 }
 
@@ -168,6 +181,29 @@ int tfa_probe_dfma(int grid, int iters, double* sink, void* stream) {
 int tfa_probe_copy(const double* src, double* dst, int64_t n, void* stream) {
   if (!src || !dst || n <= 0 || (n & 1)) return set_error(TFA_EINVAL, "bad argument (n must be even)");
   return launch_probe_copy(src, dst, n, (cudaStream_t)stream);
+}
+
+int tfa_timing_enable(tfa_ctx* ctx, int on) {
+  if (!ctx) return set_error(TFA_EINVAL, "null argument");
+  ctx->timing = on != 0;
+  ctx->timed = 0;
+  return 0;
+}
+
+int tfa_timing_read(tfa_ctx* ctx, double* ms, int* n_calls) {
+  if (!ctx || !ms || !n_calls) return set_error(TFA_EINVAL, "null argument");
+  ms[0] = ms[1] = 0.0;
+  *n_calls = ctx->timed;
+  for (int q = 0; q < ctx->timed; ++q) {
+    TFA_CUDA(cudaEventSynchronize(ctx->ev[q][2]));
+    float a = 0.f, b = 0.f;
+    TFA_CUDA(cudaEventElapsedTime(&a, ctx->ev[q][0], ctx->ev[q][1]));
+    TFA_CUDA(cudaEventElapsedTime(&b, ctx->ev[q][1], ctx->ev[q][2]));
+    ms[0] += a;
+    ms[1] += b;
+  }
+  ctx->timed = 0;
+  return 0;
 }
 
 int tfa_launches_per_assemble(const tfa_ctx* ctx) { return ctx ? ctx->launches : 0; }

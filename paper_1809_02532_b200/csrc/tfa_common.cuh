@@ -97,4 +97,14 @@ struct tfa_ctx {
   // staging for tfa_assemble_host
   tfa::DevBuf<double> h_state[3], h_rhs, h_vals;
   int launches = 0;
+  // optional per-kernel timing (tfa_timing_enable): a ring of event triples
+  static constexpr int kMaxTimed = 64;
+  bool timing = false;
+  int timed = 0;
+  cudaEvent_t ev[kMaxTimed][3] = {};
+  ~tfa_ctx() {
+    for (auto& t : ev)
+      for (auto& e : t)
+        if (e) cudaEventDestroy(e);
+  }
 };
