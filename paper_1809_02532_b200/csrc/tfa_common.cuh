@@ -80,6 +80,7 @@ struct tfa_mesh {
   tfa::DevBuf<int32_t> st_ptr, st_idx;          // CSR stencil
   tfa::DevBuf<double> st_d;                     // [nst][2] centroid displacement (S9)
   tfa::DevBuf<int32_t> bsr_rowptr, bsr_col;
+  tfa::DevBuf<int32_t> blk4;                    // [nc][4] BSR block index of (i,i) and of (nbr_k, i); -1 if none
   tfa::DevBuf<double> cen;                      // [nc][2]
   tfa::DevBuf<double> cgeo;                     // [nc][24]
 };

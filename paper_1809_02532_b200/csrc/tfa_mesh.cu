@@ -233,6 +233,35 @@ __global__ void k_stencil_fill(int64_t nc, const int32_t* __restrict__ cell_node
   }
 }
 
+// ---- where cell i writes: its diagonal block (i,i) and, for each local face k with neighbour j,
+// the block (j,i) of the NEIGHBOUR's row ("mirror" block); -1 on the boundary ----
+__global__ void k_blk4(int64_t nc, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ rowptr,
+                       int32_t* __restrict__ blk4) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  const int32_t me = (int32_t)i;
+  int32_t n[3] = {cell_nbr[3 * i], cell_nbr[3 * i + 1], cell_nbr[3 * i + 2]};
+  int rank = 0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) rank += (n[k] >= 0 && n[k] < me);
+  blk4[4 * i] = rowptr[i] + rank;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const int64_t j = n[k];
+    int32_t b = -1;
+    if (j >= 0) {
+      int r = (int32_t)j < me;   // the neighbour's own diagonal column
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        const int32_t c = cell_nbr[3 * j + q];
+        r += (c >= 0 && c < me);
+      }
+      b = rowptr[j] + r;
+    }
+    blk4[4 * i + 1 + k] = b;
+  }
+}
+
 // ---- per-cell geometry record in canonical face orientation (tfa_common.cuh CGEO) ----
 __global__ void k_cgeo(int64_t nc, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ cell_faces,
                        const double* __restrict__ vol, const double* __restrict__ olen,
@@ -475,7 +504,7 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
     TFA_CUDA(cudaMemsetAsync(m.bsr_rowptr.p, 0, 4, st));
     TFA_CUDA(m.face_nodes.alloc(0)); TFA_CUDA(m.face_cells.alloc(0)); TFA_CUDA(m.cell_faces.alloc(0));
     TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
-    TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0));
+    TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0)); TFA_CUDA(m.blk4.alloc(0));
     ++m.generation;
     return 0;
   }
@@ -530,6 +559,8 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
   TFA_TRY(exclusive_scan_with_total(cnt, nc, m.bsr_rowptr, &m.nnzb, st));
   TFA_CUDA(m.bsr_col.alloc(m.nnzb));
   k_bsr_cols<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.bsr_rowptr.p, m.bsr_col.p);
+  TFA_CUDA(m.blk4.alloc(4 * nc));
+  k_blk4<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.bsr_rowptr.p, m.blk4.p);
 
   // vertex-neighbour stencil
   {

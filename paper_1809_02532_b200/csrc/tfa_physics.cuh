@@ -88,9 +88,9 @@ __device__ __forceinline__ void maxwell_flux(const Consts& K, const double* L, c
 
 // Multi-fluid AUSM+-up for one species (Eq. 10; Liou's scheme = ref. [30]; S4).
 // L, R = (rho, u, v, w, T).  Returns true if the states are physical.
-__device__ __forceinline__ bool ausm_flux(const Consts& K, int s, const double* L, const double* R, double nx,
-                                          double ny, double* H) {
-  const double Rs = K.Rs[s], gR = K.gR[s], cp = K.cp[s];
+// Rs, gR, cp, Minf2: the species' constants (K.Rs[s], ...), passed in registers (warp uniform).
+__device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, double Minf2, const Consts& K,
+                                          const double* L, const double* R, double nx, double ny, double* H) {
   const double rL = L[0], rR = R[0], TL = L[4], TR = R[4];
   const bool ok = (rL > 0.0) & (rR > 0.0) & (TL > 0.0) & (TR > 0.0);
   const double aL = sqrt(gR * TL), aR = sqrt(gR * TR);
@@ -102,7 +102,7 @@ __device__ __forceinline__ bool ausm_flux(const Consts& K, int s, const double* 
   const double ia = 1.0 / a12;
   const double ML = unL * ia, MR = unR * ia;
   const double Mb2 = 0.5 * (unL * unL + unR * unR) * (ia * ia);
-  const double Mo = sqrt(fmin(1.0, fmax(Mb2, K.Minf2[s])));
+  const double Mo = sqrt(fmin(1.0, fmax(Mb2, Minf2)));
   const double fa = Mo * (2.0 - Mo);
   const double al16 = 3.0 * (5.0 * fa * fa - 4.0);             // 16 alpha, alpha = 3/16 (-4 + 5 fa^2)
   // split Mach numbers and pressures; for |M| >= 1:  M4+ = max(M,0), P5+ = (M > 0), etc.
@@ -159,6 +159,46 @@ __device__ __forceinline__ void cons_species(const Consts& K, int s, const doubl
   U[2] = rho * Q[2];
   U[3] = rho * Q[3];
   U[4] = rho * (K.cv[s] * Q[4] + 0.5 * (Q[1] * Q[1] + Q[2] * Q[2] + Q[3] * Q[3]));
+}
+
+// static-index access to the five rows/variables of species SP inside an 18-vector held in registers
+template <int SP>
+__device__ __forceinline__ void sp_get(const double* v18, double* v5) {
+  v5[0] = v18[8 + SP];
+  v5[1] = v18[10 + 3 * SP];
+  v5[2] = v18[11 + 3 * SP];
+  v5[3] = v18[12 + 3 * SP];
+  v5[4] = v18[16 + SP];
+}
+template <int SP>
+__device__ __forceinline__ void sp_put(double* v18, const double* v5) {
+  v18[8 + SP] = v5[0];
+  v18[10 + 3 * SP] = v5[1];
+  v18[11 + 3 * SP] = v5[2];
+  v18[12 + 3 * SP] = v5[3];
+  v18[16 + SP] = v5[4];
+}
+// column v of (3 Omega / 2 dt) dU/dP for a species variable v (analytic, S15)
+template <int SP>
+__device__ __forceinline__ void time_column(const Consts& K, double* col, int v, const double* P, double ft) {
+  constexpr int ir = 8 + SP, iu = 10 + 3 * SP, iT = 16 + SP;
+  const double rho = P[ir], ux = P[iu], uy = P[iu + 1], uz = P[iu + 2], T = P[iT];
+  if (v == ir) {
+    col[ir] += ft;
+    col[iu] += ft * ux;
+    col[iu + 1] += ft * uy;
+    col[iu + 2] += ft * uz;
+    col[iT] += ft * (K.cv[SP] * T + 0.5 * (ux * ux + uy * uy + uz * uz));
+  } else if (v == iT) {
+    col[iT] += ft * rho * K.cv[SP];
+  } else {
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+      if (v == iu + d) {
+        col[iu + d] += ft * rho;
+        col[iT] += ft * rho * P[iu + d];
+      }
+  }
 }
 
 }  // namespace tfa
