@@ -3,21 +3,22 @@
 // Design, replacing Alg. 1's thread-per-cell loop (L221-256):
 //
 //  * A persistent CTA walks tiles of T consecutive cells.  Cell i evaluates, for each of its three
-//    faces, the base numerical flux and the fluxes with each variable of ITS OWN side perturbed
-//    (Alg. 1).  The column (H_pert - H)/eps * s_if * Sigma_f is (a) accumulated into the
-//    diagonal block (i,i) and (b) written, negated, as the block (j,i) of the NEIGHBOUR's row:
-//    s_jf = -s_if, so d R_j / d P_i through the shared face is exactly minus cell i's own
-//    contribution (same inputs, same code, bit-identical).  Every BSR block has exactly one
-//    writer (cell i writes (i,i) and the (j,i)), so there are no atomics, no memset, and the
-//    perturbed fluxes towards the other side are never evaluated: 6+6+9 = 21 flux evaluations per
-//    cell-face instead of Alg. 1's 3*19 = 57 full ones.
+//    faces, the numerical flux through the face in ITS OWN outward frame (own state first, outward
+//    normal) and the fluxes with each variable of its own side perturbed (Alg. 1).  The
+//    column (H_pert - H)/eps * Sigma_f is (a) accumulated into the diagonal block (i,i) and (b)
+//    written, negated, as the block (j,i) of the NEIGHBOUR's row: the face enters R_j with the
+//    opposite sign, so d R_j / d P_i through it is exactly minus cell i's own contribution.  Every
+//    BSR block has exactly one writer, so there are no atomics and no memset, and the perturbed
+//    fluxes towards the other side are never evaluated: 6+6+9 = 21 flux evaluations per cell-face
+//    instead of Alg. 1's 3*19 = 57 full ones.
 //  * Lanes: an AUSM warp holds 5 groups of 6 lanes = (cell, species) x {base, 5 perturbed variables}
 //    (Eq. 10); a Maxwell warp holds 3 groups of 9 lanes = cell x {base, 8 perturbed} (Eq. 9
-//    L91).  The base flux reaches the group by warp shuffle; the flux Jacobian is block diagonal
-//    (8x8, 5x5, 5x5), the source (Eq. 4/6) couples the blocks on the diagonal block only.
-//  * 18x18 blocks are staged in shared memory (the structural zeros of the mirror blocks are
-//    written once per CTA) and leave the SM as 2592-byte TMA bulk stores
-//    (cp.async.bulk.global.shared::cta), rhs as one bulk store per tile.
+//    L91).  Each lane reconstructs the face states it needs itself (L232: P + phi grad P . dx) from
+//    the cell records (L1/L2 hits; every lane of a group reads the same addresses), the base flux
+//    reaches the group by warp shuffle; the flux Jacobian is block diagonal (8x8, 5x5, 5x5), the
+//    source (Eq. 4/6) couples the blocks on the diagonal block only.
+//  * 18x18 blocks are staged in shared memory (their structural zeros are written once per CTA)
+//    and leave the SM as 2592-byte TMA bulk stores (cp.async.bulk.global.shared::cta).
 #include "tfa_common.cuh"
 #include "tfa_physics.cuh"
 
@@ -37,6 +38,8 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 // make generic-proxy shared-memory writes visible to the async proxy (TMA) before the barrier
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// CTA barrier reached from role-specialised code (every warp executes the same number of them)
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------------
 template <int T>
@@ -49,21 +52,30 @@ struct AsmCfg {
 
 template <int T>
 struct __align__(128) AsmSmem {
-  double mir[T][BLK];          // staged mirror block (j,i) of the current face; zeros persist
-  double diag[T][BLK];         // staged diagonal block (i,i)
-  double fb[T][3][2][NEQ];     // reconstructed face states, canonical side 0 = L, 1 = R
-  double fpert[T][3][NEQ];     // own-side face state with variable v of the CELL perturbed
-  double eps[T][NEQ];          // representable perturbation sizes of the own cell (S7)
-  double pc[T][NEQ];           // own cell-centre state
-  double s0[T][NEQ];           // source S(P_i)
-  double rs[T][NEQ];           // non-flux part of R~: Omega (BDF2 term) - Omega S
-  double rhs[T][NEQ];          // staged -R~
-  double fg[T][3][4];          // nx, ny, s_if * Sigma_f, unused
-  double vol[T];
-  double ref[NEQ];
-  alignas(16) int32_t blk[T][4];   // BSR block index of (i,i), (nbr0,i), (nbr1,i), (nbr2,i); -1 if absent
-  int32_t nbr[T][3];
+  double mir[T][BLK];    // staged mirror block (j,i) of the current face; structural zeros persist
+  double diag[T][BLK];   // staged diagonal block (i,i); structural zeros persist
+  double rs[T][NEQ];     // non-flux part of R~: Omega (BDF2 term) - Omega S
+  double s0[T][8];       // Lorentz-force and Joule-heating rows of S(P_i): equations 10..17
 };
+
+// roles: 0 = ion AUSM lanes, 1 = electron AUSM lanes, 2 = Maxwell lanes.
+// index of the q-th variable of the role's group inside the 18-vector
+template <int ROLE>
+__device__ __forceinline__ constexpr int vidx(int q) {
+  return ROLE == 2 ? q : (q == 0 ? 8 + ROLE : (q == 4 ? 16 + ROLE : 9 + 3 * ROLE + q));
+}
+
+// Momentum and energy source rows of one species (Eq. 6; S5) with the rounding sequence
+// pinned, so that the base values kept in shared memory and the perturbed re-evaluations of the
+// source Jacobian (Alg. 1) agree bit for bit wherever the perturbed variable does not enter.
+__device__ __forceinline__ void lorentz_rows(double qn, const double* E, const double* B, double u, double v,
+                                             double w, double* out4) {
+  double t;
+  t = __dmul_rn(w, B[1]); t = __fma_rn(v, B[2], -t); out4[0] = __dmul_rn(qn, __dadd_rn(E[0], t));
+  t = __dmul_rn(u, B[2]); t = __fma_rn(w, B[0], -t); out4[1] = __dmul_rn(qn, __dadd_rn(E[1], t));
+  t = __dmul_rn(v, B[0]); t = __fma_rn(u, B[1], -t); out4[2] = __dmul_rn(qn, __dadd_rn(E[2], t));
+  t = __dmul_rn(u, E[0]); t = __fma_rn(v, E[1], t); t = __fma_rn(w, E[2], t); out4[3] = __dmul_rn(qn, t);
+}
 
 // conservative variables of one species from (rho, u, v, w, T)
 __device__ __forceinline__ void cons5(double cv, const double* Q, double* U) {
@@ -74,249 +86,194 @@ __device__ __forceinline__ void cons5(double cv, const double* Q, double* U) {
   U[4] = Q[0] * (cv * Q[4] + 0.5 * (Q[1] * Q[1] + Q[2] * Q[2] + Q[3] * Q[3]));
 }
 
-template <int T, bool JAC>
-__global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
-    int64_t nc, Consts K, const double* __restrict__ state, const double* __restrict__ state_n,
-    const double* __restrict__ state_nm1, double inv2dt, const double* __restrict__ lgrad,
-    const double* __restrict__ cgeo, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ blk4,
-    double* __restrict__ rhs, double* __restrict__ vals, int32_t* __restrict__ flags) {
+// ------------------------------------------------------------------------------------------------
+// Non-flux part of the residual of one (cell, group): source (Alg. 1) and BDF2 term (Eq. 13).
+// grp 0 = field rows 0..7, 1 = ion rows, 2 = electron rows.  Writes S.rs (all rows) and S.s0.
+// ------------------------------------------------------------------------------------------------
+template <int T>
+__device__ __forceinline__ void cell_group_rest(AsmSmem<T>& S, const Consts& K, int c, int grp, int64_t i,
+                                                const double* __restrict__ state,
+                                                const double* __restrict__ state_n,
+                                                const double* __restrict__ state_nm1, double vol, double inv2dt) {
+  const bool do_src = K.mask & 2, do_time = K.mask & 4;
+  const double* P = state + NEQ * i;
+  const double ft = vol * inv2dt;
+  if (grp == 0) {
+    // S_E = -c^2 sum_s q_s n_s u_s, S_Phi = c^2 sum_s q_s n_s  (Eq. 4; eps0 = 1/c^2)
+    const double qi = K.qm[0] * P[8], qe = K.qm[1] * P[9];
+    double Sf[8];
+    Sf[0] = Sf[1] = Sf[2] = Sf[6] = 0.0;
+    Sf[3] = -K.c2 * (qi * P[10] + qe * P[13]);
+    Sf[4] = -K.c2 * (qi * P[11] + qe * P[14]);
+    Sf[5] = -K.c2 * (qi * P[12] + qe * P[15]);
+    Sf[7] = K.c2 * (qi + qe);
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      double a = 0.0;
+      if (do_src) a -= Sf[r] * vol;
+      if (do_time) a += ft * (3.0 * P[r] - 4.0 * state_n[NEQ * i + r] + state_nm1[NEQ * i + r]);
+      S.rs[c][r] = a;
+    }
+  } else {
+    const int s = grp - 1;
+    const int rows[5] = {8 + s, 10 + 3 * s, 11 + 3 * s, 12 + 3 * s, 16 + s};
+    double Q[5], Qn[5], Qm[5], U[5], Un[5], Um[5], S5[5], E[3], B[3];
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {
+      Q[r] = P[rows[r]];
+      Qn[r] = state_n[NEQ * i + rows[r]];
+      Qm[r] = state_nm1[NEQ * i + rows[r]];
+    }
+#pragma unroll
+    for (int r = 0; r < 3; ++r) { B[r] = P[r]; E[r] = P[3 + r]; }
+    S5[0] = 0.0;
+    lorentz_rows(K.qm[s] * Q[0], E, B, Q[1], Q[2], Q[3], S5 + 1);
+    const double cv = K.cv[s];
+    cons5(cv, Q, U);
+    cons5(cv, Qn, Un);
+    cons5(cv, Qm, Um);
+#pragma unroll
+    for (int r = 0; r < 5; ++r) {
+      double a = 0.0;
+      if (do_src) a -= S5[r] * vol;
+      if (do_time) a += ft * (3.0 * U[r] - 4.0 * Un[r] + Um[r]);
+      S.rs[c][rows[r]] = a;
+    }
+    S.s0[c][3 * s] = S5[1];
+    S.s0[c][3 * s + 1] = S5[2];
+    S.s0[c][3 * s + 2] = S5[3];
+    S.s0[c][6 + s] = S5[4];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// The tile loop of one warp role.  All roles execute the same sequence of CTA barriers.
+// ------------------------------------------------------------------------------------------------
+template <int T, int ROLE>
+__device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const int64_t nc, const Consts& K,
+                                          const double* __restrict__ state, const double* __restrict__ state_n,
+                                          const double* __restrict__ state_nm1, const double inv2dt,
+                                          const double* __restrict__ lgrad, const double* __restrict__ cgeo,
+                                          const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ blk4,
+                                          double* __restrict__ rhs, double* __restrict__ vals,
+                                          int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  AsmSmem<T>& S = *reinterpret_cast<AsmSmem<T>*>(smem_raw);
+  constexpr int NV = ROLE == 2 ? 8 : 5;   // variables (= rows) of the role's group
+  constexpr int GL = NV + 1;              // lanes per group: base + NV perturbed
+  constexpr int NG = ROLE == 2 ? 3 : 5;   // groups per warp
+  constexpr int SPC = ROLE == 2 ? 0 : ROLE;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool do_flux = K.mask & 1, do_src = K.mask & 2, do_time = K.mask & 4;
   const int64_t ntiles = (nc + T - 1) / T;
 
-  // ---- role of this lane (tile independent) ----
-  const bool is_ausm = warp < C::AW;
-  int cl, p, sp = 0, base_lane;
-  bool lane_ok;
-  if (is_ausm) {
-    const int g = lane / 6;
-    p = lane - 6 * g;
-    sp = warp & 1;
-    cl = 5 * (warp >> 1) + g;
-    lane_ok = lane < 30;
-    base_lane = 6 * g;
-  } else {
-    const int g = lane / 9;
-    p = lane - 9 * g;
-    cl = 3 * (warp - C::AW) + g;
-    lane_ok = lane < 27 && cl < T;
-    base_lane = 9 * g;
-  }
-  if (!lane_ok) cl = 0;   // idle lanes shadow cell 0 (they take part in the shuffles, never store)
-  // rows = variables of this lane's group; a_v / m_v = the variable this lane perturbs
-  const int ir = 8 + sp, iu = 10 + 3 * sp, iT = 16 + sp;
-  const int pj = p > 0 ? p - 1 : 0;
-  const int v = is_ausm ? (pj == 0 ? ir : (pj == 4 ? iT : iu + pj - 1)) : pj;
-  // species constants (warp uniform)
-  const double cRs = K.Rs[sp], cgR = K.gR[sp], ccp = K.cp[sp], cMinf2 = K.Minf2[sp];
-
-  if (JAC)
-    for (int q = tid; q < T * BLK; q += C::NT) (&S.mir[0][0])[q] = 0.0;
-  if (tid < NEQ) S.ref[tid] = K.ref[tid];
-  __syncthreads();
-
+  const int g = lane / GL, p = lane - GL * g;
+  int cl = ROLE == 2 ? 3 * (warp - C::AW) + g : 5 * (warp >> 1) + g;
+  const bool lane_ok = lane < GL * NG && cl < T;
+  if (!lane_ok) cl = 0;   // idle lanes shadow the tile's first cell (they join the shuffles, never store)
+  const int base_lane = GL * g;
+  const bool pert = p != 0;
+  const int pj = p - 1;   // perturbed variable of the group; -1 on the base lane
+  const int v = ROLE == 2 ? max(pj, 0) : (pj <= 0 ? 8 + ROLE : (pj == 4 ? 16 + ROLE : 9 + 3 * ROLE + pj));
+  const bool run = do_flux && (JAC || !pert);
   bool nonphys = false;
 
 #pragma unroll 1
   for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const int64_t cell0 = tile * T;
     const int ncell = (int)min((int64_t)T, nc - cell0);
+    const bool act = lane_ok && cl < ncell;
+    const int64_t i = cell0 + (act ? cl : 0);
+    const double* __restrict__ cg = cgeo + CGEO * i;
+    const double* __restrict__ sO = state + NEQ * i;
+    const double2* __restrict__ gO = reinterpret_cast<const double2*>(lgrad) + NEQ * i;
 
-    // ---- phase 0: topology and face geometry of the tile ----
-    if (tid < 3 * T) {
-      const int c = tid / 3, k = tid - 3 * c;
-      const int64_t i = cell0 + c;
-      if (c < ncell) {
-        const double* g = cgeo + CGEO * i + 8 * k;
-        const int32_t j = cell_nbr[3 * i + k];
-        const bool own_is_L = j < 0 || i < j;
-        S.nbr[c][k] = j;
-        S.fg[c][k][0] = g[0];
-        S.fg[c][k][1] = g[1];
-        S.fg[c][k][2] = own_is_L ? g[2] : -g[2];
-        if (k == 0) S.vol[c] = g[7];
-      }
-    }
-    // S.blk[t] is written and read (when the bulk stores are issued) by thread t only
-    if (tid < ncell) *reinterpret_cast<int4*>(&S.blk[tid][0]) = *reinterpret_cast<const int4*>(blk4 + 4 * (cell0 + tid));
-    // ---- phase A: reconstruct L/R face states and the own-side perturbed ones (Alg. 1)
-    for (int q = tid; q < ncell * (6 * NEQ); q += C::NT) {
-      const int c = q / (6 * NEQ), rem = q - c * (6 * NEQ);
-      const int k = rem / (2 * NEQ), rem2 = rem - k * (2 * NEQ);
-      const int side = rem2 / NEQ, w = rem2 - side * NEQ;
-      const int64_t i = cell0 + c;
-      const int32_t j = cell_nbr[3 * i + k];
-      const bool own_is_L = j < 0 || i < j;
-      const bool is_own = (j < 0) || (side == (own_is_L ? 0 : 1));   // boundary: P_R := P_L (S9)
-      const int64_t X = is_own ? i : j;
-      const double* g = cgeo + CGEO * i + 8 * k;
-      const double dx = is_own ? g[3] : g[5], dy = is_own ? g[4] : g[6];
-      const double Pc = state[NEQ * X + w];
-      const double2 lg = *reinterpret_cast<const double2*>(lgrad + 2 * (NEQ * X + w));
-      const double inc = lg.x * dx + lg.y * dy;
-      S.fb[c][k][side][w] = Pc + inc;
-      if (is_own && (side == 0 || j >= 0)) {
-        // eps_k = delta * max(|P_cell,k|, ref_k), made representable (S7)
-        const double t = Pc + K.delta * fmax(fabs(Pc), S.ref[w]);
-        S.fpert[c][k][w] = t + inc;
-        if (k == 0) {
-          S.eps[c][w] = t - Pc;
-          S.pc[c][w] = Pc;
-        }
-      }
-    }
-    // ---- phase A2: the non-flux part of the residual (source L245, BDF2 Eq. 13), per (cell, group)
-    if (tid >= C::NT - 3 * T) {
+    // ---- the non-flux part of the residual, one thread per (cell, group) ----
+    if (ROLE == 2 && tid >= C::NT - 3 * T) {
       const int q = tid - (C::NT - 3 * T);
-      const int c = q / 3, grp = q - 3 * c;   // 0 fields, 1 ions, 2 electrons
-      const int64_t i = cell0 + c;
-      if (c < ncell) {
-        double P[NEQ], Ss[NEQ];
-#pragma unroll
-        for (int r = 0; r < NEQ; r += 2) {
-          const double2 t2 = *reinterpret_cast<const double2*>(state + NEQ * i + r);
-          P[r] = t2.x;
-          P[r + 1] = t2.y;
-        }
-        source_terms(K, P, Ss);
-        const double vol = cgeo[CGEO * i + 7];
-        const double ft = vol * inv2dt;
-        if (grp == 0) {
-#pragma unroll
-          for (int r = 0; r < 8; ++r) {
-            double a = 0.0;
-            if (do_src) a -= Ss[r] * vol;
-            if (do_time) a += ft * (3.0 * P[r] - 4.0 * state_n[NEQ * i + r] + state_nm1[NEQ * i + r]);
-            S.rs[c][r] = a;
-            S.s0[c][r] = Ss[r];
-          }
-        } else {
-          const int s = grp - 1;
-          const int rows[5] = {8 + s, 10 + 3 * s, 11 + 3 * s, 12 + 3 * s, 16 + s};
-          double Q[5], Qn[5], Qm[5], U[5], Un[5], Um[5], S5[5];
-          if (s == 0) { sp_get<0>(P, Q); sp_get<0>(Ss, S5); } else { sp_get<1>(P, Q); sp_get<1>(Ss, S5); }
-#pragma unroll
-          for (int r = 0; r < 5; ++r) {
-            Qn[r] = state_n[NEQ * i + rows[r]];
-            Qm[r] = state_nm1[NEQ * i + rows[r]];
-          }
-          const double cv = K.cv[s];
-          cons5(cv, Q, U);
-          cons5(cv, Qn, Un);
-          cons5(cv, Qm, Um);
-#pragma unroll
-          for (int r = 0; r < 5; ++r) {
-            double a = 0.0;
-            if (do_src) a -= S5[r] * vol;
-            if (do_time) a += ft * (3.0 * U[r] - 4.0 * Un[r] + Um[r]);
-            S.rs[c][rows[r]] = a;
-            S.s0[c][rows[r]] = S5[r];
-          }
-        }
-      }
+      const int c = q / 3, grp = q - 3 * c;
+      if (c < ncell)
+        cell_group_rest<T>(S, K, c, grp, cell0 + c, state, state_n, state_nm1, cgeo[CGEO * (cell0 + c) + 7], inv2dt);
     }
-    __syncthreads();   // B0: tile inputs staged
+    // where this tile's blocks go: thread t < ncell issues the bulk stores of cell t
+    int4 b4 = make_int4(-1, -1, -1, -1);
+    if (ROLE == 0 && JAC && tid < ncell) b4 = *reinterpret_cast<const int4*>(blk4 + 4 * (cell0 + tid));
 
-    const bool cell_ok = lane_ok && cl < ncell;
-    const bool pert = p != 0;
-    double acc[8];     // base lane: residual rows; perturbed lane: its column of the diagonal block
+    // eps_k = delta * max(|P_cell,k|, ref_k), made representable (S7)
+    const double Pcv = sO[v];
+    const double tv = Pcv + K.delta * fmax(fabs(Pcv), K.ref[v]);
+    const double eps = tv - Pcv;
+    const double inv_e = 1.0 / eps;
+
+    double acc[NV];   // base lane: residual rows; perturbed lane: its column of the diagonal block
 #pragma unroll
-    for (int q = 0; q < 8; ++q) acc[q] = 0.0;
-    const double inv_e = (JAC && pert) ? 1.0 / S.eps[cl][v] : 0.0;
+    for (int q = 0; q < NV; ++q) acc[q] = 0.0;
 
-    // ---- phase B: faces (Alg. 1) ----
+    // ---- faces (Alg. 1) ----
 #pragma unroll 1
     for (int k = 0; k < 3; ++k) {
-      const int32_t j = S.nbr[cl][k];
-      const double nx = S.fg[cl][k][0], ny = S.fg[cl][k][1], sl = S.fg[cl][k][2];
-      const bool own_is_L = sl > 0.0, bnd = j < 0;
-      const bool run = do_flux && (JAC || !pert);
-      double d[8];
-      if (is_ausm) {
-        double H[5];
-        if (run) {
-          double L[5], R[5];
-          L[0] = S.fb[cl][k][0][ir]; R[0] = S.fb[cl][k][1][ir];
+      const int32_t j = cell_nbr[3 * i + k];
+      const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);       // canonical unit normal
+      const double2 g23 = *reinterpret_cast<const double2*>(cg + 8 * k + 2);   // Sigma_f, x_f - x_i (x)
+      const double2 g45 = *reinterpret_cast<const double2*>(cg + 8 * k + 4);   // x_f - x_i (y), x_f - x_j (x)
+      const double dyn = cg[8 * k + 6];
+      const bool bnd = j < 0;
+      const bool own_is_L = bnd || i < (int64_t)j;
+      const double nx = own_is_L ? g01.x : -g01.x, ny = own_is_L ? g01.y : -g01.y;   // outward normal
+      const double len = g23.x, dxo = g23.y, dyo = g45.x;
+      const double dxx = bnd ? dxo : g45.y, dyx = bnd ? dyo : dyn;   // boundary: P_R := P_L (S9)
+      const int64_t X = bnd ? i : (int64_t)j;
+      const double* __restrict__ sX = state + NEQ * X;
+      const double2* __restrict__ gX = reinterpret_cast<const double2*>(lgrad) + NEQ * X;
+
+      double H[NV];
+      if (run) {
+        // face states: own side and the other side (L232); the perturbed variable enters at the
+        // cell centre and is re-extrapolated with the frozen limited gradient (L236-237; S8)
+        double own[NV], oth[NV];
 #pragma unroll
-          for (int q = 0; q < 3; ++q) { L[1 + q] = S.fb[cl][k][0][iu + q]; R[1 + q] = S.fb[cl][k][1][iu + q]; }
-          L[4] = S.fb[cl][k][0][iT]; R[4] = S.fb[cl][k][1][iT];
-          if (pert) {
-            const double pv = S.fpert[cl][k][v];
-            const bool pl = own_is_L || bnd, pr = !own_is_L || bnd;   // boundary: both arguments move (S9)
-#pragma unroll
-            for (int q = 0; q < 5; ++q)
-              if (q == pj) {
-                if (pl) L[q] = pv;
-                if (pr) R[q] = pv;
-              }
+        for (int q = 0; q < NV; ++q) {
+          const int ix = vidx<ROLE>(q);
+          double po = sO[ix], px = sX[ix];
+          const double2 go = gO[ix], gx = gX[ix];
+          if (q == pj) {
+            po = tv;
+            if (bnd) px = tv;   // boundary: the perturbation moves both arguments (S9)
           }
-          const bool ok = ausm_flux(cRs, cgR, ccp, cMinf2, K, L, R, nx, ny, H);
-          if (!pert && cell_ok) nonphys |= !ok;
-        } else {
-#pragma unroll
-          for (int q = 0; q < 5; ++q) H[q] = 0.0;
+          own[q] = po + (go.x * dxo + go.y * dyo);
+          oth[q] = px + (gx.x * dxx + gx.y * dyx);
         }
-        const double f = pert ? sl * inv_e : sl;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const double hb = __shfl_sync(0xffffffffu, H[q], base_lane);
-          // explicit rounding: the residual must not depend on JAC through FMA contraction
-          d[q] = __dmul_rn(pert ? H[q] - hb : H[q], f);
-          acc[q] = __dadd_rn(acc[q], d[q]);
+        if (ROLE == 2) {
+          maxwell_flux(K, own, oth, nx, ny, H);
+        } else {
+          const bool ok = ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nx, ny, H);
+          if (!pert && act) nonphys |= !ok;
         }
       } else {
-        double H[8];
-        if (run) {
-          double L[8], R[8];
 #pragma unroll
-          for (int q = 0; q < 8; ++q) { L[q] = S.fb[cl][k][0][q]; R[q] = S.fb[cl][k][1][q]; }
-          if (pert) {
-            const double pv = S.fpert[cl][k][v];
-            const bool pl = own_is_L || bnd, pr = !own_is_L || bnd;
+        for (int q = 0; q < NV; ++q) H[q] = 0.0;
+      }
+      const double f = pert ? len * inv_e : len;
+      double d[NV];
 #pragma unroll
-            for (int q = 0; q < 8; ++q)
-              if (q == pj) {
-                if (pl) L[q] = pv;
-                if (pr) R[q] = pv;
-              }
-          }
-          maxwell_flux(K, L, R, nx, ny, H);
-        } else {
-#pragma unroll
-          for (int q = 0; q < 8; ++q) H[q] = 0.0;
-        }
-        const double f = pert ? sl * inv_e : sl;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          const double hb = __shfl_sync(0xffffffffu, H[q], base_lane);
-          // explicit rounding: the residual must not depend on JAC through FMA contraction
-          d[q] = __dmul_rn(pert ? H[q] - hb : H[q], f);
-          acc[q] = __dadd_rn(acc[q], d[q]);
-        }
+      for (int q = 0; q < NV; ++q) {
+        const double hb = __shfl_sync(0xffffffffu, H[q], base_lane);
+        // explicit rounding: the residual must not depend on JAC through FMA contraction
+        d[q] = __dmul_rn(pert ? H[q] - hb : H[q], f);
+        acc[q] = __dadd_rn(acc[q], d[q]);
       }
       if (!JAC) continue;
       // the staging of the previous face / tile has been read by the TMA
-      if (tid < T) bulk_wait_read();
-      __syncthreads();   // B1
-      if (pert && cell_ok && !bnd) {
-        if (is_ausm) {
-          S.mir[cl][ir * NEQ + v] = -d[0];
+      if (ROLE == 0 && tid < T) bulk_wait_read();
+      cta_sync();   // B1
+      if (pert && act && !bnd) {
 #pragma unroll
-          for (int q = 0; q < 3; ++q) S.mir[cl][(iu + q) * NEQ + v] = -d[1 + q];
-          S.mir[cl][iT * NEQ + v] = -d[4];
-        } else {
-#pragma unroll
-          for (int q = 0; q < 8; ++q) S.mir[cl][q * NEQ + v] = -d[q];
-        }
+        for (int q = 0; q < NV; ++q) S.mir[cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
       }
       fence_async_smem();
-      __syncthreads();   // B2
+      cta_sync();   // B2
       // a7: the block (j,i) leaves the SM as one 2592-byte bulk store
-      if (tid < ncell) {
-        const int32_t b = S.blk[tid][1 + k];
+      if (ROLE == 0 && tid < ncell) {
+        const int32_t b = k == 0 ? b4.y : (k == 1 ? b4.z : b4.w);
         if (b >= 0) {
           bulk_store(vals + (int64_t)b * BLK, &S.mir[tid][0], BLK * 8);
           bulk_commit();
@@ -324,76 +281,125 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
       }
     }
 
-    // ---- phase C: residual, source Jacobian (L245-253), BDF2 diagonal (Eq. 13), diagonal block ----
-    if (!JAC) {
-      if (tid < T) bulk_wait_read();
-      __syncthreads();
+    // ---- residual, source Jacobian (L245-253), BDF2 diagonal (Eq. 13), diagonal block ----
+    if (!JAC) cta_sync();   // S.rs of this tile is complete
+    if (act && !pert) {
+#pragma unroll
+      for (int q = 0; q < NV; ++q) rhs[NEQ * i + vidx<ROLE>(q)] = -(acc[q] + S.rs[cl][vidx<ROLE>(q)]);
     }
-    if (cell_ok && !pert) {
-      if (is_ausm) {
-        S.rhs[cl][ir] = -(acc[0] + S.rs[cl][ir]);
-#pragma unroll
-        for (int q = 0; q < 3; ++q) S.rhs[cl][iu + q] = -(acc[1 + q] + S.rs[cl][iu + q]);
-        S.rhs[cl][iT] = -(acc[4] + S.rs[cl][iT]);
-      } else {
-#pragma unroll
-        for (int q = 0; q < 8; ++q) S.rhs[cl][q] = -(acc[q] + S.rs[cl][q]);
-      }
-    }
-    if (JAC && cell_ok && pert) {
-      const double vol = S.vol[cl];
-      double col[NEQ];
-#pragma unroll
-      for (int r = 0; r < NEQ; ++r) col[r] = 0.0;
-      if (is_ausm) {
-        // flux part: rows of this species (static indices per species keep col[] in registers)
-        if (sp == 0) sp_put<0>(col, acc); else sp_put<1>(col, acc);
-      } else {
-#pragma unroll
-        for (int q = 0; q < 8; ++q) col[q] = acc[q];
-      }
-      double P[NEQ];
-#pragma unroll
-      for (int r = 0; r < NEQ; ++r) P[r] = S.pc[cl][r];
-      if (do_time) {
-        // analytic dU/dP (S15): identity on the field rows; species rows below
+    if (JAC) {
+      if (act && pert) {
+        const double vol = cg[7];
         const double ft = 3.0 * vol * inv2dt;
-        if (!is_ausm) {
+        const double fs = vol * inv_e;
+        if (ROLE == 2) {
+          // column v = pj of the field variables: flux rows 0..7 (+ BDF2 identity, S15) and, for B and E,
+          // the Lorentz / Joule rows of both species
+          if (do_time) {
 #pragma unroll
-          for (int r = 0; r < 8; ++r)
-            if (r == v) col[r] += ft;
-        } else if (sp == 0) time_column<0>(K, col, v, P, ft);
-        else time_column<1>(K, col, v, P, ft);
+            for (int q = 0; q < 8; ++q)
+              if (q == pj) acc[q] += ft;
+          }
+#pragma unroll
+          for (int q = 0; q < 8; ++q) S.diag[cl][q * NEQ + v] = acc[q];
+          double E[3], B[3];
+#pragma unroll
+          for (int r = 0; r < 3; ++r) {
+            B[r] = r == pj ? tv : sO[r];
+            E[r] = 3 + r == pj ? tv : sO[3 + r];
+          }
+#pragma unroll
+          for (int s = 0; s < 2; ++s) {
+            double S1[4];
+            lorentz_rows(K.qm[s] * sO[8 + s], E, B, sO[10 + 3 * s], sO[11 + 3 * s], sO[12 + 3 * s], S1);
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+              S.diag[cl][(10 + 3 * s + r) * NEQ + v] = do_src ? -(S1[r] - S.s0[cl][3 * s + r]) * fs : 0.0;
+            S.diag[cl][(16 + s) * NEQ + v] = do_src ? -(S1[3] - S.s0[cl][6 + s]) * fs : 0.0;
+          }
+        } else {
+          // column v of species ROLE: own flux rows (+ BDF2 dU/dP, analytic, S15), own Lorentz / Joule
+          // rows, and the current / charge rows of E and Phi
+          double Q[5], Qp[5], E[3], B[3];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            Q[q] = sO[vidx<ROLE>(q)];
+            Qp[q] = q == pj ? tv : Q[q];
+          }
+#pragma unroll
+          for (int r = 0; r < 3; ++r) { B[r] = sO[r]; E[r] = sO[3 + r]; }
+          if (do_time) {
+            const double cv = K.cv[SPC];
+            if (pj == 0) {
+              acc[0] += ft;
+              acc[1] += ft * Q[1];
+              acc[2] += ft * Q[2];
+              acc[3] += ft * Q[3];
+              acc[4] += ft * (cv * Q[4] + 0.5 * (Q[1] * Q[1] + Q[2] * Q[2] + Q[3] * Q[3]));
+            } else if (pj == 4) {
+              acc[4] += ft * Q[0] * cv;
+            } else {
+#pragma unroll
+              for (int dd = 1; dd <= 3; ++dd)
+                if (pj == dd) {
+                  acc[dd] += ft * Q[0];
+                  acc[4] += ft * Q[0] * Q[dd];
+                }
+            }
+          }
+          const double qn = K.qm[SPC] * Q[0], qnp = K.qm[SPC] * Qp[0];
+          double S1[4];
+          lorentz_rows(qnp, E, B, Qp[1], Qp[2], Qp[3], S1);
+          if (do_src) {
+#pragma unroll
+            for (int r = 0; r < 3; ++r) acc[1 + r] -= (S1[r] - S.s0[cl][3 * SPC + r]) * fs;
+            acc[4] -= (S1[3] - S.s0[cl][6 + SPC]) * fs;
+          }
+#pragma unroll
+          for (int q = 0; q < 5; ++q) S.diag[cl][vidx<ROLE>(q) * NEQ + v] = acc[q];
+          // S_E = -c^2 sum_s q_s n_s u_s and S_Phi = c^2 sum_s q_s n_s: only this species' term moves
+#pragma unroll
+          for (int r = 0; r < 3; ++r)
+            S.diag[cl][(3 + r) * NEQ + v] = do_src ? K.c2 * (qnp * Qp[1 + r] - qn * Q[1 + r]) * fs : 0.0;
+          S.diag[cl][7 * NEQ + v] = do_src ? -K.c2 * (qnp - qn) * fs : 0.0;
+        }
       }
-      if (do_src) {
-        const double e = S.eps[cl][v];
-#pragma unroll
-        for (int r = 0; r < NEQ; ++r)
-          if (r == v) P[r] += e;
-        double S1[NEQ];
-        source_terms(K, P, S1);
-        const double f = vol * inv_e;
-        // rows 0,1,2 (B), 6 (Psi), 8,9 (mass) have no source: S1 - S0 = 0 exactly
-#pragma unroll
-        for (int r = 0; r < NEQ; ++r)
-          if (!(r < 3 || r == 6 || r == 8 || r == 9)) col[r] -= (S1[r] - S.s0[cl][r]) * f;
+      fence_async_smem();
+      cta_sync();   // B3
+      if (ROLE == 0 && tid < ncell) {
+        bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[tid][0], BLK * 8);
+        bulk_commit();
       }
-#pragma unroll
-      for (int r = 0; r < NEQ; ++r) S.diag[cl][r * NEQ + v] = col[r];
-    }
-    fence_async_smem();
-    __syncthreads();   // B3
-    if (tid < ncell && JAC) {
-      bulk_store(vals + (int64_t)S.blk[tid][0] * BLK, &S.diag[tid][0], BLK * 8);
-      bulk_commit();
-    }
-    if (tid == T - 1) {
-      bulk_store(rhs + NEQ * cell0, &S.rhs[0][0], (uint32_t)ncell * NEQ * 8);
-      bulk_commit();
     }
   }
-  if (tid < T) bulk_wait_all();
+  if (ROLE == 0 && JAC && tid < T) bulk_wait_all();
   if (nonphys) atomicAdd(flags, 1);
+}
+
+template <int T>
+__global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
+    const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
+    const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
+    const double* __restrict__ lgrad, const double* __restrict__ cgeo, const int32_t* __restrict__ cell_nbr,
+    const int32_t* __restrict__ blk4, double* __restrict__ rhs, double* __restrict__ vals,
+    int32_t* __restrict__ flags) {
+  using C = AsmCfg<T>;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  AsmSmem<T>& S = *reinterpret_cast<AsmSmem<T>*>(smem_raw);
+  // one instantiation serves both calls, so that the residual does not depend on whether the
+  // Jacobian is asked for (same instructions on the base lanes)
+  const bool JAC = vals != nullptr;
+  if (JAC) {
+    for (int q = threadIdx.x; q < 2 * T * BLK; q += C::NT) (&S.mir[0][0])[q] = 0.0;   // mir and diag
+    __syncthreads();
+  }
+  const int warp = threadIdx.x >> 5;
+  if (warp >= C::AW)
+    role_loop<T, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+  else if (warp & 1)
+    role_loop<T, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+  else
+    role_loop<T, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
 }
 
 // ================================================================================================
@@ -406,24 +412,19 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
   static int ctas_per_sm = 0, n_sm = 0;
   const int smem = (int)sizeof(AsmSmem<T>);
   if (!ctas_per_sm) {
-    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int dev = 0, occ = 0;
     TFA_CUDA(cudaGetDevice(&dev));
     TFA_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, true>, C::NT, smem));
+    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T>, C::NT, smem));
     if (occ < 1) return set_error(TFA_ECUDA, "k_assemble does not fit on an SM");
     ctas_per_sm = occ;
   }
   const int64_t ntiles = (m.nc + T - 1) / T;
   const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)n_sm * ctas_per_sm);
   const double inv2dt = 1.0 / (2.0 * dt);
-  if (vals)
-    k_assemble<T, true><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, lgrad, m.cgeo.p,
-                                                   m.cell_nbr.p, m.blk4.p, rhs, vals, flags);
-  else
-    k_assemble<T, false><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, lgrad, m.cgeo.p,
-                                                    m.cell_nbr.p, m.blk4.p, rhs, vals, flags);
+  k_assemble<T><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, lgrad, m.cgeo.p, m.cell_nbr.p,
+                                           m.blk4.p, rhs, vals, flags);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
