@@ -19,8 +19,14 @@
 //    source (Eq. 4/6) couples the blocks on the diagonal block only.
 //  * 18x18 blocks are staged in shared memory (their structural zeros are written once per CTA)
 //    and leave the SM as 2592-byte TMA bulk stores (cp.async.bulk.global.shared::cta).
+#include <cstdlib>
+
 #include "tfa_common.cuh"
 #include "tfa_physics.cuh"
+
+#ifndef TFA_ASM_NM
+#define TFA_ASM_NM 3   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
+#endif
 
 namespace tfa {
 
@@ -40,6 +46,8 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // CTA barrier reached from role-specialised code (every warp executes the same number of them)
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
+// pull one 128-byte line towards L2 ahead of use (read latency under the Jacobian's write stream is long)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ------------------------------------------------------------------------------------------------
 template <int T>
@@ -50,10 +58,10 @@ struct AsmCfg {
   static constexpr int NT = 32 * (AW + MW);
 };
 
-template <int T>
+template <int T, int NM>
 struct __align__(128) AsmSmem {
-  double mir[T][BLK];    // staged mirror block (j,i) of the current face; structural zeros persist
-  double diag[T][BLK];   // staged diagonal block (i,i); structural zeros persist
+  double mir[NM][T][BLK];  // staged mirror blocks (j,i), face k in buffer k % NM; structural zeros persist
+  double diag[T][BLK];     // staged diagonal block (i,i); structural zeros persist
   double rs[T][NEQ];     // non-flux part of R~: Omega (BDF2 term) - Omega S
   double s0[T][8];       // Lorentz-force and Joule-heating rows of S(P_i): equations 10..17
 };
@@ -90,8 +98,8 @@ __device__ __forceinline__ void cons5(double cv, const double* Q, double* U) {
 // Non-flux part of the residual of one (cell, group): source (Alg. 1) and BDF2 term (Eq. 13).
 // grp 0 = field rows 0..7, 1 = ion rows, 2 = electron rows.  Writes S.rs (all rows) and S.s0.
 // ------------------------------------------------------------------------------------------------
-template <int T>
-__device__ __forceinline__ void cell_group_rest(AsmSmem<T>& S, const Consts& K, int c, int grp, int64_t i,
+template <int T, int NM>
+__device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts& K, int c, int grp, int64_t i,
                                                 const double* __restrict__ state,
                                                 const double* __restrict__ state_n,
                                                 const double* __restrict__ state_nm1, double vol, double inv2dt) {
@@ -149,8 +157,8 @@ __device__ __forceinline__ void cell_group_rest(AsmSmem<T>& S, const Consts& K, 
 // ------------------------------------------------------------------------------------------------
 // The tile loop of one warp role.  All roles execute the same sequence of CTA barriers.
 // ------------------------------------------------------------------------------------------------
-template <int T, int ROLE>
-__device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const int64_t nc, const Consts& K,
+template <int T, int NM, int ROLE>
+__device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, const int64_t nc, const Consts& K,
                                           const double* __restrict__ state, const double* __restrict__ state_n,
                                           const double* __restrict__ state_nm1, const double inv2dt,
                                           const double* __restrict__ lgrad, const double* __restrict__ cgeo,
@@ -175,6 +183,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
   const int pj = p - 1;   // perturbed variable of the group; -1 on the base lane
   const int v = ROLE == 2 ? max(pj, 0) : (pj <= 0 ? 8 + ROLE : (pj == 4 ? 16 + ROLE : 9 + 3 * ROLE + pj));
   const bool run = do_flux && (JAC || !pert);
+  const double pm = pert ? 1.0 : 0.0;
   bool nonphys = false;
 
 #pragma unroll 1
@@ -192,8 +201,46 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
       const int q = tid - (C::NT - 3 * T);
       const int c = q / 3, grp = q - 3 * c;
       if (c < ncell)
-        cell_group_rest<T>(S, K, c, grp, cell0 + c, state, state_n, state_nm1, cgeo[CGEO * (cell0 + c) + 7], inv2dt);
+        cell_group_rest<T, NM>(S, K, c, grp, cell0 + c, state, state_n, state_nm1, cgeo[CGEO * (cell0 + c) + 7], inv2dt);
     }
+    // the next tile of this CTA: pull its cell records towards L2 now, its neighbours' later
+    const int64_t cellN = cell0 + (int64_t)gridDim.x * T;
+    if (cellN < nc) {
+      const int nN = (int)min((int64_t)T, nc - cellN);
+      if (tid < 104) {
+        // region r of [state, state_n, state_nm1 | lgrad | cgeo | cell_nbr, blk4], line l of it
+        const char* base;
+        int l, bytes;
+        if (tid < 39) {
+          const int r = tid / 13;
+          l = tid - 13 * r;
+          base = reinterpret_cast<const char*>((r == 0 ? state : (r == 1 ? state_n : state_nm1)) + NEQ * cellN);
+          bytes = nN * NEQ * 8;
+        } else if (tid < 63) {
+          l = tid - 39;
+          base = reinterpret_cast<const char*>(lgrad + 2 * NEQ * cellN);
+          bytes = nN * NEQ * 16;
+        } else if (tid < 79) {
+          l = tid - 63;
+          base = reinterpret_cast<const char*>(cgeo + CGEO * cellN);
+          bytes = nN * CGEO * 8;
+        } else if (tid < 81) {
+          l = tid - 79;
+          base = reinterpret_cast<const char*>(cell_nbr + 3 * cellN);
+          bytes = nN * 12;
+        } else {
+          l = tid - 81;
+          base = reinterpret_cast<const char*>(blk4 + 4 * cellN);
+          bytes = nN * 16;
+        }
+        if (l * 128 < bytes + 127 && tid < 84) prefetch_l2(base + min(l * 128, bytes - 1));
+      }
+    }
+    int32_t nbN = -1;   // neighbour (cell, face) = lane of the next tile, held by the last warp
+    if (ROLE == 2 && warp == C::AW + C::MW - 1 && cellN < nc && lane < 3 * (int)min((int64_t)T, nc - cellN))
+      nbN = cell_nbr[3 * cellN + lane];
+    const int32_t nb0 = cell_nbr[3 * i], nb1 = cell_nbr[3 * i + 1], nb2 = cell_nbr[3 * i + 2];
+
     // where this tile's blocks go: thread t < ncell issues the bulk stores of cell t
     int4 b4 = make_int4(-1, -1, -1, -1);
     if (ROLE == 0 && JAC && tid < ncell) b4 = *reinterpret_cast<const int4*>(blk4 + 4 * (cell0 + tid));
@@ -204,6 +251,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
     const double eps = tv - Pcv;
     const double inv_e = 1.0 / eps;
 
+    // own cell-centre values of the group, this lane's perturbation folded in (Alg. 1)
+    double pc[NV];
+#pragma unroll
+    for (int q = 0; q < NV; ++q) pc[q] = q == pj ? tv : sO[vidx<ROLE>(q)];
+
     double acc[NV];   // base lane: residual rows; perturbed lane: its column of the diagonal block
 #pragma unroll
     for (int q = 0; q < NV; ++q) acc[q] = 0.0;
@@ -211,36 +263,36 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
     // ---- faces (Alg. 1) ----
 #pragma unroll 1
     for (int k = 0; k < 3; ++k) {
-      const int32_t j = cell_nbr[3 * i + k];
-      const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);       // canonical unit normal
+      const int32_t j = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);
+      const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);       // outward unit normal
       const double2 g23 = *reinterpret_cast<const double2*>(cg + 8 * k + 2);   // Sigma_f, x_f - x_i (x)
       const double2 g45 = *reinterpret_cast<const double2*>(cg + 8 * k + 4);   // x_f - x_i (y), x_f - x_j (x)
-      const double dyn = cg[8 * k + 6];
+      const double dyx = cg[8 * k + 6];                                        // x_f - x_j (y)
       const bool bnd = j < 0;
-      const bool own_is_L = bnd || i < (int64_t)j;
-      const double nx = own_is_L ? g01.x : -g01.x, ny = own_is_L ? g01.y : -g01.y;   // outward normal
-      const double len = g23.x, dxo = g23.y, dyo = g45.x;
-      const double dxx = bnd ? dxo : g45.y, dyx = bnd ? dyo : dyn;   // boundary: P_R := P_L (S9)
+      const double nx = g01.x, ny = g01.y, len = g23.x, dxo = g23.y, dyo = g45.x, dxx = g45.y;
       const int64_t X = bnd ? i : (int64_t)j;
       const double* __restrict__ sX = state + NEQ * X;
       const double2* __restrict__ gX = reinterpret_cast<const double2*>(lgrad) + NEQ * X;
 
+      const bool any_bnd = __any_sync(0xffffffffu, bnd);   // warp-uniform; boundary faces are rare
       double H[NV];
       if (run) {
-        // face states: own side and the other side (L232); the perturbed variable enters at the
+        // face states: own side and the other side (L232); the perturbed variable entered at the
         // cell centre and is re-extrapolated with the frozen limited gradient (L236-237; S8)
         double own[NV], oth[NV];
 #pragma unroll
         for (int q = 0; q < NV; ++q) {
           const int ix = vidx<ROLE>(q);
-          double po = sO[ix], px = sX[ix];
           const double2 go = gO[ix], gx = gX[ix];
-          if (q == pj) {
-            po = tv;
-            if (bnd) px = tv;   // boundary: the perturbation moves both arguments (S9)
+          own[q] = pc[q] + (go.x * dxo + go.y * dyo);
+          oth[q] = sX[ix] + (gx.x * dxx + gx.y * dyx);
+        }
+        if (any_bnd) {
+          // boundary face: P_R := P_L, so the perturbation moves both arguments (S9)
+          if (bnd) {
+#pragma unroll
+            for (int q = 0; q < NV; ++q) oth[q] = own[q];
           }
-          own[q] = po + (go.x * dxo + go.y * dyo);
-          oth[q] = px + (gx.x * dxx + gx.y * dyx);
         }
         if (ROLE == 2) {
           maxwell_flux(K, own, oth, nx, ny, H);
@@ -257,32 +309,35 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         const double hb = __shfl_sync(0xffffffffu, H[q], base_lane);
-        // explicit rounding: the residual must not depend on JAC through FMA contraction
-        d[q] = __dmul_rn(pert ? H[q] - hb : H[q], f);
+        // perturbed lane: (H_pert - H) Sigma_f / eps; base lane: H Sigma_f  (pm = 1 or 0, exact)
+        d[q] = __dmul_rn(__fma_rn(-hb, pm, H[q]), f);
         acc[q] = __dadd_rn(acc[q], d[q]);
       }
-      if (!JAC) continue;
-      // the staging of the previous face / tile has been read by the TMA
-      if (ROLE == 0 && tid < T) bulk_wait_read();
-      cta_sync();   // B1
-      if (pert && act && !bnd) {
-#pragma unroll
-        for (int q = 0; q < NV; ++q) S.mir[cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
+      if (k == 0 || k >= NM) {
+        // buffer k % NM is free: its last bulk store (previous tile / face k - NM) has read it.
+        // At k == 0 this barrier also publishes S.rs / S.s0 of the tile.
+        if (ROLE == 0 && tid < T) bulk_wait_read();
+        cta_sync();
       }
-      fence_async_smem();
-      cta_sync();   // B2
-      // a7: the block (j,i) leaves the SM as one 2592-byte bulk store
-      if (ROLE == 0 && tid < ncell) {
-        const int32_t b = k == 0 ? b4.y : (k == 1 ? b4.z : b4.w);
-        if (b >= 0) {
-          bulk_store(vals + (int64_t)b * BLK, &S.mir[tid][0], BLK * 8);
-          bulk_commit();
+      if (JAC && pert && act && !bnd) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) S.mir[k % NM][cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
+      }
+      if (k + NM < 3) {
+        // the buffer is needed again by face k + NM: this face's blocks leave now
+        fence_async_smem();
+        cta_sync();
+        if (ROLE == 0 && JAC && tid < ncell) {
+          const int32_t b = k == 0 ? b4.y : b4.z;
+          if (b >= 0) {
+            bulk_store(vals + (int64_t)b * BLK, &S.mir[k % NM][tid][0], BLK * 8);
+            bulk_commit();
+          }
         }
       }
     }
 
     // ---- residual, source Jacobian (L245-253), BDF2 diagonal (Eq. 13), diagonal block ----
-    if (!JAC) cta_sync();   // S.rs of this tile is complete
     if (act && !pert) {
 #pragma unroll
       for (int q = 0; q < NV; ++q) rhs[NEQ * i + vidx<ROLE>(q)] = -(acc[q] + S.rs[cl][vidx<ROLE>(q)]);
@@ -323,8 +378,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
           double Q[5], Qp[5], E[3], B[3];
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            Q[q] = sO[vidx<ROLE>(q)];
-            Qp[q] = q == pj ? tv : Q[q];
+            Qp[q] = pc[q];
+            Q[q] = q == pj ? Pcv : pc[q];
           }
 #pragma unroll
           for (int r = 0; r < 3; ++r) { B[r] = sO[r]; E[r] = sO[3 + r]; }
@@ -364,19 +419,33 @@ __device__ __forceinline__ void role_loop(AsmSmem<T>& S, const bool JAC, const i
           S.diag[cl][7 * NEQ + v] = do_src ? -K.c2 * (qnp - qn) * fs : 0.0;
         }
       }
-      fence_async_smem();
-      cta_sync();   // B3
-      if (ROLE == 0 && tid < ncell) {
-        bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[tid][0], BLK * 8);
-        bulk_commit();
-      }
+    }
+    if (nbN >= 0) {
+      // the records the next tile reads across its faces: 144 B of state (2 lines), 288 B of gradient (3)
+      const char* ps = reinterpret_cast<const char*>(state + NEQ * (int64_t)nbN);
+      const char* pg = reinterpret_cast<const char*>(lgrad + 2 * NEQ * (int64_t)nbN);
+      prefetch_l2(ps);
+      prefetch_l2(ps + 143);
+      prefetch_l2(pg);
+      prefetch_l2(pg + 128);
+      prefetch_l2(pg + 287);
+    }
+    fence_async_smem();
+    cta_sync();   // B: every block of the tile is staged
+    // a7: each block leaves the SM as one 2592-byte bulk store
+    if (ROLE == 0 && JAC && tid < ncell) {
+      bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[tid][0], BLK * 8);
+      if (NM >= 3 && b4.y >= 0) bulk_store(vals + (int64_t)b4.y * BLK, &S.mir[0][tid][0], BLK * 8);
+      if (NM >= 2 && b4.z >= 0) bulk_store(vals + (int64_t)b4.z * BLK, &S.mir[1 % NM][tid][0], BLK * 8);
+      if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[2 % NM][tid][0], BLK * 8);
+      bulk_commit();
     }
   }
   if (ROLE == 0 && JAC && tid < T) bulk_wait_all();
   if (nonphys) atomicAdd(flags, 1);
 }
 
-template <int T>
+template <int T, int NM>
 __global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
@@ -385,48 +454,64 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
     int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  AsmSmem<T>& S = *reinterpret_cast<AsmSmem<T>*>(smem_raw);
+  AsmSmem<T, NM>& S = *reinterpret_cast<AsmSmem<T, NM>*>(smem_raw);
   // one instantiation serves both calls, so that the residual does not depend on whether the
   // Jacobian is asked for (same instructions on the base lanes)
   const bool JAC = vals != nullptr;
   if (JAC) {
-    for (int q = threadIdx.x; q < 2 * T * BLK; q += C::NT) (&S.mir[0][0])[q] = 0.0;   // mir and diag
+    for (int q = threadIdx.x; q < (NM + 1) * T * BLK; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;   // mir and diag
     __syncthreads();
   }
   const int warp = threadIdx.x >> 5;
   if (warp >= C::AW)
-    role_loop<T, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+    role_loop<T, NM, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
   else if (warp & 1)
-    role_loop<T, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+    role_loop<T, NM, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
   else
-    role_loop<T, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+    role_loop<T, NM, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
 }
 
 // ================================================================================================
-int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-                    const double* state_nm1, double dt, const double* lgrad, double* rhs, double* vals,
-                    int32_t* flags, cudaStream_t st) {
-  if (m.nc == 0) return 0;
-  constexpr int T = 10;
+namespace {
+template <int T, int NM>
+int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
+              const double* state_nm1, double dt, const double* lgrad, double* rhs, double* vals, int32_t* flags,
+              cudaStream_t st) {
   using C = AsmCfg<T>;
   static int ctas_per_sm = 0, n_sm = 0;
-  const int smem = (int)sizeof(AsmSmem<T>);
+  const int smem = (int)sizeof(AsmSmem<T, NM>);
   if (!ctas_per_sm) {
-    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int dev = 0, occ = 0;
     TFA_CUDA(cudaGetDevice(&dev));
     TFA_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T>, C::NT, smem));
+    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, NM>, C::NT, smem));
     if (occ < 1) return set_error(TFA_ECUDA, "k_assemble does not fit on an SM");
     ctas_per_sm = occ;
   }
   const int64_t ntiles = (m.nc + T - 1) / T;
   const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)n_sm * ctas_per_sm);
   const double inv2dt = 1.0 / (2.0 * dt);
-  k_assemble<T><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, lgrad, m.cgeo.p, m.cell_nbr.p,
-                                           m.blk4.p, rhs, vals, flags);
+  k_assemble<T, NM><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, lgrad, m.cgeo.p,
+                                               m.cell_nbr.p, m.blk4.p, rhs, vals, flags);
   TFA_CUDA(cudaGetLastError());
   return 0;
+}
+}  // namespace
+
+int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
+                    const double* state_nm1, double dt, const double* lgrad, double* rhs, double* vals,
+                    int32_t* flags, cudaStream_t st) {
+  if (m.nc == 0) return 0;
+  // TFA_ASM_NM in the environment overrides the compiled-in staging depth (tuning sweeps only)
+  static const int nm = [] {
+    const char* e = getenv("TFA_ASM_NM");
+    const int x = e ? atoi(e) : TFA_ASM_NM;
+    return x >= 1 && x <= 3 ? x : TFA_ASM_NM;
+  }();
+  if (nm == 1) return launch_nm<10, 1>(m, K, state, state_n, state_nm1, dt, lgrad, rhs, vals, flags, st);
+  if (nm == 2) return launch_nm<10, 2>(m, K, state, state_n, state_nm1, dt, lgrad, rhs, vals, flags, st);
+  return launch_nm<10, 3>(m, K, state, state_n, state_nm1, dt, lgrad, rhs, vals, flags, st);
 }
 
 }  // namespace tfa

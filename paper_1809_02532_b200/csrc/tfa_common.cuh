@@ -32,10 +32,12 @@ inline unsigned cdiv(int64_t a, int64_t b) { return (unsigned)((a + b - 1) / b);
 
 // Per-cell geometry record, 24 doubles = 192 B:
 //   for local face k = 0..2 at [8k .. 8k+7]:
-//     0 nx, 1 ny   unit normal in CANONICAL orientation (from the face's L cell towards R)
+//     0 nx, 1 ny   unit normal pointing OUT of this cell: the face's normal, computed from its L
+//                  cell's corners (S10), with the sign flipped when this cell is the face's R cell
 //     2 len        face length Sigma_f
 //     3 dxo, 4 dyo face midpoint minus OWN centroid (own corner coordinates)
-//     5 dxn, 6 dyn face midpoint minus NEIGHBOUR centroid (neighbour's corner coordinates)
+//     5 dxn, 6 dyn face midpoint minus NEIGHBOUR centroid (neighbour's corner coordinates);
+//                  on a boundary face the own-side values again (P_R := P_L, S9)
 //     7 extra      k=0: volume Omega_i;  k=1: sqrt(Omega_i);  k=2: unused (0)
 constexpr int CGEO = 24;
 

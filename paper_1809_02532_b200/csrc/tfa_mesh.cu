@@ -262,7 +262,7 @@ __global__ void k_blk4(int64_t nc, const int32_t* __restrict__ cell_nbr, const i
   }
 }
 
-// ---- per-cell geometry record in canonical face orientation (tfa_common.cuh CGEO) ----
+// ---- per-cell geometry record, face normals pointing out of the cell (tfa_common.cuh CGEO) ----
 __global__ void k_cgeo(int64_t nc, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ cell_faces,
                        const double* __restrict__ vol, const double* __restrict__ olen,
                        const double* __restrict__ onrm, const double* __restrict__ ooff,
@@ -281,13 +281,15 @@ __global__ void k_cgeo(int64_t nc, const int32_t* __restrict__ cell_nbr, const i
     const bool own_is_L = (j < 0) || (i < j);
     const int64_t cL = own_is_L ? i : j;
     const int kL = own_is_L ? k : kj;
-    g[8 * k + 0] = onrm[6 * cL + 2 * kL];
-    g[8 * k + 1] = onrm[6 * cL + 2 * kL + 1];
+    // the face's normal is its L cell's (S10); seen from the R cell it is exactly minus that
+    g[8 * k + 0] = own_is_L ? onrm[6 * cL + 2 * kL] : -onrm[6 * cL + 2 * kL];
+    g[8 * k + 1] = own_is_L ? onrm[6 * cL + 2 * kL + 1] : -onrm[6 * cL + 2 * kL + 1];
     g[8 * k + 2] = olen[3 * cL + kL];
     g[8 * k + 3] = ooff[6 * i + 2 * k];
     g[8 * k + 4] = ooff[6 * i + 2 * k + 1];
-    g[8 * k + 5] = j >= 0 ? ooff[6 * j + 2 * kj] : 0.0;
-    g[8 * k + 6] = j >= 0 ? ooff[6 * j + 2 * kj + 1] : 0.0;
+    // boundary face: the other side is the cell itself (P_R := P_L, S9)
+    g[8 * k + 5] = j >= 0 ? ooff[6 * j + 2 * kj] : ooff[6 * i + 2 * k];
+    g[8 * k + 6] = j >= 0 ? ooff[6 * j + 2 * kj + 1] : ooff[6 * i + 2 * k + 1];
   }
   g[7] = vol[i];
   g[15] = sqrt(vol[i]);
