@@ -6,17 +6,17 @@
 
 namespace tfa {
 int launch_lsq_coef(const tfa_mesh& m, double power, double* coef, cudaStream_t st);
-int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* lgrad,
+int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* fown,
                     double* grad, double* phi, cudaStream_t st);
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-                    const double* state_nm1, double dt, const double* lgrad, double* rhs, double* vals,
+                    const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
                     int32_t* flags, cudaStream_t st);
 int launch_probe_dfma(int grid, int iters, double* sink, cudaStream_t st);
 int launch_probe_copy(const double* src, double* dst, int64_t n, cudaStream_t st);
 
 namespace {
 
-// (re)build the per-mesh workspace: LS coefficients and the limited-gradient buffer
+// (re)build the per-mesh workspace: LS coefficients and the face-state buffer
 int prepare(tfa_ctx* ctx, const tfa_mesh* m, cudaStream_t st) {
   if (!ctx->flags.p) {
     TFA_CUDA(ctx->flags.alloc(4));
@@ -25,7 +25,7 @@ int prepare(tfa_ctx* ctx, const tfa_mesh* m, cudaStream_t st) {
   if (ctx->ws_mesh == m && ctx->ws_generation == m->generation && ctx->ws_power == ctx->nu.lsq_weight_power)
     return 0;
   TFA_CUDA(ctx->lsq_coef.alloc(2 * m->nst));
-  TFA_CUDA(ctx->lgrad.alloc(2 * NEQ * m->nc));
+  TFA_CUDA(ctx->fown.alloc(3 * NEQ * m->nc));
   TFA_TRY(launch_lsq_coef(*m, ctx->nu.lsq_weight_power, ctx->lsq_coef.p, st));
   ctx->ws_mesh = m;
   ctx->ws_generation = m->generation;
@@ -123,9 +123,9 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
       if (!ev[q]) TFA_CUDA(cudaEventCreate(&ev[q]));
     TFA_CUDA(cudaEventRecord(ev[0], st));
   }
-  TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->lgrad.p, nullptr, nullptr, st));
+  TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
-  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->lgrad.p, rhs, bsr_vals, ctx->flags.p, st));
+  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, rhs, bsr_vals, ctx->flags.p, st));
   if (ev) {
     TFA_CUDA(cudaEventRecord(ev[2], st));
     ++ctx->timed;

@@ -13,9 +13,9 @@
 //    instead of Alg. 1's 3*19 = 57 full ones.
 //  * Lanes: an AUSM warp holds 5 groups of 6 lanes = (cell, species) x {base, 5 perturbed variables}
 //    (Eq. 10); a Maxwell warp holds 3 groups of 9 lanes = cell x {base, 8 perturbed} (Eq. 9
-//    L91).  Each lane reconstructs the face states it needs itself (L232: P + phi grad P . dx) from
-//    the cell records (L1/L2 hits; every lane of a group reads the same addresses), the base flux
-//    reaches the group by warp shuffle; the flux Jacobian is block diagonal (8x8, 5x5, 5x5), the
+//    L91).  The reconstructed face states (L232: P + phi grad P . dx) of both sides come from the
+//    gradient kernel's face-state array (every lane of a group reads the same addresses; the
+//    perturbation is added to the own-side value), the base flux reaches the group by warp shuffle; the flux Jacobian is block diagonal (8x8, 5x5, 5x5), the
 //    source (Eq. 4/6) couples the blocks on the diagonal block only.
 //  * 18x18 blocks are staged in shared memory (their structural zeros are written once per CTA)
 //    and leave the SM as 2592-byte TMA bulk stores (cp.async.bulk.global.shared::cta).
@@ -161,8 +161,8 @@ template <int T, int NM, int ROLE>
 __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, const int64_t nc, const Consts& K,
                                           const double* __restrict__ state, const double* __restrict__ state_n,
                                           const double* __restrict__ state_nm1, const double inv2dt,
-                                          const double* __restrict__ lgrad, const double* __restrict__ cgeo,
-                                          const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ blk4,
+                                          const double* __restrict__ fown, const double* __restrict__ cgeo,
+                                          const int32_t* __restrict__ nbrf, const int32_t* __restrict__ blk4,
                                           double* __restrict__ rhs, double* __restrict__ vals,
                                           int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
@@ -194,7 +194,6 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     const int64_t i = cell0 + (act ? cl : 0);
     const double* __restrict__ cg = cgeo + CGEO * i;
     const double* __restrict__ sO = state + NEQ * i;
-    const double2* __restrict__ gO = reinterpret_cast<const double2*>(lgrad) + NEQ * i;
 
     // ---- the non-flux part of the residual, one thread per (cell, group) ----
     if (ROLE == 2 && tid >= C::NT - 3 * T) {
@@ -207,8 +206,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     const int64_t cellN = cell0 + (int64_t)gridDim.x * T;
     if (cellN < nc) {
       const int nN = (int)min((int64_t)T, nc - cellN);
-      if (tid < 104) {
-        // region r of [state, state_n, state_nm1 | lgrad | cgeo | cell_nbr, blk4], line l of it
+      if (warp < 3) {
+        // line l of region [state, state_n, state_nm1 | face states | geometry | neighbours | block map]
         const char* base;
         int l, bytes;
         if (tid < 39) {
@@ -216,30 +215,30 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
           l = tid - 13 * r;
           base = reinterpret_cast<const char*>((r == 0 ? state : (r == 1 ? state_n : state_nm1)) + NEQ * cellN);
           bytes = nN * NEQ * 8;
-        } else if (tid < 63) {
+        } else if (tid < 74) {
           l = tid - 39;
-          base = reinterpret_cast<const char*>(lgrad + 2 * NEQ * cellN);
-          bytes = nN * NEQ * 16;
-        } else if (tid < 79) {
-          l = tid - 63;
+          base = reinterpret_cast<const char*>(fown + 3 * NEQ * cellN);
+          bytes = nN * 3 * NEQ * 8;
+        } else if (tid < 90) {
+          l = tid - 74;
           base = reinterpret_cast<const char*>(cgeo + CGEO * cellN);
           bytes = nN * CGEO * 8;
-        } else if (tid < 81) {
-          l = tid - 79;
-          base = reinterpret_cast<const char*>(cell_nbr + 3 * cellN);
+        } else if (tid < 92) {
+          l = tid - 90;
+          base = reinterpret_cast<const char*>(nbrf + 3 * cellN);
           bytes = nN * 12;
         } else {
-          l = tid - 81;
+          l = tid - 92;
           base = reinterpret_cast<const char*>(blk4 + 4 * cellN);
           bytes = nN * 16;
         }
-        if (l * 128 < bytes + 127 && tid < 84) prefetch_l2(base + min(l * 128, bytes - 1));
+        if (l * 128 < bytes + 127 && tid < 95) prefetch_l2(base + min(l * 128, bytes - 1));
       }
     }
     int32_t nbN = -1;   // neighbour (cell, face) = lane of the next tile, held by the last warp
     if (ROLE == 2 && warp == C::AW + C::MW - 1 && cellN < nc && lane < 3 * (int)min((int64_t)T, nc - cellN))
-      nbN = cell_nbr[3 * cellN + lane];
-    const int32_t nb0 = cell_nbr[3 * i], nb1 = cell_nbr[3 * i + 1], nb2 = cell_nbr[3 * i + 2];
+      nbN = nbrf[3 * cellN + lane];
+    const int32_t nb0 = nbrf[3 * i], nb1 = nbrf[3 * i + 1], nb2 = nbrf[3 * i + 2];
 
     // where this tile's blocks go: thread t < ncell issues the bulk stores of cell t
     int4 b4 = make_int4(-1, -1, -1, -1);
@@ -251,10 +250,10 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     const double eps = tv - Pcv;
     const double inv_e = 1.0 / eps;
 
-    // own cell-centre values of the group, this lane's perturbation folded in (Alg. 1)
-    double pc[NV];
+    // this lane's perturbation of the group's variables (Alg. 1): eps on its own one, 0 elsewhere
+    double me[NV];
 #pragma unroll
-    for (int q = 0; q < NV; ++q) pc[q] = q == pj ? tv : sO[vidx<ROLE>(q)];
+    for (int q = 0; q < NV; ++q) me[q] = q == pj ? eps : 0.0;
 
     double acc[NV];   // base lane: residual rows; perturbed lane: its column of the diagonal block
 #pragma unroll
@@ -263,29 +262,37 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     // ---- faces (Alg. 1) ----
 #pragma unroll 1
     for (int k = 0; k < 3; ++k) {
-      const int32_t j = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);
-      const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);       // outward unit normal
-      const double2 g23 = *reinterpret_cast<const double2*>(cg + 8 * k + 2);   // Sigma_f, x_f - x_i (x)
-      const double2 g45 = *reinterpret_cast<const double2*>(cg + 8 * k + 4);   // x_f - x_i (y), x_f - x_j (x)
-      const double dyx = cg[8 * k + 6];                                        // x_f - x_j (y)
-      const bool bnd = j < 0;
-      const double nx = g01.x, ny = g01.y, len = g23.x, dxo = g23.y, dyo = g45.x, dxx = g45.y;
-      const int64_t X = bnd ? i : (int64_t)j;
-      const double* __restrict__ sX = state + NEQ * X;
-      const double2* __restrict__ gX = reinterpret_cast<const double2*>(lgrad) + NEQ * X;
+      const int32_t nf = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);   // 4 * neighbour + its local face, or -1
+      const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);   // outward unit normal
+      const double len = cg[8 * k + 2];                                    // Sigma_f
+      const bool bnd = nf < 0;
+      const double nx = g01.x, ny = g01.y;
+      // own-side and other-side face states of this face (L232), written by k_gradient_limiter
+      const double* __restrict__ fo = fown + (3 * i + k) * NEQ;
+      const double* __restrict__ fx = bnd ? fo : fown + (3 * (int64_t)(nf >> 2) + (nf & 3)) * NEQ;
 
       const bool any_bnd = __any_sync(0xffffffffu, bnd);   // warp-uniform; boundary faces are rare
       double H[NV];
       if (run) {
-        // face states: own side and the other side (L232); the perturbed variable entered at the
-        // cell centre and is re-extrapolated with the frozen limited gradient (L236-237; S8)
+        // the perturbed variable enters at the cell centre and is re-extrapolated with the frozen
+        // limited gradient (L236-237; S8): (P + eps) + phi grad P . dx = face state + eps
         double own[NV], oth[NV];
+        if (ROLE == 2) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) {
-          const int ix = vidx<ROLE>(q);
-          const double2 go = gO[ix], gx = gX[ix];
-          own[q] = pc[q] + (go.x * dxo + go.y * dyo);
-          oth[q] = sX[ix] + (gx.x * dxx + gx.y * dyx);
+          for (int q = 0; q < NV; q += 2) {
+            const double2 o2 = *reinterpret_cast<const double2*>(fo + q);
+            const double2 x2 = *reinterpret_cast<const double2*>(fx + q);
+            own[q] = o2.x + me[q];
+            own[q + 1] = o2.y + me[q + 1];
+            oth[q] = x2.x;
+            oth[q + 1] = x2.y;
+          }
+        } else {
+#pragma unroll
+          for (int q = 0; q < NV; ++q) {
+            own[q] = fo[vidx<ROLE>(q)] + me[q];
+            oth[q] = fx[vidx<ROLE>(q)];
+          }
         }
         if (any_bnd) {
           // boundary face: P_R := P_L, so the perturbation moves both arguments (S9)
@@ -378,8 +385,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
           double Q[5], Qp[5], E[3], B[3];
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            Qp[q] = pc[q];
-            Q[q] = q == pj ? Pcv : pc[q];
+            Q[q] = sO[vidx<ROLE>(q)];
+            Qp[q] = q == pj ? tv : Q[q];
           }
 #pragma unroll
           for (int r = 0; r < 3; ++r) { B[r] = sO[r]; E[r] = sO[3 + r]; }
@@ -421,14 +428,10 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
       }
     }
     if (nbN >= 0) {
-      // the records the next tile reads across its faces: 144 B of state (2 lines), 288 B of gradient (3)
-      const char* ps = reinterpret_cast<const char*>(state + NEQ * (int64_t)nbN);
-      const char* pg = reinterpret_cast<const char*>(lgrad + 2 * NEQ * (int64_t)nbN);
-      prefetch_l2(ps);
-      prefetch_l2(ps + 143);
-      prefetch_l2(pg);
-      prefetch_l2(pg + 128);
-      prefetch_l2(pg + 287);
+      // the other-side face states the next tile reads: one 144-byte row (2 lines) per face
+      const char* px = reinterpret_cast<const char*>(fown + (3 * (int64_t)(nbN >> 2) + (nbN & 3)) * NEQ);
+      prefetch_l2(px);
+      prefetch_l2(px + 143);
     }
     fence_async_smem();
     cta_sync();   // B: every block of the tile is staged
@@ -449,7 +452,7 @@ template <int T, int NM>
 __global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
-    const double* __restrict__ lgrad, const double* __restrict__ cgeo, const int32_t* __restrict__ cell_nbr,
+    const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
     const int32_t* __restrict__ blk4, double* __restrict__ rhs, double* __restrict__ vals,
     int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
@@ -464,18 +467,18 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
   }
   const int warp = threadIdx.x >> 5;
   if (warp >= C::AW)
-    role_loop<T, NM, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+    role_loop<T, NM, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
   else if (warp & 1)
-    role_loop<T, NM, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+    role_loop<T, NM, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
   else
-    role_loop<T, NM, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, lgrad, cgeo, cell_nbr, blk4, rhs, vals, flags);
+    role_loop<T, NM, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
 }
 
 // ================================================================================================
 namespace {
 template <int T, int NM>
 int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-              const double* state_nm1, double dt, const double* lgrad, double* rhs, double* vals, int32_t* flags,
+              const double* state_nm1, double dt, const double* fown, double* rhs, double* vals, int32_t* flags,
               cudaStream_t st) {
   using C = AsmCfg<T>;
   static int ctas_per_sm = 0, n_sm = 0;
@@ -492,15 +495,15 @@ int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const dou
   const int64_t ntiles = (m.nc + T - 1) / T;
   const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)n_sm * ctas_per_sm);
   const double inv2dt = 1.0 / (2.0 * dt);
-  k_assemble<T, NM><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, lgrad, m.cgeo.p,
-                                               m.cell_nbr.p, m.blk4.p, rhs, vals, flags);
+  k_assemble<T, NM><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
+                                               m.nbrf.p, m.blk4.p, rhs, vals, flags);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
 }  // namespace
 
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-                    const double* state_nm1, double dt, const double* lgrad, double* rhs, double* vals,
+                    const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
                     int32_t* flags, cudaStream_t st) {
   if (m.nc == 0) return 0;
   // TFA_ASM_NM in the environment overrides the compiled-in staging depth (tuning sweeps only)
@@ -509,9 +512,9 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
     const int x = e ? atoi(e) : TFA_ASM_NM;
     return x >= 1 && x <= 3 ? x : TFA_ASM_NM;
   }();
-  if (nm == 1) return launch_nm<10, 1>(m, K, state, state_n, state_nm1, dt, lgrad, rhs, vals, flags, st);
-  if (nm == 2) return launch_nm<10, 2>(m, K, state, state_n, state_nm1, dt, lgrad, rhs, vals, flags, st);
-  return launch_nm<10, 3>(m, K, state, state_n, state_nm1, dt, lgrad, rhs, vals, flags, st);
+  if (nm == 1) return launch_nm<10, 1>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
+  if (nm == 2) return launch_nm<10, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
+  return launch_nm<10, 3>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
 }
 
 }  // namespace tfa

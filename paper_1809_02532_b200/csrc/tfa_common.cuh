@@ -79,6 +79,7 @@ struct tfa_mesh {
   // derived
   tfa::DevBuf<int32_t> face_nodes, face_cells;  // [nf][2]
   tfa::DevBuf<int32_t> cell_faces, cell_nbr;    // [nc][3]
+  tfa::DevBuf<int32_t> nbrf;                    // [nc][3] 4 * neighbour + its local face index, -1 on the boundary
   tfa::DevBuf<int32_t> st_ptr, st_idx;          // CSR stencil
   tfa::DevBuf<double> st_d;                     // [nst][2] centroid displacement (S9)
   tfa::DevBuf<int32_t> bsr_rowptr, bsr_col;
@@ -95,7 +96,7 @@ struct tfa_ctx {
   uint64_t ws_generation = 0;
   double ws_power = -1.0;
   tfa::DevBuf<double> lsq_coef;   // [nst][2]
-  tfa::DevBuf<double> lgrad;      // [nc][18][2] limited gradient phi*grad
+  tfa::DevBuf<double> fown;       // [nc][3][18] own-side face states P_i + phi grad P_i . (x_f - x_i)  (L232)
   tfa::DevBuf<int32_t> flags;     // [4] device counters: 0 = non-physical states
   // staging for tfa_assemble_host
   tfa::DevBuf<double> h_state[3], h_rhs, h_vals;

@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(GL_T) k_gradient_limiter(int64_t nc, const dou
                                                           const int32_t* __restrict__ st_idx,
                                                           const double* __restrict__ coef,
                                                           const double* __restrict__ cgeo, double venkK,
-                                                          double* __restrict__ lgrad, double* __restrict__ grad_out,
+                                                          double* __restrict__ fown, double* __restrict__ grad_out,
                                                           double* __restrict__ phi_out) {
   const int v = threadIdx.x % NEQ;
   const int64_t i = blockIdx.x * (int64_t)GL_CELLS + threadIdx.x / NEQ;
@@ -80,9 +80,11 @@ __global__ void __launch_bounds__(GL_T) k_gradient_limiter(int64_t nc, const dou
     phi = fmin(phi, pf);
   }
   phi = fmin(phi, 1.0);
-  if (lgrad) {
-    lgrad[2 * (NEQ * i + v)] = phi * gx;
-    lgrad[2 * (NEQ * i + v) + 1] = phi * gy;
+  if (fown) {
+    // own-side face states of the three faces (L232), the gradient limited once: phi grad P
+    const double lx = phi * gx, ly = phi * gy;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) fown[(3 * i + k) * NEQ + v] = Pi + (lx * g[8 * k + 3] + ly * g[8 * k + 4]);
   }
   if (grad_out) {
     grad_out[2 * (NEQ * i + v)] = gx;
@@ -122,11 +124,11 @@ int launch_lsq_coef(const tfa_mesh& m, double power, double* coef, cudaStream_t 
   return 0;
 }
 
-int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* lgrad,
+int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* fown,
                     double* grad, double* phi, cudaStream_t st) {
   if (m.nc == 0) return 0;
   k_gradient_limiter<<<cdiv(m.nc, GL_CELLS), GL_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
-                                                           venkK, lgrad, grad, phi);
+                                                           venkK, fown, grad, phi);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }

@@ -262,6 +262,24 @@ __global__ void k_blk4(int64_t nc, const int32_t* __restrict__ cell_nbr, const i
   }
 }
 
+// ---- for each local face k of cell i: 4 * neighbour + (the face's local index in the neighbour), -1 on the
+// boundary: the assembly reads the neighbour's face state of exactly that face ----
+__global__ void k_nbr_face(int64_t nc, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ cell_faces,
+                           int32_t* __restrict__ nbrf) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const int64_t j = cell_nbr[3 * i + k];
+    const int32_t f = cell_faces[3 * i + k];
+    int kj = 0;
+    if (j >= 0)
+      for (int q = 0; q < 3; ++q)
+        if (cell_faces[3 * j + q] == f) kj = q;
+    nbrf[3 * i + k] = j >= 0 ? (int32_t)(4 * j + kj) : -1;
+  }
+}
+
 // ---- per-cell geometry record, face normals pointing out of the cell (tfa_common.cuh CGEO) ----
 __global__ void k_cgeo(int64_t nc, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ cell_faces,
                        const double* __restrict__ vol, const double* __restrict__ olen,
@@ -505,7 +523,7 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
     TFA_CUDA(cudaMemsetAsync(m.st_ptr.p, 0, 4, st));
     TFA_CUDA(cudaMemsetAsync(m.bsr_rowptr.p, 0, 4, st));
     TFA_CUDA(m.face_nodes.alloc(0)); TFA_CUDA(m.face_cells.alloc(0)); TFA_CUDA(m.cell_faces.alloc(0));
-    TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
+    TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.nbrf.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
     TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0)); TFA_CUDA(m.blk4.alloc(0));
     ++m.generation;
     return 0;
@@ -594,6 +612,8 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
   }
   TFA_CUDA(m.cgeo.alloc(CGEO * nc));
   k_cgeo<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.cell_faces.p, vol.p, olen.p, onrm.p, ooff.p, m.cgeo.p);
+  TFA_CUDA(m.nbrf.alloc(3 * nc));
+  k_nbr_face<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.cell_faces.p, m.nbrf.p);
   TFA_CUDA(cudaGetLastError());
   TFA_CUDA(cudaStreamSynchronize(st));
   ++m.generation;
