@@ -25,7 +25,7 @@
 #include "tfa_physics.cuh"
 
 #ifndef TFA_ASM_NM
-#define TFA_ASM_NM 3   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
+#define TFA_ASM_NM 2   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
 #endif
 
 namespace tfa {
@@ -46,6 +46,31 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // CTA barrier reached from role-specialised code (every warp executes the same number of them)
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
+// ---- TMA bulk loads into shared memory, completion counted on an mbarrier (PTX ISA: mbarrier, cp.async.bulk) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t a = smem_u32(bar);
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(a), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void bulk_load(void* sdst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(sdst)),
+               "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
 // pull one 128-byte line towards L2 ahead of use (read latency under the Jacobian's write stream is long)
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
@@ -58,8 +83,22 @@ struct AsmCfg {
   static constexpr int NT = 32 * (AW + MW);
 };
 
+// Inputs of one tile, fetched by TMA one tile ahead (read latency under the Jacobian's write stream is
+// long): own-side and other-side face states of every (cell, face), geometry records, cell-centre states.
+template <int T>
+struct __align__(16) AsmIn {
+  double fx[T][3][NEQ];   // other side of face k of cell c (the cell's own row again on a boundary face)
+  double fo[T][3][NEQ];   // own side
+  double cg[T][CGEO];
+  double st[T][NEQ];
+  int32_t nf[T][3];       // 4 * neighbour + its local face, -1 on the boundary
+  int32_t pad_[2];
+};
+
 template <int T, int NM>
 struct __align__(128) AsmSmem {
+  AsmIn<T> in[2];
+  uint64_t full[2];        // mbarriers: stage s has landed
   double mir[NM][T][BLK];  // staged mirror blocks (j,i), face k in buffer k % NM; structural zeros persist
   double diag[T][BLK];     // staged diagonal block (i,i); structural zeros persist
   double rs[T][NEQ];     // non-flux part of R~: Omega (BDF2 term) - Omega S
@@ -100,11 +139,10 @@ __device__ __forceinline__ void cons5(double cv, const double* Q, double* U) {
 // ------------------------------------------------------------------------------------------------
 template <int T, int NM>
 __device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts& K, int c, int grp, int64_t i,
-                                                const double* __restrict__ state,
+                                                const double* __restrict__ P,
                                                 const double* __restrict__ state_n,
                                                 const double* __restrict__ state_nm1, double vol, double inv2dt) {
   const bool do_src = K.mask & 2, do_time = K.mask & 4;
-  const double* P = state + NEQ * i;
   const double ft = vol * inv2dt;
   if (grp == 0) {
     // S_E = -c^2 sum_s q_s n_s u_s, S_Phi = c^2 sum_s q_s n_s  (Eq. 4; eps0 = 1/c^2)
@@ -155,6 +193,27 @@ __device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts&
 }
 
 // ------------------------------------------------------------------------------------------------
+// One warp fetches the inputs of the tile starting at cell cellN (nN cells) into a stage: lane l < 3 nN
+// holds nfN = the packed neighbour of (cell, face) = l and copies that face's other-side row.
+// ------------------------------------------------------------------------------------------------
+template <int T>
+__device__ __forceinline__ void stage_inputs(AsmIn<T>& in, uint64_t* bar, int lane, int32_t nfN, int64_t cellN,
+                                             int nN, const double* __restrict__ state,
+                                             const double* __restrict__ fown, const double* __restrict__ cgeo) {
+  static_assert(3 * T <= 30, "one lane per (cell, face) plus two for the contiguous arrays");
+  if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)nN * (3 * NEQ * 8 + 3 * NEQ * 8 + CGEO * 8 + NEQ * 8));
+  if (lane < 3 * nN) {
+    // boundary face: the other side is the cell itself (P_R := P_L, S9)
+    const int64_t row = nfN < 0 ? 3 * cellN + lane : 3 * (int64_t)(nfN >> 2) + (nfN & 3);
+    bulk_load(&in.fx[0][0][0] + lane * NEQ, fown + row * NEQ, NEQ * 8, bar);
+    (&in.nf[0][0])[lane] = nfN;
+  }
+  if (lane == 30) bulk_load(&in.fo[0][0][0], fown + 3 * NEQ * cellN, (uint32_t)nN * 3 * NEQ * 8, bar);
+  if (lane == 31) bulk_load(&in.cg[0][0], cgeo + CGEO * cellN, (uint32_t)nN * CGEO * 8, bar);
+  if (lane == 0) bulk_load(&in.st[0][0], state + NEQ * cellN, (uint32_t)nN * NEQ * 8, bar);
+}
+
+// ------------------------------------------------------------------------------------------------
 // The tile loop of one warp role.  All roles execute the same sequence of CTA barriers.
 // ------------------------------------------------------------------------------------------------
 template <int T, int NM, int ROLE>
@@ -186,59 +245,53 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
   const double pm = pert ? 1.0 : 0.0;
   bool nonphys = false;
 
+  const bool loader = ROLE == 2 && warp == C::AW + C::MW - 1;   // the (lightly loaded) last warp fetches inputs
+  int it = 0;
 #pragma unroll 1
-  for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+  for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
     const int64_t cell0 = tile * T;
     const int ncell = (int)min((int64_t)T, nc - cell0);
     const bool act = lane_ok && cl < ncell;
-    const int64_t i = cell0 + (act ? cl : 0);
-    const double* __restrict__ cg = cgeo + CGEO * i;
-    const double* __restrict__ sO = state + NEQ * i;
+    const int ca = act ? cl : 0;
+    const int64_t i = cell0 + ca;
+    // this tile's inputs were requested one tile ago (kernel prologue for the first one)
+    const AsmIn<T>& in = S.in[it & 1];
+    mbar_wait(&S.full[it & 1], (it >> 1) & 1);
+    const double* __restrict__ cg = in.cg[ca];
+    const double* __restrict__ sO = in.st[ca];
 
     // ---- the non-flux part of the residual, one thread per (cell, group) ----
     if (ROLE == 2 && tid >= C::NT - 3 * T) {
       const int q = tid - (C::NT - 3 * T);
       const int c = q / 3, grp = q - 3 * c;
       if (c < ncell)
-        cell_group_rest<T, NM>(S, K, c, grp, cell0 + c, state, state_n, state_nm1, cgeo[CGEO * (cell0 + c) + 7], inv2dt);
+        cell_group_rest<T, NM>(S, K, c, grp, cell0 + c, in.st[c], state_n, state_nm1, in.cg[c][7], inv2dt);
     }
-    // the next tile of this CTA: pull its cell records towards L2 now, its neighbours' later
+    // the next tile of this CTA: its packed neighbours (needed to request its inputs after face 0), and
+    // the lines its non-TMA reads touch, towards L2
     const int64_t cellN = cell0 + (int64_t)gridDim.x * T;
-    if (cellN < nc) {
-      const int nN = (int)min((int64_t)T, nc - cellN);
-      if (warp < 3) {
-        // line l of region [state, state_n, state_nm1 | face states | geometry | neighbours | block map]
-        const char* base;
-        int l, bytes;
-        if (tid < 39) {
-          const int r = tid / 13;
-          l = tid - 13 * r;
-          base = reinterpret_cast<const char*>((r == 0 ? state : (r == 1 ? state_n : state_nm1)) + NEQ * cellN);
-          bytes = nN * NEQ * 8;
-        } else if (tid < 74) {
-          l = tid - 39;
-          base = reinterpret_cast<const char*>(fown + 3 * NEQ * cellN);
-          bytes = nN * 3 * NEQ * 8;
-        } else if (tid < 90) {
-          l = tid - 74;
-          base = reinterpret_cast<const char*>(cgeo + CGEO * cellN);
-          bytes = nN * CGEO * 8;
-        } else if (tid < 92) {
-          l = tid - 90;
-          base = reinterpret_cast<const char*>(nbrf + 3 * cellN);
-          bytes = nN * 12;
-        } else {
-          l = tid - 92;
-          base = reinterpret_cast<const char*>(blk4 + 4 * cellN);
-          bytes = nN * 16;
-        }
-        if (l * 128 < bytes + 127 && tid < 95) prefetch_l2(base + min(l * 128, bytes - 1));
+    const int nN = cellN < nc ? (int)min((int64_t)T, nc - cellN) : 0;
+    int32_t nfN = -1;
+    if (loader && lane < 3 * nN) nfN = nbrf[3 * cellN + lane];
+    if (warp == 0 && nN > 0) {
+      const char* base;
+      int l, bytes;
+      if (lane < 26) {
+        l = lane % 13;
+        base = reinterpret_cast<const char*>((lane < 13 ? state_n : state_nm1) + NEQ * cellN);
+        bytes = nN * NEQ * 8;
+      } else if (lane < 29) {
+        l = lane - 26;
+        base = reinterpret_cast<const char*>(blk4 + 4 * cellN);
+        bytes = nN * 16;
+      } else {
+        l = lane - 29;   // the tile after the next one
+        base = reinterpret_cast<const char*>(nbrf + 3 * (cellN + (int64_t)gridDim.x * T));
+        bytes = cellN + (int64_t)gridDim.x * T + T <= nc ? T * 12 : 0;
       }
+      if (l * 128 < bytes + 127 && bytes > 0) prefetch_l2(base + min(l * 128, bytes - 1));
     }
-    int32_t nbN = -1;   // neighbour (cell, face) = lane of the next tile, held by the last warp
-    if (ROLE == 2 && warp == C::AW + C::MW - 1 && cellN < nc && lane < 3 * (int)min((int64_t)T, nc - cellN))
-      nbN = nbrf[3 * cellN + lane];
-    const int32_t nb0 = nbrf[3 * i], nb1 = nbrf[3 * i + 1], nb2 = nbrf[3 * i + 2];
+    const int32_t nb0 = in.nf[ca][0], nb1 = in.nf[ca][1], nb2 = in.nf[ca][2];
 
     // where this tile's blocks go: thread t < ncell issues the bulk stores of cell t
     int4 b4 = make_int4(-1, -1, -1, -1);
@@ -267,9 +320,9 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
       const double len = cg[8 * k + 2];                                    // Sigma_f
       const bool bnd = nf < 0;
       const double nx = g01.x, ny = g01.y;
-      // own-side and other-side face states of this face (L232), written by k_gradient_limiter
-      const double* __restrict__ fo = fown + (3 * i + k) * NEQ;
-      const double* __restrict__ fx = bnd ? fo : fown + (3 * (int64_t)(nf >> 2) + (nf & 3)) * NEQ;
+      // own-side and other-side face states of this face (L232), written by k_gradient_limiter, staged by TMA
+      const double* __restrict__ fo = in.fo[ca][k];
+      const double* __restrict__ fx = in.fx[ca][k];
 
       const bool any_bnd = __any_sync(0xffffffffu, bnd);   // warp-uniform; boundary faces are rare
       double H[NV];
@@ -329,6 +382,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
       if (JAC && pert && act && !bnd) {
 #pragma unroll
         for (int q = 0; q < NV; ++q) S.mir[k % NM][cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
+      }
+      if (k == 0 && loader && nN > 0) {
+        // request the next tile's inputs into the other stage: every read of that stage ended before
+        // the previous tile's closing barrier
+        stage_inputs<T>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo);
       }
       if (k + NM < 3) {
         // the buffer is needed again by face k + NM: this face's blocks leave now
@@ -427,12 +485,6 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
         }
       }
     }
-    if (nbN >= 0) {
-      // the other-side face states the next tile reads: one 144-byte row (2 lines) per face
-      const char* px = reinterpret_cast<const char*>(fown + (3 * (int64_t)(nbN >> 2) + (nbN & 3)) * NEQ);
-      prefetch_l2(px);
-      prefetch_l2(px + 143);
-    }
     fence_async_smem();
     cta_sync();   // B: every block of the tile is staged
     // a7: each block leaves the SM as one 2592-byte bulk store
@@ -461,11 +513,26 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
   // one instantiation serves both calls, so that the residual does not depend on whether the
   // Jacobian is asked for (same instructions on the base lanes)
   const bool JAC = vals != nullptr;
-  if (JAC) {
-    for (int q = threadIdx.x; q < (NM + 1) * T * BLK; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;   // mir and diag
-    __syncthreads();
-  }
   const int warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) {
+    mbar_init(&S.full[0], 1);
+    mbar_init(&S.full[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (JAC)
+    for (int q = threadIdx.x; q < (NM + 1) * T * BLK; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;   // mir and diag
+  __syncthreads();
+  if (warp == C::AW + C::MW - 1) {
+    // prologue: request the inputs of this CTA's first tile
+    const int lane = threadIdx.x & 31;
+    const int64_t cellF = (int64_t)blockIdx.x * T;
+    const int nF = cellF < nc ? (int)min((int64_t)T, nc - cellF) : 0;
+    if (nF > 0) {
+      const int32_t nfF = lane < 3 * nF ? nbrf[3 * cellF + lane] : -1;
+      stage_inputs<T>(S.in[0], &S.full[0], lane, nfF, cellF, nF, state, fown, cgeo);
+    }
+  }
+  __syncthreads();   // the prologue's neighbour table (plain stores) is visible
   if (warp >= C::AW)
     role_loop<T, NM, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
   else if (warp & 1)
