@@ -24,6 +24,9 @@
 #include "tfa_common.cuh"
 #include "tfa_physics.cuh"
 
+#ifndef TFA_ASM_EARLY2
+#define TFA_ASM_EARLY2 1   // bit 0: AUSM lanes, bit 1: Maxwell lanes evaluate all three faces before the first barrier
+#endif
 #ifndef TFA_ASM_NM
 #define TFA_ASM_NM 2   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
 #endif
@@ -309,12 +312,9 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     for (int q = 0; q < NV; ++q) me[q] = q == pj ? eps : 0.0;
 
     double acc[NV];   // base lane: residual rows; perturbed lane: its column of the diagonal block
-#pragma unroll
-    for (int q = 0; q < NV; ++q) acc[q] = 0.0;
 
-    // ---- faces (Alg. 1) ----
-#pragma unroll 1
-    for (int k = 0; k < 3; ++k) {
+    // ---- one face (Alg. 1): d = this lane's scaled flux (base lane) or flux-Jacobian column ----
+    auto face = [&](const int k, double* __restrict__ d) -> bool {
       const int32_t nf = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);   // 4 * neighbour + its local face, or -1
       const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);   // outward unit normal
       const double len = cg[8 * k + 2];                                    // Sigma_f
@@ -365,42 +365,51 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
         for (int q = 0; q < NV; ++q) H[q] = 0.0;
       }
       const double f = pert ? len * inv_e : len;
-      double d[NV];
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         const double hb = __shfl_sync(0xffffffffu, H[q], base_lane);
         // perturbed lane: (H_pert - H) Sigma_f / eps; base lane: H Sigma_f  (pm = 1 or 0, exact)
         d[q] = __dmul_rn(__fma_rn(-hb, pm, H[q]), f);
-        acc[q] = __dadd_rn(acc[q], d[q]);
       }
-      if (k == 0 || k >= NM) {
-        // buffer k % NM is free: its last bulk store (previous tile / face k - NM) has read it.
-        // At k == 0 this barrier also publishes S.rs / S.s0 of the tile.
-        if (ROLE == 0 && tid < T) bulk_wait_read();
-        cta_sync();
-      }
+      return bnd;
+    };
+    // block (j,i) of the neighbour across a face: minus this cell's own column (staged, structural zeros persist)
+    auto stage_mirror = [&](const int buf, const double* __restrict__ d, const bool bnd) {
       if (JAC && pert && act && !bnd) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) S.mir[k % NM][cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
+        for (int q = 0; q < NV; ++q) S.mir[buf][cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
       }
-      if (k == 0 && loader && nN > 0) {
-        // request the next tile's inputs into the other stage: every read of that stage ended before
-        // the previous tile's closing barrier
-        stage_inputs<T>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo);
-      }
-      if (k + NM < 3) {
-        // the buffer is needed again by face k + NM: this face's blocks leave now
-        fence_async_smem();
-        cta_sync();
-        if (ROLE == 0 && JAC && tid < ncell) {
-          const int32_t b = k == 0 ? b4.y : b4.z;
-          if (b >= 0) {
-            bulk_store(vals + (int64_t)b * BLK, &S.mir[k % NM][tid][0], BLK * 8);
-            bulk_commit();
-          }
-        }
-      }
+    };
+    static_assert(NM == 2, "the barrier sequence below is written for two mirror buffers");
+    constexpr bool EARLY2 = TFA_ASM_EARLY2 & (ROLE == 2 ? 2 : 1);   // evaluate face 2 together with faces 0, 1
+
+    double d0[NV], d1[NV], d2[NV];
+    const bool bnd0 = face(0, d0);
+    const bool bnd1 = face(1, d1);
+    bool bnd2 = false;
+    if (EARLY2) bnd2 = face(2, d2);
+    // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
+    // them.  This barrier also publishes S.rs / S.s0 of the tile.
+    if (ROLE == 0 && tid < T) bulk_wait_read();
+    cta_sync();   // A
+    stage_mirror(0, d0, bnd0);
+    stage_mirror(1, d1, bnd1);
+    if (loader && nN > 0) {
+      // request the next tile's inputs into the other stage: every read of that stage ended before
+      // the previous tile's closing barrier
+      stage_inputs<T>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo);
     }
+    fence_async_smem();
+    cta_sync();   // 1
+    // a7: each block leaves the SM as one 2592-byte bulk store
+    if (ROLE == 0 && JAC && tid < ncell) {
+      if (b4.y >= 0) bulk_store(vals + (int64_t)b4.y * BLK, &S.mir[0][tid][0], BLK * 8);
+      if (b4.z >= 0) bulk_store(vals + (int64_t)b4.z * BLK, &S.mir[1][tid][0], BLK * 8);
+      bulk_commit();
+    }
+    if (!EARLY2) bnd2 = face(2, d2);
+#pragma unroll
+    for (int q = 0; q < NV; ++q) acc[q] = __dadd_rn(__dadd_rn(d0[q], d1[q]), d2[q]);
 
     // ---- residual, source Jacobian (L245-253), BDF2 diagonal (Eq. 13), diagonal block ----
     if (act && !pert) {
@@ -485,14 +494,15 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
         }
       }
     }
+    // mirror buffer 0 has been read by face 0's bulk store: face 2 takes it
+    if (ROLE == 0 && tid < T) bulk_wait_read();
+    cta_sync();   // 2
+    stage_mirror(0, d2, bnd2);
     fence_async_smem();
     cta_sync();   // B: every block of the tile is staged
-    // a7: each block leaves the SM as one 2592-byte bulk store
     if (ROLE == 0 && JAC && tid < ncell) {
       bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[tid][0], BLK * 8);
-      if (NM >= 3 && b4.y >= 0) bulk_store(vals + (int64_t)b4.y * BLK, &S.mir[0][tid][0], BLK * 8);
-      if (NM >= 2 && b4.z >= 0) bulk_store(vals + (int64_t)b4.z * BLK, &S.mir[1 % NM][tid][0], BLK * 8);
-      if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[2 % NM][tid][0], BLK * 8);
+      if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[0][tid][0], BLK * 8);
       bulk_commit();
     }
   }
@@ -501,7 +511,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
 }
 
 template <int T, int NM>
-__global__ void __launch_bounds__(AsmCfg<T>::NT) k_assemble(
+__global__ void __launch_bounds__(AsmCfg<T>::NT, 2) k_assemble(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
@@ -573,15 +583,7 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
                     const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
                     int32_t* flags, cudaStream_t st) {
   if (m.nc == 0) return 0;
-  // TFA_ASM_NM in the environment overrides the compiled-in staging depth (tuning sweeps only)
-  static const int nm = [] {
-    const char* e = getenv("TFA_ASM_NM");
-    const int x = e ? atoi(e) : TFA_ASM_NM;
-    return x >= 1 && x <= 3 ? x : TFA_ASM_NM;
-  }();
-  if (nm == 1) return launch_nm<10, 1>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
-  if (nm == 2) return launch_nm<10, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
-  return launch_nm<10, 3>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
+  return launch_nm<10, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
 }
 
 }  // namespace tfa
