@@ -27,6 +27,9 @@
 #ifndef TFA_ASM_EARLY2
 #define TFA_ASM_EARLY2 1   // bit 0: AUSM lanes, bit 1: Maxwell lanes evaluate all three faces before the first barrier
 #endif
+#ifndef TFA_ASM_VEC3
+#define TFA_ASM_VEC3 0     // AUSM lanes evaluate their three faces through ausm_flux_n<3>
+#endif
 #ifndef TFA_ASM_NM
 #define TFA_ASM_NM 2   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
 #endif
@@ -384,10 +387,69 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     constexpr bool EARLY2 = TFA_ASM_EARLY2 & (ROLE == 2 ? 2 : 1);   // evaluate face 2 together with faces 0, 1
 
     double d0[NV], d1[NV], d2[NV];
-    const bool bnd0 = face(0, d0);
-    const bool bnd1 = face(1, d1);
-    bool bnd2 = false;
-    if (EARLY2) bnd2 = face(2, d2);
+    bool bnd0, bnd1, bnd2 = false;
+    if (ROLE != 2 && EARLY2 && TFA_ASM_VEC3) {
+      // AUSM lanes: VF faces through one face-vectorised flux call (interleaved dependency chains)
+      constexpr int VF = TFA_ASM_VEC3 >= 3 ? 3 : 2;
+      double own[VF][5], oth[VF][5], nrm[VF][2], H[VF][5];
+      bool bn[VF], okf[VF];
+#pragma unroll
+      for (int k = 0; k < VF; ++k) {
+        const int32_t nf = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);
+        bn[k] = nf < 0;
+        const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);
+        nrm[k][0] = g01.x;
+        nrm[k][1] = g01.y;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          own[k][q] = in.fo[ca][k][vidx<ROLE>(q)] + me[q];
+          oth[k][q] = in.fx[ca][k][vidx<ROLE>(q)];
+        }
+      }
+      bool anyb = false;
+#pragma unroll
+      for (int k = 0; k < VF; ++k) anyb |= bn[k];
+      if (__any_sync(0xffffffffu, anyb)) {
+        // boundary face: P_R := P_L, so the perturbation moves both arguments (S9)
+#pragma unroll
+        for (int k = 0; k < VF; ++k)
+          if (bn[k]) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) oth[k][q] = own[k][q];
+          }
+      }
+      if (run) {
+        ausm_flux_n<VF>(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nrm, H, okf);
+        bool okall = true;
+#pragma unroll
+        for (int k = 0; k < VF; ++k) okall &= okf[k];
+        if (!pert && act) nonphys |= !okall;
+      } else {
+#pragma unroll
+        for (int k = 0; k < VF; ++k)
+#pragma unroll
+          for (int q = 0; q < 5; ++q) H[k][q] = 0.0;
+      }
+#pragma unroll
+      for (int k = 0; k < VF; ++k) {
+        const double len = cg[8 * k + 2];
+        const double f = pert ? len * inv_e : len;
+        double* d = k == 0 ? d0 : (k == 1 ? d1 : d2);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          const double hb = __shfl_sync(0xffffffffu, H[k][q], base_lane);
+          d[q] = __dmul_rn(__fma_rn(-hb, pm, H[k][q]), f);
+        }
+      }
+      bnd0 = bn[0];
+      bnd1 = bn[1];
+      if (VF == 3) bnd2 = bn[VF - 1];
+      else bnd2 = face(2, d2);
+    } else {
+      bnd0 = face(0, d0);
+      bnd1 = face(1, d1);
+      if (EARLY2) bnd2 = face(2, d2);
+    }
     // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
     // them.  This barrier also publishes S.rs / S.s0 of the tile.
     if (ROLE == 0 && tid < T) bulk_wait_read();
@@ -407,7 +469,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
       if (b4.z >= 0) bulk_store(vals + (int64_t)b4.z * BLK, &S.mir[1][tid][0], BLK * 8);
       bulk_commit();
     }
-    if (!EARLY2) bnd2 = face(2, d2);
+    if (!EARLY2) bnd2 = face(2, d2);   // (the Maxwell lanes: while the bulk stores read the buffers)
 #pragma unroll
     for (int q = 0; q < NV; ++q) acc[q] = __dadd_rn(__dadd_rn(d0[q], d1[q]), d2[q]);
 

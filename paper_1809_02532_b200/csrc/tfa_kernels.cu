@@ -5,6 +5,8 @@
 //                      grad P_i = sum_j c_ij (P_j - P_i)                                   (L74)
 //  k_gradient_limiter  thread = (cell, variable): LS gradient + Venkatakrishnan phi      (L74, L208)
 //  (k_assemble, the fused flux / Jacobian / source / BDF2 / BSR-write kernel, is in tfa_assemble.cu)
+#include <type_traits>
+
 #include "tfa_common.cuh"
 #include "tfa_physics.cuh"
 
@@ -54,37 +56,77 @@ __global__ void __launch_bounds__(GL_T) k_gradient_limiter(int64_t nc, const dou
   const int64_t i = blockIdx.x * (int64_t)GL_CELLS + threadIdx.x / NEQ;
   if (i >= nc) return;
   const double Pi = state[NEQ * i + v];
-  double gx = 0.0, gy = 0.0, umax = Pi, umin = Pi;
-  const int32_t b = st_ptr[i], e = st_ptr[i + 1];
-  for (int32_t q = b; q < e; ++q) {
-    const int64_t j = st_idx[q];
-    const double Pj = state[NEQ * j + v];
-    const double dP = Pj - Pi;
-    gx += coef[2 * (int64_t)q] * dP;
-    gy += coef[2 * (int64_t)q + 1] * dP;
-    umax = fmax(umax, Pj);
-    umin = fmin(umin, Pj);
-  }
-  // Venkatakrishnan (L208; S13): eps^2 = (K h)^3, Delta2 sampled at the cell's three face midpoints
+  // geometry of the limiter and of the face extrapolation, requested before the stencil walk
   const double* g = cgeo + CGEO * i;
-  const double Kh = venkK * g[15];
-  const double eps2 = Kh * Kh * Kh;
-  double phi = 1.0;
+  double ox[3], oy[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    const double d2 = gx * g[8 * k + 3] + gy * g[8 * k + 4];
-    const double d1 = d2 > 0.0 ? umax - Pi : umin - Pi;
+    ox[k] = g[8 * k + 3];
+    oy[k] = g[8 * k + 4];
+  }
+  const double sqrt_vol = g[15];
+  // dmax / dmin = max / min over {i} U stencil of P_j - P_i: the limiter's Delta_1 (u_max - P_i, u_min - P_i)
+  double gx = 0.0, gy = 0.0, dmax = 0.0, dmin = 0.0;
+  const int32_t b = st_ptr[i], e = st_ptr[i + 1];
+  // the stencil walk is a chain of dependent loads (index -> state); eight (then four) entries are fetched at a
+  // time so that their latencies overlap.  The summation order stays that of the stencil.
+  const double2* __restrict__ coef2 = reinterpret_cast<const double2*>(coef);
+  int32_t q = b;
+  auto batch = [&](auto nu) {
+    constexpr int NU = decltype(nu)::value;
+    int64_t j[NU];
+    double2 c[NU];
+    double Pj[NU];
+#pragma unroll
+    for (int u = 0; u < NU; ++u) j[u] = st_idx[q + u];
+#pragma unroll
+    for (int u = 0; u < NU; ++u) c[u] = coef2[q + u];
+#pragma unroll
+    for (int u = 0; u < NU; ++u) Pj[u] = state[NEQ * j[u] + v];
+#pragma unroll
+    for (int u = 0; u < NU; ++u) {
+      const double dP = Pj[u] - Pi;
+      gx += c[u].x * dP;
+      gy += c[u].y * dP;
+      dmax = dP > dmax ? dP : dmax;
+      dmin = dP < dmin ? dP : dmin;
+    }
+    q += NU;
+  };
+  while (q + 8 <= e) batch(std::integral_constant<int, 8>{});
+  if (q + 4 <= e) batch(std::integral_constant<int, 4>{});
+  for (; q < e; ++q) {
+    const int64_t j = st_idx[q];
+    const double2 c = coef2[q];
+    const double Pj = state[NEQ * j + v];
+    const double dP = Pj - Pi;
+    gx += c.x * dP;
+    gy += c.y * dP;
+    dmax = dP > dmax ? dP : dmax;
+    dmin = dP < dmin ? dP : dmin;
+  }
+  // Venkatakrishnan (L208; S13): eps^2 = (K h)^3, Delta2 sampled at the cell's three face midpoints
+  const double Kh = venkK * sqrt_vol;
+  const double eps2 = Kh * Kh * Kh;
+  // phi = min(1, min_f num_f / den_f): the smallest ratio is found by cross-multiplication
+  // (den > 0), so that one division serves the three faces
+  double nb = 1.0, db = 1.0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double d2 = gx * ox[k] + gy * oy[k];
+    const double d1 = d2 > 0.0 ? dmax : dmin;
     const double num = d1 * d1 + eps2 + 2.0 * d1 * d2;
     const double den = d1 * d1 + 2.0 * d2 * d2 + d1 * d2 + eps2;
-    const double pf = d2 != 0.0 ? num / den : 1.0;
-    phi = fmin(phi, pf);
+    const bool smaller = d2 != 0.0 && num * db < nb * den;   // Delta_2 = 0: phi_f = 1
+    nb = smaller ? num : nb;
+    db = smaller ? den : db;
   }
-  phi = fmin(phi, 1.0);
+  const double phi = nb / db;
   if (fown) {
     // own-side face states of the three faces (L232), the gradient limited once: phi grad P
     const double lx = phi * gx, ly = phi * gy;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) fown[(3 * i + k) * NEQ + v] = Pi + (lx * g[8 * k + 3] + ly * g[8 * k + 4]);
+    for (int k = 0; k < 3; ++k) fown[(3 * i + k) * NEQ + v] = Pi + (lx * ox[k] + ly * oy[k]);
   }
   if (grad_out) {
     grad_out[2 * (NEQ * i + v)] = gx;
