@@ -323,3 +323,47 @@ def test_config2_first_and_last_of_ten_calls(api, orc, W):
             assert er < RES_TOL and ej < JAC_TOL, (call, er, ej)
         P_prev2, P_prev, P = P_prev, P, W.perturb(P, 100 + call, 1e-6)
     ctx.check()
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4a", "c4b", "c5"])
+def test_full_size_sampled_rows(api, orc, W, name):
+    """BASELINE configs 2-5 at their full sizes, in the launch configuration bench.py times (device
+    buffers, RCM where the config says so): rhs and whole BSR rows of a seeded row sample (plus the first
+    and the last tile of the mesh) against the oracle's row-subset mode; pattern compared bit-exactly on
+    the sample; every entry of the value array written (NaN canary)."""
+    import torch
+    w = W.make_workload(name)
+    g, o = api.Mesh.from_input(w.mesh), orc.OracleMesh.from_input(w.mesh)
+    if w.reorder == "rcm":
+        g.reorder("rcm")
+        o.reorder("rcm")
+    perm = g.get("perm")
+    assert np.array_equal(perm, o.get("perm"))
+    P = np.ascontiguousarray(w.state[perm])
+    nc = g.n_cells
+    rng = np.random.default_rng(77)
+    rows = np.unique(np.concatenate([rng.choice(nc, size=3000, replace=False), np.arange(25), np.arange(nc - 25, nc)]))
+    rows = rows.astype(np.int32)
+    ctx = api.Context(w.physics)
+    rhs = torch.empty((nc, 18), dtype=torch.float64, device="cuda")
+    vals = torch.full((g.nnzb, 18, 18), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.assemble(g, dev(P), dt=w.dt, rhs=rhs, vals=vals)
+    ctx.check()
+    assert not bool(torch.isnan(vals).any()), "an entry of the BSR value array was not written"
+    rp, rp_o = g.get("bsr_rowptr"), o.get("bsr_rowptr")
+    col, col_o = g.get("bsr_col"), o.get("bsr_col")
+    assert np.array_equal(rp, rp_o)
+    blk = np.concatenate([np.arange(rp[i], rp[i + 1]) for i in rows])
+    assert np.array_equal(col[blk], col_o[blk])
+    vals_s = vals[torch.from_numpy(blk).cuda()].cpu().numpy()
+    got = np.zeros((len(rows), 4, 18, 18))
+    q = 0
+    for r, i in enumerate(rows):
+        n = rp[i + 1] - rp[i]
+        got[r, :n] = vals_s[q:q + n]
+        q += n
+    ph_o = orc.physics_c(w.physics)
+    rhs_o, sc_o, vals_o = orc.assemble(o, ph_o, orc.default_numerics(ph_o), P, dt=w.dt, rows=rows)
+    er = residual_error(rhs[torch.from_numpy(rows.astype(np.int64)).cuda()].cpu().numpy(), rhs_o, sc_o)
+    ej = jacobian_error_rows(got, vals_o)
+    assert er < RES_TOL and ej < JAC_TOL, (name, er, ej)
