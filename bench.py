@@ -35,10 +35,14 @@ def algorithmic_bytes(nc: int, nnzb: int, nst: int):
     asm = (nnzb * 18 * 18 * 8      # BSR Jacobian blocks written once
            + nc * 144 * 3          # state, state_n, state_nm1 read
            + nc * 144              # rhs written
-           + nc * 288              # limited gradient read
+           + nc * 432              # own-side face states of the three faces (read once; both users hit L2)
            + nc * 192              # per-cell geometry record
-           + nc * 12 + nc * 4)     # neighbour table, row pointers
-    grad = (nc * 144 + nst * 4 + nst * 16 + nc * 4 + nc * 192 + nc * 288)
+           + nc * 12 + nc * 16)    # packed neighbour table, block map
+    grad = (nc * 144               # state read
+            + nst * 4 + nst * 16   # stencil indices and least-squares coefficient vectors
+            + nc * 4               # stencil row pointers
+            + nc * 192             # geometry record
+            + nc * 432)            # face states written
     return asm, grad
 
 
@@ -101,9 +105,14 @@ def measured_peaks():
 
 
 def ncu_traffic(workload: str):
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum of k_assemble per launch, from the committed
+    `ncu --set full` capture (profiles/ncu_traffic.csv: workload,kernel,dram_bytes_per_launch)."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if os.path.exists(p):
-        return json.load(open(p)).get(workload, {}).get("k_assemble_dram_bytes_per_launch")
+        for line in open(p):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 3 and f[0] == workload and f[1] == "k_assemble":
+                return float(f[2])
     return None
 
 
@@ -308,7 +317,7 @@ def main():
     asm_ms = ms_asm / max(ncalls, 1)
     grad_ms = ms_grad / max(ncalls, 1)
     achieved = asm_bytes / (asm_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_assemble<true>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "k_assemble", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": ncu_traffic(args.workload),
                 "algorithmic_bytes_per_launch": asm_bytes, "kernel_ms": asm_ms, "peak_source": peak_src,
                 "kernel_share_of_step": asm_ms / ms_per_step,

@@ -30,6 +30,12 @@
 #ifndef TFA_ASM_VEC3
 #define TFA_ASM_VEC3 0     // AUSM lanes evaluate their three faces through ausm_flux_n<3>
 #endif
+#ifndef TFA_ASM_L2HINT
+#define TFA_ASM_L2HINT 0   // bit 0: bulk stores evict_first, bit 1: bulk loads evict_last
+#endif
+#ifndef TFA_ASM_T
+#define TFA_ASM_T 10      // cells per tile (multiple of 5)
+#endif
 #ifndef TFA_ASM_NM
 #define TFA_ASM_NM 2   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
 #endif
@@ -41,8 +47,17 @@ namespace tfa {
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, uint32_t bytes) {
   const uint32_t s = (uint32_t)__cvta_generic_to_shared(ssrc);
+#if TFA_ASM_L2HINT & 1
+  // the Jacobian is written once and not read again by this kernel: first in line for eviction from L2
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst), "r"(s),
+               "r"(bytes), "l"(pol)
+               : "memory");
+#else
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes)
                : "memory");
+#endif
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // all bulk stores of this thread have finished READING shared memory (the staging may be reused)
@@ -72,10 +87,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   } while (!done);
 }
 __device__ __forceinline__ void bulk_load(void* sdst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+#if TFA_ASM_L2HINT & 2
+  // face states are read twice (by the cell and by its neighbour): keep them in L2 against the write stream
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(sdst)),
+      "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+      : "memory");
+#else
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
                    smem_u32(sdst)),
                "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
+#endif
 }
 // pull one 128-byte line towards L2 ahead of use (read latency under the Jacobian's write stream is long)
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -573,7 +599,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
 }
 
 template <int T, int NM>
-__global__ void __launch_bounds__(AsmCfg<T>::NT, 2) k_assemble(
+__global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
@@ -645,7 +671,7 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
                     const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
                     int32_t* flags, cudaStream_t st) {
   if (m.nc == 0) return 0;
-  return launch_nm<10, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
+  return launch_nm<TFA_ASM_T, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
 }
 
 }  // namespace tfa

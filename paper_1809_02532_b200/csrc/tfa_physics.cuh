@@ -5,6 +5,17 @@
 #pragma once
 #include "tfa_common.cuh"
 
+#ifndef TFA_FAST_MATH64
+#define TFA_FAST_MATH64 1   // 1: Newton-refined sqrt / reciprocal in the AUSM flux; 0: IEEE library sequences
+#endif
+#if TFA_FAST_MATH64
+#define TFA_SQRT(x) nsqrt(x)
+#define TFA_RCP(x) nrcp(x)
+#else
+#define TFA_SQRT(x) sqrt(x)
+#define TFA_RCP(x) (1.0 / (x))
+#endif
+
 namespace tfa {
 
 // Derived constants, computed once on the host and passed by value as a kernel parameter
@@ -86,6 +97,32 @@ __device__ __forceinline__ void maxwell_flux(const Consts& K, const double* L, c
   H[7] = h * (s[3] * nx + s[4] * ny) - a * (K.xc * d[7]);
 }
 
+// Square root and reciprocal for the flux: a single-precision hardware seed (MUFU.RSQ / MUFU.RCP, 23
+// bits) refined by two Newton steps in FP64 (fused multiply-adds only) -- about half the instructions
+// and latency of the correctly rounded library sequences, error below 1 ulp.  Arguments are the
+// positive, O(1)-scaled quantities of a physical state (a non-physical one is reported by the
+// rho, T > 0 test, whatever these return).
+__device__ __forceinline__ double nsqrt(double x) {
+  const double y = (double)rsqrtf((float)x);
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  return fma(fma(-g, g, x), h, g);   // last correction: g + (x - g^2) / (2 g)
+}
+__device__ __forceinline__ double nrcp(double d) {
+  double y = (double)__frcp_rn((float)d);
+  double e = fma(-d, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-d, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-d, y, 1.0);
+  return fma(y, e, y);
+}
+
 // Multi-fluid AUSM+-up for one species (Eq. 10; Liou's scheme = ref. [30]; S4).
 // L, R = (rho, u, v, w, T).  Returns true if the states are physical.
 // Rs, gR, cp, Minf2: the species' constants (K.Rs[s], ...), passed in registers (warp uniform).
@@ -93,16 +130,16 @@ __device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, doubl
                                           const double* L, const double* R, double nx, double ny, double* H) {
   const double rL = L[0], rR = R[0], TL = L[4], TR = R[4];
   const bool ok = (rL > 0.0) & (rR > 0.0) & (TL > 0.0) & (TR > 0.0);
-  const double aL = sqrt(gR * TL), aR = sqrt(gR * TR);
+  const double aL = TFA_SQRT(gR * TL), aR = TFA_SQRT(gR * TR);
   const double pL = rL * Rs * TL, pR = rR * Rs * TR;
   const double unL = L[1] * nx + L[2] * ny, unR = R[1] * nx + R[2] * ny;
   const double HtL = cp * TL + 0.5 * (L[1] * L[1] + L[2] * L[2] + L[3] * L[3]);
   const double HtR = cp * TR + 0.5 * (R[1] * R[1] + R[2] * R[2] + R[3] * R[3]);
   const double a12 = 0.5 * (aL + aR);
-  const double ia = 1.0 / a12;
+  const double ia = TFA_RCP(a12);
   const double ML = unL * ia, MR = unR * ia;
   const double Mb2 = 0.5 * (unL * unL + unR * unR) * (ia * ia);
-  const double Mo = sqrt(fmin(1.0, fmax(Mb2, Minf2)));
+  const double Mo = TFA_SQRT(fmin(1.0, fmax(Mb2, Minf2)));
   const double fa = Mo * (2.0 - Mo);
   const double al16 = 3.0 * (5.0 * fa * fa - 4.0);             // 16 alpha, alpha = 3/16 (-4 + 5 fa^2)
   // split Mach numbers and pressures; for |M| >= 1:  M4+ = max(M,0), P5+ = (M > 0), etc.
@@ -114,7 +151,7 @@ __device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, doubl
   const double P5p = supL ? (ML > 0.0 ? 1.0 : 0.0) : m2pL * ((2.0 - ML) - al16 * ML * m2mL);
   const double P5m = supR ? (MR < 0.0 ? 1.0 : 0.0) : m2mR * ((-2.0 - MR) + al16 * MR * m2pR);
   const double rsum = rL + rR;
-  const double Mp = -K.Kp * fmax(1.0 - K.sigma * Mb2, 0.0) * (pR - pL) * (ia * ia) / (fa * 0.5 * rsum);
+  const double Mp = -K.Kp * fmax(1.0 - K.sigma * Mb2, 0.0) * (pR - pL) * (ia * ia) * TFA_RCP(fa * 0.5 * rsum);
   const double M12 = M4p + M4m + Mp;
   const bool up = M12 > 0.0;
   const double mdot = a12 * M12 * (up ? rL : rR);
