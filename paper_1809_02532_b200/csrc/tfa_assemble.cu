@@ -15,10 +15,13 @@
 //    (Eq. 10); a Maxwell warp holds 3 groups of 9 lanes = cell x {base, 8 perturbed} (Eq. 9
 //    L91).  The reconstructed face states (L232: P + phi grad P . dx) of both sides come from the
 //    gradient kernel's face-state array (every lane of a group reads the same addresses; the
-//    perturbation is added to the own-side value), the base flux reaches the group by warp shuffle; the flux Jacobian is block diagonal (8x8, 5x5, 5x5), the
-//    source (Eq. 4/6) couples the blocks on the diagonal block only.
+//    perturbation is added to the own-side value), staged one tile ahead into shared memory by TMA
+//    bulk loads; the base flux reaches the group by warp shuffle; the flux Jacobian is block diagonal
+//    (8x8, 5x5, 5x5), the source (Eq. 4/6) couples the blocks on the diagonal block only.
 //  * 18x18 blocks are staged in shared memory (their structural zeros are written once per CTA)
 //    and leave the SM as 2592-byte TMA bulk stores (cp.async.bulk.global.shared::cta).
+//  * The TFA_ASM_* switches below select variants that were measured and rejected;
+//    the defaults are the measured best.
 #include <cstdlib>
 
 #include "tfa_common.cuh"
