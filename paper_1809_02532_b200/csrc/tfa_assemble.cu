@@ -36,6 +36,9 @@
 #ifndef TFA_ASM_L2HINT
 #define TFA_ASM_L2HINT 0   // bit 0: bulk stores evict_first, bit 1: bulk loads evict_last
 #endif
+#ifndef TFA_ASM_BLKP
+#define TFA_ASM_BLKP 330   // doubles between staged blocks (324 = dense)
+#endif
 #ifndef TFA_ASM_T
 #define TFA_ASM_T 10      // cells per tile (multiple of 5)
 #endif
@@ -44,6 +47,8 @@
 #endif
 
 namespace tfa {
+
+constexpr int BLKP = TFA_ASM_BLKP;
 
 // ------------------------------------------------------------------------------------------------
 // TMA bulk-store helpers (PTX ISA: cp.async.bulk, bulk async-groups, async proxy fence)
@@ -134,8 +139,10 @@ template <int T, int NM>
 struct __align__(128) AsmSmem {
   AsmIn<T> in[2];
   uint64_t full[2];        // mbarriers: stage s has landed
-  double mir[NM][T][BLK];  // staged mirror blocks (j,i), face k in buffer k % NM; structural zeros persist
-  double diag[T][BLK];     // staged diagonal block (i,i); structural zeros persist
+  // staged blocks: a stride of BLKP doubles (16-byte multiple, odd number of 16-byte units) spreads the
+  // column stores of different cells over the banks
+  double mir[NM][T][BLKP];  // mirror blocks (j,i), face k in buffer k % NM; structural zeros persist
+  double diag[T][BLKP];     // diagonal block (i,i); structural zeros persist
   double rs[T][NEQ];     // non-flux part of R~: Omega (BDF2 term) - Omega S
   double s0[T][8];       // Lorentz-force and Joule-heating rows of S(P_i): equations 10..17
 };
@@ -621,7 +628,7 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (JAC)
-    for (int q = threadIdx.x; q < (NM + 1) * T * BLK; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;   // mir and diag
+    for (int q = threadIdx.x; q < (NM + 1) * T * BLKP; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;   // mir and diag
   __syncthreads();
   if (warp == C::AW + C::MW - 1) {
     // prologue: request the inputs of this CTA's first tile
