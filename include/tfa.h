@@ -140,6 +140,10 @@ int tfa_check(tfa_ctx* ctx, void* stream);
  * doubles with 16-byte vector accesses -> bytes = 16*n.  Both asynchronous on `stream`. */
 int tfa_probe_dfma(int grid, int iters, double* sink, void* stream);
 int tfa_probe_copy(const double* src, double* dst, int64_t n, void* stream);
+/* The square root and the reciprocal the AUSM flux kernel uses (single-precision hardware seed refined by
+ * Newton steps in FP64), applied to x[0..n): sqrt_out[i], rcp_out[i].  DEVICE pointers.
+ * Lets the tests bound their error against the correctly rounded results. */
+int tfa_probe_math(const double* x, double* sqrt_out, double* rcp_out, int64_t n, void* stream);
 
 /* Per-kernel timing with CUDA events recorded on the launching stream (bench.py's roofline).
  * tfa_timing_enable(ctx, 1): every later tfa_assemble records events before, between and after

@@ -205,6 +205,13 @@ def probe_copy(src: torch.Tensor, dst: torch.Tensor):
     return 16 * n                       # bytes read + written
 
 
+def probe_math(x: torch.Tensor):
+    """(sqrt, reciprocal) of x as the AUSM flux kernel computes them."""
+    s, r = torch.empty_like(x), torch.empty_like(x)
+    _lib.check(_lib.load().tfa_probe_math(_dp(x), _dp(s), _dp(r), x.numel(), _stream()))
+    return s, r
+
+
 # C-style aliases, same names as the ABI
 def mesh_create(node_xy, cell_nodes, cell_xy=None) -> Mesh:
     return Mesh(node_xy, cell_nodes, cell_xy)

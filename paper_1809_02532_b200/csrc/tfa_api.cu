@@ -13,6 +13,7 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
                     int32_t* flags, cudaStream_t st);
 int launch_probe_dfma(int grid, int iters, double* sink, cudaStream_t st);
 int launch_probe_copy(const double* src, double* dst, int64_t n, cudaStream_t st);
+int launch_probe_math(const double* x, double* s, double* r, int64_t n, cudaStream_t st);
 
 namespace {
 
@@ -181,6 +182,11 @@ int tfa_probe_dfma(int grid, int iters, double* sink, void* stream) {
 int tfa_probe_copy(const double* src, double* dst, int64_t n, void* stream) {
   if (!src || !dst || n <= 0 || (n & 1)) return set_error(TFA_EINVAL, "bad argument (n must be even)");
   return launch_probe_copy(src, dst, n, (cudaStream_t)stream);
+}
+
+int tfa_probe_math(const double* x, double* sqrt_out, double* rcp_out, int64_t n, void* stream) {
+  if (!x || !sqrt_out || !rcp_out || n <= 0) return set_error(TFA_EINVAL, "bad argument");
+  return launch_probe_math(x, sqrt_out, rcp_out, n, (cudaStream_t)stream);
 }
 
 int tfa_timing_enable(tfa_ctx* ctx, int on) {

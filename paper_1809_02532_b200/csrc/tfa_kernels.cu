@@ -156,6 +156,14 @@ __global__ void __launch_bounds__(256) k_probe_copy(const double2* __restrict__ 
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n2; i += stride) dst[i] = src[i];
 }
 
+__global__ void k_probe_math(const double* __restrict__ x, double* __restrict__ s, double* __restrict__ r, int64_t n) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) {
+    s[i] = TFA_SQRT(x[i]);
+    r[i] = TFA_RCP(x[i]);
+  }
+}
+
 // ================================================================================================
 // host-side launchers used by tfa_api.cu
 // ================================================================================================
@@ -171,6 +179,12 @@ int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, 
   if (m.nc == 0) return 0;
   k_gradient_limiter<<<cdiv(m.nc, GL_CELLS), GL_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
                                                            venkK, fown, grad, phi);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int launch_probe_math(const double* x, double* s, double* r, int64_t n, cudaStream_t st) {
+  k_probe_math<<<cdiv(n, 256), 256, 0, st>>>(x, s, r, n);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }

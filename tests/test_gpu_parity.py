@@ -367,3 +367,17 @@ def test_full_size_sampled_rows(api, orc, W, name):
     er = residual_error(rhs[torch.from_numpy(rows.astype(np.int64)).cuda()].cpu().numpy(), rhs_o, sc_o)
     ej = jacobian_error_rows(got, vals_o)
     assert er < RES_TOL and ej < JAC_TOL, (name, er, ej)
+
+
+def test_flux_sqrt_and_reciprocal_error_bound(api):
+    """The Newton-refined square root and reciprocal of the AUSM flux kernel against the
+    correctly rounded numpy results over 12 decades: within 1 ulp (the claim the Jacobian tolerance
+    budget in DESIGN.md section 7 rests on)."""
+    import torch
+    rng = np.random.default_rng(5)
+    x = np.concatenate([10.0 ** rng.uniform(-6, 6, 200000), [1.0, 4.0, 0.25, 2.0, 3.0, 1e-6, 1e6]])
+    s, r = api.probe_math(torch.from_numpy(x).cuda())
+    s, r = s.cpu().numpy(), r.cpu().numpy()
+    es = np.abs(s - np.sqrt(x)) / np.spacing(np.sqrt(x))
+    er = np.abs(r - 1.0 / x) / np.spacing(1.0 / x)
+    assert es.max() <= 1.0 and er.max() <= 1.0, (es.max(), er.max())
