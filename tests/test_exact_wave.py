@@ -154,3 +154,30 @@ def test_gpu_residual_of_the_exact_wave_converges_at_second_order(W):
         e, scale, w = residual_error(None, W, n, 20.0, 25.0, 0, run)
         errs.append(e)
     check_convergence(np.array(errs), scale, 20.0)
+
+
+def test_harris_sheet_total_force_balance_and_ampere(orc, W):
+    """The unperturbed GEM Harris sheet (L551-559: B_x = tanh(y/lambda), n = sech^2 + 0.2, T_i + T_e = 1/2,
+    electrons carrying J = curl B) is in total force balance, grad(p_i + p_e) = J x B, and satisfies Ampere's law;
+    the single species are not balanced (E = 0 in the set-up).  Discretely: the sum of the two y-momentum
+    residuals and the E_z residual go to zero with the mesh, while each species' own residual stays O(1).
+    Pins p_s = rho_s T_s / m_s, the q_s n_s u_s x B normalisation and mu0 = 1 against the GEM set-up."""
+    out = []
+    for n in (32, 64, 128):
+        m = W.split_quad_mesh(n // 2, n, -3.2, 3.2, -6.4, 6.4, periodic_x=True, periodic_y=False)
+        cen = m.centroids()
+        P = W.gem_state(cen, psi0=0.0)
+        o = orc.OracleMesh.from_input(m)
+        pc = orc.physics_c(W.Physics())
+        rhs, _, _ = orc.assemble(o, pc, orc.default_numerics(pc, venkat_K=1e9, term_mask=3), P, dt=1.0,
+                                 jacobian=False)
+        vol = o.get("volume")
+        r2 = (rhs[0::2] + rhs[1::2]) / (vol[0::2] + vol[1::2])[:, None]
+        inner = np.abs(0.5 * (cen[0::2, 1] + cen[1::2, 1])) < 5.0          # away from the transmissive walls
+        r2 = r2[inner]
+        out.append((np.abs(r2[:, 11] + r2[:, 14]).max(), np.abs(r2[:, 5]).max(), np.abs(r2[:, 11]).max()))
+    out = np.array(out)
+    c2_over_lam = 20.0 ** 2 / 0.5                     # size of c^2 J_z and of c^2 (curl B)_z
+    assert out[2, 2] > 0.5                            # a single species is far from balance ...
+    assert out[2, 0] < 1e-2 * out[2, 2] and out[2, 0] < out[1, 0] < out[0, 0]      # ... the sum is balanced
+    assert out[2, 1] < 3e-3 * c2_over_lam and out[2, 1] < out[1, 1] < out[0, 1]    # Ampere: c^2 (curl B - J) -> 0
