@@ -181,3 +181,72 @@ def test_harris_sheet_total_force_balance_and_ampere(orc, W):
     assert out[2, 2] > 0.5                            # a single species is far from balance ...
     assert out[2, 0] < 1e-2 * out[2, 2] and out[2, 0] < out[1, 0] < out[0, 0]      # ... the sum is balanced
     assert out[2, 1] < 3e-3 * c2_over_lam and out[2, 1] < out[1, 1] < out[0, 1]    # Ampere: c^2 (curl B - J) -> 0
+
+
+def newton_bdf2_step(assemble_fn, rowptr, col, n_cells, x, c, mass_ratio, dt, t0=0.3, iters=5):
+    """One BDF2 step (Eq. 12-13) from the exact wave at t0 - dt and t0, Newton's method on the
+    pseudo-steady residual (Eq. 14: A dP = rhs, P += dP) with a direct sparse solve of the assembled
+    BSR system.  Returns the residual maxima per iteration (last one after the final update) and P^{n+1}."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spl
+    Pm = exact_wave(x, t0 - dt, c, mass_ratio)[0]
+    Pn = exact_wave(x, t0, c, mass_ratio)[0]
+    P = Pn.copy()
+    norms = []
+    for _ in range(iters):
+        rhs, vals = assemble_fn(P, Pn, Pm, dt, True)
+        norms.append(np.abs(rhs).max())
+        A = sp.bsr_matrix((vals, col, rowptr), shape=(18 * n_cells, 18 * n_cells)).tocsc()
+        P = P + spl.spsolve(A, rhs.ravel()).reshape(-1, 18)
+    norms.append(np.abs(assemble_fn(P, Pn, Pm, dt, False)[0]).max())
+    return np.array(norms), P, Pn
+
+
+def check_newton(norms, P, Pn, x, c, mass_ratio, dt):
+    # the Jacobian (frozen gradient and limiter, S8; forward differences, S7) is a good enough derivative of
+    # the residual, with the right sign (S6) and the right BDF2 diagonal, for Newton to contract fast
+    assert (norms[1:] < 0.4 * norms[:-1]).all() and norms[-1] < 1e-4 * norms[0], norms
+    # and the converged step lands on the exact solution at t0 + dt up to the truncation error
+    Pex = exact_wave(x, 0.3 + dt, c, mass_ratio)[0]
+    err, change = np.abs(P - Pex).max(axis=0), np.abs(Pn - Pex).max(axis=0)
+    moving = [1, 2, 4, 5, 11, 12, 14, 15]
+    assert (err[moving] < 0.06 * change[moving]).all(), (err[moving], change[moving])
+    assert np.delete(err, moving).max() < 0.05 * change.max(), err
+
+
+def test_newton_converges_on_a_bdf2_step_of_the_exact_wave_oracle(orc, W):
+    c, mass_ratio, dt = 20.0, 25.0, 0.05
+    m = W.split_quad_mesh(32, 16, 0.0, 2.0 * np.pi, 0.0, np.pi)
+    o = orc.OracleMesh.from_input(m)
+    pc = orc.physics_c(W.Physics(mass_ratio=mass_ratio, c=c))
+    nu = orc.default_numerics(pc)
+
+    def assemble_fn(P, Pn, Pm, dt_, jac):
+        rhs, _, vals = orc.assemble(o, pc, nu, P, Pn, Pm, dt_, jacobian=jac)
+        return rhs, vals
+
+    x = m.centroids()[:, 0]
+    norms, P, Pn = newton_bdf2_step(assemble_fn, o.get("bsr_rowptr"), o.get("bsr_col"), o.n_cells, x, c, mass_ratio, dt)
+    check_newton(norms, P, Pn, x, c, mass_ratio, dt)
+
+
+@pytest.mark.gpu
+def test_newton_converges_on_a_bdf2_step_of_the_exact_wave_gpu(W):
+    """The CUDA path's own residual and Jacobian close the Newton loop (no oracle involved)."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    c, mass_ratio, dt = 20.0, 25.0, 0.05
+    m = W.split_quad_mesh(32, 16, 0.0, 2.0 * np.pi, 0.0, np.pi)
+    g = api.Mesh.from_input(m)
+    ctx = api.Context(W.Physics(mass_ratio=mass_ratio, c=c))
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    def assemble_fn(P, Pn, Pm, dt_, jac):
+        rhs, vals = ctx.assemble(g, dev(P), dev(Pn), dev(Pm), dt_, jacobian=jac)
+        return rhs.cpu().numpy(), (vals.cpu().numpy() if jac else None)
+
+    x = m.centroids()[:, 0]
+    norms, P, Pn = newton_bdf2_step(assemble_fn, g.get("bsr_rowptr"), g.get("bsr_col"), g.n_cells, x, c, mass_ratio, dt)
+    ctx.check()
+    check_newton(norms, P, Pn, x, c, mass_ratio, dt)
