@@ -195,6 +195,7 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="linear lattice scale (tests only)")
     ap.add_argument("--cpu-rows", type=int, default=200000, help="rows of the oracle's timed sample")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--solve", action="store_true", help="also time the linear-solve step (SpMV, block-Jacobi, GMRES)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
@@ -322,6 +323,36 @@ def main():
                "note": "tfa_assemble_host: pinned host buffers, H2D of 3 states and D2H of rhs + BSR values inside"}
         del sh, rhs_h, vals_h
 
+    # ---- optional: the next step of the method, the linear solve on the assembled system ----
+    solve = None
+    if args.solve and rank == 0:
+        n = 18 * nc
+        xv = torch.randn(n, dtype=torch.float64, device="cuda")
+        yv = torch.empty_like(xv)
+        def timed(fn, reps):
+            fn(); torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record()
+            for _ in range(reps):
+                fn()
+            b.record(); torch.cuda.synchronize()
+            return a.elapsed_time(b) / reps
+        spmv_ms = timed(lambda: api.bsr_spmv(mesh, vals, xv, yv), 10)
+        dinv = torch.empty((nc, 18, 18), dtype=torch.float64, device="cuda")
+        bj_ms = timed(lambda: ctx.block_jacobi(mesh, vals, dinv), 3)
+        bvec = rhs.reshape(-1).contiguous()
+        tt = time.perf_counter()
+        xs, its, rel = ctx.gmres(mesh, vals, bvec, dinv=dinv, restart=30, max_iters=300, rtol=1e-6)
+        torch.cuda.synchronize()
+        gm_s = time.perf_counter() - tt
+        ctx.check()
+        spmv_bytes = nnzb * 2592 + 2 * n * 8 + nnzb * 4 + nc * 4
+        solve = {"spmv_ms": spmv_ms, "spmv_algorithmic_bytes": spmv_bytes,
+                 "spmv_gbs": spmv_bytes / (spmv_ms * 1e-3) / 1e9, "block_jacobi_ms": bj_ms,
+                 "gmres": {"restart": 30, "rtol": 1e-6, "iterations": its, "relative_residual": rel, "seconds": gm_s,
+                           "preconditioner": "block-Jacobi (18x18 diagonal blocks)"}}
+        del xv, yv, dinv, xs
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -356,6 +387,9 @@ def main():
                        "dt": wl.dt, "reorder": wl.reorder},
             "clocks": clocks, "e2e": e2e, "gpu_launches": ctx.launches_per_assemble * args.steps,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "setup": setup_ms}
+    if solve is not None:
+        line["solve"] = solve
+        line["solve"]["spmv_frac_of_hbm"] = solve["spmv_gbs"] / peak
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -39,7 +39,7 @@ extern "C" {
 #define TFA_NEQ 18
 #define TFA_BLOCK (TFA_NEQ * TFA_NEQ)
 
-enum { TFA_OK = 0, TFA_EINVAL = -1, TFA_EMESH = -2, TFA_ENOMEM = -3, TFA_ECUDA = -4, TFA_ENONPHYS = -5 };
+enum { TFA_OK = 0, TFA_EINVAL = -1, TFA_EMESH = -2, TFA_ENOMEM = -3, TFA_ECUDA = -4, TFA_ENONPHYS = -5, TFA_ESINGULAR = -6 };
 
 /* Physical constants of the model (the paper's "dco" of EulerMFMHDTerm, L177). */
 typedef struct tfa_physics {
@@ -144,6 +144,24 @@ int tfa_probe_copy(const double* src, double* dst, int64_t n, void* stream);
  * Newton steps in FP64), applied to x[0..n): sqrt_out[i], rcp_out[i].  DEVICE pointers.
  * Lets the tests bound their error against the correctly rounded results. */
 int tfa_probe_math(const double* x, double* sqrt_out, double* rcp_out, int64_t n, void* stream);
+
+/* ---- next step of the method: the linear solve of Eq. 14 (L123) on the assembled BSR system,
+ * restarted GMRES with a block-Jacobi preconditioner as in the paper's runs (L28, L392).  All vector and
+ * matrix arguments are DEVICE pointers owned by the caller; x, y, b have 18 * n_cells entries. ---- */
+/* y = A x for A = bsr_vals in the mesh's BSR pattern. */
+int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, double* y, void* stream);
+/* dinv [n_cells][18][18] = inverses of the diagonal blocks (Gauss-Jordan with partial pivoting, one warp per
+ * block).  A singular block (pivot 0 or not finite) gets a zero inverse and is reported by tfa_check as TFA_ESINGULAR. */
+int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream);
+/* Solve A x = b by right-preconditioned GMRES(restart): A M^-1 u = b, x = x0 + M^-1 u, M^-1 = dinv (block
+ * diagonal; NULL = no preconditioner).  x holds the initial guess on entry and the solution on return.
+ * Orthogonalisation: classical Gram-Schmidt applied twice; the small Hessenberg problem is solved on the host
+ * with Givens rotations (each iteration synchronises the stream).  Stops when the true residual norm
+ * ||b - A x|| <= rtol * ||b|| (checked at every restart; the recurrence's estimate ends a cycle) or after
+ * max_iters iterations.  info[0] = iterations done, info[1] = ||b - A x|| / ||b|| on return.
+ * The Krylov basis ((restart + 2) vectors) lives in the context's workspace. */
+int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
+              double* x, int restart, int max_iters, double rtol, double* info, void* stream);
 
 /* Per-kernel timing with CUDA events recorded on the launching stream (bench.py's roofline).
  * tfa_timing_enable(ctx, 1): every later tfa_assemble records events before, between and after

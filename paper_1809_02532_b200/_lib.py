@@ -52,6 +52,9 @@ SYMBOLS = {
     "tfa_probe_dfma": (_int, [_int, _int, _vp, _vp]),
     "tfa_probe_copy": (_int, [_vp, _vp, _i64, _vp]),
     "tfa_probe_math": (_int, [_vp, _vp, _vp, _i64, _vp]),
+    "tfa_bsr_spmv": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "tfa_block_jacobi": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "tfa_gmres": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
     "tfa_timing_enable": (_int, [_vp, _int]),
     "tfa_timing_read": (_int, [_vp, C.POINTER(C.c_double), C.POINTER(_int)]),
     "tfa_launches_per_assemble": (_int, [_vp]),

@@ -165,6 +165,22 @@ class Context:
                                                  hp(rhs), hp(vals), _stream()))
         return rhs, vals
 
+    def block_jacobi(self, mesh: Mesh, vals, dinv=None):
+        """tfa_block_jacobi: inverses of the diagonal blocks, [n_cells][18][18]."""
+        if dinv is None:
+            dinv = torch.empty((mesh.n_cells, NEQ, NEQ), dtype=torch.float64, device=vals.device)
+        _lib.check(_lib.load().tfa_block_jacobi(self._h, mesh._h, _dp(vals), _dp(dinv), _stream()))
+        return dinv
+
+    def gmres(self, mesh: Mesh, vals, b, x=None, dinv=None, restart=30, max_iters=300, rtol=1e-8):
+        """tfa_gmres: returns (x, iterations, relative residual).  x (initial guess) is updated in place."""
+        if x is None:
+            x = torch.zeros_like(b)
+        info = (C.c_double * 2)()
+        _lib.check(_lib.load().tfa_gmres(self._h, mesh._h, _dp(vals), _dp(dinv), _dp(b), _dp(x), int(restart),
+                                         int(max_iters), float(rtol), info, _stream()))
+        return x, int(info[0]), float(info[1])
+
     def check(self):
         _lib.check(_lib.load().tfa_check(self._h, _stream()))
 
@@ -210,6 +226,14 @@ def probe_math(x: torch.Tensor):
     s, r = torch.empty_like(x), torch.empty_like(x)
     _lib.check(_lib.load().tfa_probe_math(_dp(x), _dp(s), _dp(r), x.numel(), _stream()))
     return s, r
+
+
+def bsr_spmv(mesh: Mesh, vals: torch.Tensor, x: torch.Tensor, y: torch.Tensor | None = None):
+    """tfa_bsr_spmv: y = A x in the mesh's BSR pattern."""
+    if y is None:
+        y = torch.empty_like(x)
+    _lib.check(_lib.load().tfa_bsr_spmv(mesh._h, _dp(vals), _dp(x), _dp(y), _stream()))
+    return y
 
 
 # C-style aliases, same names as the ABI

@@ -171,6 +171,7 @@ int tfa_check(tfa_ctx* ctx, void* stream) {
   TFA_CUDA(cudaMemset(ctx->flags.p, 0, 16));
   if (h[0]) return set_error(TFA_ENONPHYS, "non-physical face state (rho <= 0 or T <= 0) met in " +
                                                std::to_string(h[0]) + " tiles");
+  if (h[1]) return set_error(TFA_ESINGULAR, "singular diagonal block in tfa_block_jacobi: " + std::to_string(h[1]));
   return 0;
 }
 

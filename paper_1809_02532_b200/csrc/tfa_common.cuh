@@ -98,6 +98,8 @@ struct tfa_ctx {
   tfa::DevBuf<double> lsq_coef;   // [nst][2]
   tfa::DevBuf<double> fown;       // [nc][3][18] own-side face states P_i + phi grad P_i . (x_f - x_i)  (L232)
   tfa::DevBuf<int32_t> flags;     // [4] device counters: 0 = non-physical states
+  // Krylov workspace of tfa_gmres: (restart + 2) vectors of 18 nc doubles, and reduction scratch
+  tfa::DevBuf<double> krylov, red;
   // staging for tfa_assemble_host
   tfa::DevBuf<double> h_state[3], h_rhs, h_vals;
   int launches = 0;

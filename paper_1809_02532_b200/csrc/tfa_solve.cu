@@ -1,0 +1,324 @@
+// tfa_solve.cu — the linear solve of Eq. 14 (L123) on the assembled BSR system: BSR
+// matrix-vector product, block-Jacobi preconditioner, restarted GMRES (the paper's solver configuration,
+// L28, L392).  Kernels are HBM-bound streams; the Hessenberg least-squares problem lives on the host.
+#include <cmath>
+#include <vector>
+
+#include "tfa_common.cuh"
+
+namespace tfa {
+
+constexpr int SV_CELLS = 16;              // cells per CTA: thread = (cell, scalar row)
+constexpr int SV_T = SV_CELLS * NEQ;      // 288 threads
+constexpr int MAXK = 64;                  // largest restart length
+
+// ------------------------------------------------------------------------------------------------
+// y = A x: thread (i, r) walks the blocks of BSR row i and reads scalar row r of each block (18 contiguous
+// doubles; the 18 threads of a cell read the whole 2592-byte block contiguously).  Algorithmic bytes =
+// the matrix (2592 per block) + x + y: HBM-bound.  With DIAG_ONLY the "matrix" is the block-diagonal
+// dinv [nc][18][18] (the preconditioner's application).
+// ------------------------------------------------------------------------------------------------
+template <bool DIAG_ONLY>
+__global__ void __launch_bounds__(SV_T) k_bsr_spmv(int64_t nc, const int32_t* __restrict__ rowptr,
+                                                  const int32_t* __restrict__ col, const double* __restrict__ vals,
+                                                  const double* __restrict__ x, double* __restrict__ y) {
+  const int r = threadIdx.x % NEQ;
+  const int64_t i = blockIdx.x * (int64_t)SV_CELLS + threadIdx.x / NEQ;
+  if (i >= nc) return;
+  const int64_t b0 = DIAG_ONLY ? i : rowptr[i], b1 = DIAG_ONLY ? i + 1 : rowptr[i + 1];
+  double acc = 0.0;
+  for (int64_t b = b0; b < b1; ++b) {
+    const int64_t j = DIAG_ONLY ? i : col[b];
+    const double2* __restrict__ a = reinterpret_cast<const double2*>(vals + b * BLK + r * NEQ);
+    const double2* __restrict__ xv = reinterpret_cast<const double2*>(x + NEQ * j);
+#pragma unroll
+    for (int c = 0; c < NEQ / 2; ++c) {
+      const double2 av = a[c], xx = xv[c];
+      acc = fma(av.x, xx.x, acc);
+      acc = fma(av.y, xx.y, acc);
+    }
+  }
+  y[NEQ * i + r] = acc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Inverse of each diagonal block: one warp per cell, Gauss-Jordan with partial pivoting on [A | I] in
+// shared memory (lane l < 18 owns row l).
+// ------------------------------------------------------------------------------------------------
+constexpr int BJ_WARPS = 4;
+__global__ void __launch_bounds__(32 * BJ_WARPS) k_block_jacobi(int64_t nc, const int32_t* __restrict__ rowptr,
+                                                               const int32_t* __restrict__ col,
+                                                               const double* __restrict__ vals,
+                                                               double* __restrict__ dinv, int32_t* __restrict__ flags) {
+  __shared__ double M[BJ_WARPS][NEQ][2 * NEQ + 1];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
+  if (i >= nc) return;
+  int64_t bd = -1;
+  for (int32_t b = rowptr[i]; b < rowptr[i + 1]; ++b)
+    if (col[b] == (int32_t)i) bd = b;
+  double(*A)[2 * NEQ + 1] = M[w];
+  for (int e = lane; e < BLK; e += 32) {
+    const int r = e / NEQ, c = e - NEQ * r;
+    A[r][c] = vals[bd * BLK + e];
+    A[r][NEQ + c] = r == c ? 1.0 : 0.0;
+  }
+  __syncwarp();
+  bool singular = false;
+  for (int k = 0; k < NEQ; ++k) {
+    // pivot: largest |A[r][k]| over r >= k (ties: smallest r)
+    double best = lane >= k && lane < NEQ ? fabs(A[lane][k]) : -1.0;
+    int arg = lane;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oa = __shfl_xor_sync(0xffffffffu, arg, o);
+      if (ob > best || (ob == best && oa < arg)) { best = ob; arg = oa; }
+    }
+    if (!(best > 0.0) || !isfinite(best)) { singular = true; break; }
+    if (arg != k) {   // swap rows k and arg
+      for (int c = lane; c < 2 * NEQ; c += 32) {
+        const double t = A[k][c];
+        A[k][c] = A[arg][c];
+        A[arg][c] = t;
+      }
+      __syncwarp();
+    }
+    const double ip = 1.0 / A[k][k];
+    __syncwarp();
+    for (int c = lane; c < 2 * NEQ; c += 32) A[k][c] *= ip;
+    __syncwarp();
+    if (lane < NEQ && lane != k) {
+      const double f = A[lane][k];
+      for (int c = 0; c < 2 * NEQ; ++c) A[lane][c] = fma(-f, A[k][c], A[lane][c]);
+    }
+    __syncwarp();
+  }
+  if (singular) {
+    if (lane == 0) atomicAdd(flags + 1, 1);
+    for (int e = lane; e < BLK; e += 32) dinv[i * BLK + e] = 0.0;
+    return;
+  }
+  for (int e = lane; e < BLK; e += 32) dinv[i * BLK + e] = A[e / NEQ][NEQ + e % NEQ];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Vector kernels of GMRES.  Reductions are two-pass and deterministic: pass 1 writes per-CTA partial sums,
+// pass 2 (one CTA) adds them in a fixed order.
+// ------------------------------------------------------------------------------------------------
+constexpr int RED_T = 256, RED_B = 592;
+
+// part[b][j] = sum over the CTA's share of V_j . w, j < k  (V_j = V + j * ld)
+__global__ void __launch_bounds__(RED_T) k_dots(int64_t n, int k, const double* __restrict__ V, int64_t ld,
+                                               const double* __restrict__ w, double* __restrict__ part) {
+  __shared__ double sm[RED_T / 32];
+  for (int j0 = 0; j0 < k; j0 += 8) {
+    double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const int kj = min(8, k - j0);
+    for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
+      const double we = w[e];
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        if (q < kj) acc[q] = fma(V[(j0 + q) * ld + e], we, acc[q]);
+    }
+    for (int q = 0; q < kj; ++q) {
+      double v = acc[q];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int t = 0; t < RED_T / 32; ++t) s += sm[t];
+        part[(int64_t)blockIdx.x * MAXK + j0 + q] = s;
+      }
+      __syncthreads();
+    }
+  }
+}
+__global__ void k_dots_final(int k, int nblocks, const double* __restrict__ part, double* __restrict__ out) {
+  const int j = threadIdx.x;
+  if (j >= k) return;
+  double s = 0.0;
+  for (int b = 0; b < nblocks; ++b) s += part[(int64_t)b * MAXK + j];
+  out[j] = s;
+}
+// w -= sum_j h[j] V_j
+__global__ void __launch_bounds__(RED_T) k_sub_combination(int64_t n, int k, const double* __restrict__ V, int64_t ld,
+                                                          const double* __restrict__ h, double* __restrict__ w) {
+  __shared__ double hs[MAXK];
+  if (threadIdx.x < k) hs[threadIdx.x] = h[threadIdx.x];
+  __syncthreads();
+  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
+    double v = w[e];
+    for (int j = 0; j < k; ++j) v = fma(-hs[j], V[j * ld + e], v);
+    w[e] = v;
+  }
+}
+// out = a * x + c * y   (y may be null with c = 0)
+__global__ void __launch_bounds__(RED_T) k_axpby(int64_t n, double a, const double* __restrict__ x, double c,
+                                                const double* __restrict__ y, double* __restrict__ out) {
+  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x)
+    out[e] = y ? fma(a, x[e], c * y[e]) : a * x[e];
+}
+
+
+namespace {
+
+struct Gm {
+  const tfa_mesh* m;
+  const double *vals, *dinv;
+  int64_t n;
+  cudaStream_t st;
+  double *part, *out;   // reduction scratch (device)
+  double host[MAXK];
+
+  void spmv(const double* x, double* y) const {
+    k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, vals, x, y);
+  }
+  // z = M^-1 v (block-diagonal product), or a copy without preconditioner
+  void precond(const double* v, double* z) const {
+    if (dinv) k_bsr_spmv<true><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, nullptr, nullptr, dinv, v, z);
+    else k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, v, 0.0, nullptr, z);
+  }
+  // host[j] = V_j . w for j < k (synchronises)
+  int dots(int k, const double* V, int64_t ld, const double* w) {
+    k_dots<<<RED_B, RED_T, 0, st>>>(n, k, V, ld, w, part);
+    k_dots_final<<<1, MAXK, 0, st>>>(k, RED_B, part, out);
+    TFA_CUDA(cudaMemcpyAsync(host, out, sizeof(double) * k, cudaMemcpyDeviceToHost, st));
+    TFA_CUDA(cudaStreamSynchronize(st));
+    return 0;
+  }
+};
+
+}  // namespace
+}  // namespace tfa
+
+using namespace tfa;
+
+extern "C" {
+
+int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, double* y, void* stream) {
+  if (!m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!bsr_vals || !x || !y) return set_error(TFA_EINVAL, "null argument");
+  k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, (cudaStream_t)stream>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p,
+                                                                            bsr_vals, x, y);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream) {
+  if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!bsr_vals || !dinv) return set_error(TFA_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!ctx->flags.p) {
+    TFA_CUDA(ctx->flags.alloc(4));
+    TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
+  }
+  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, bsr_vals, dinv,
+                                                                  ctx->flags.p);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
+              double* x, int restart, int max_iters, double rtol, double* info, void* stream) {
+  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
+  info[0] = 0.0;
+  info[1] = 0.0;
+  if (m->nc == 0) return 0;
+  if (!bsr_vals || !b || !x) return set_error(TFA_EINVAL, "null argument");
+  if (restart < 1 || restart > MAXK - 2 || max_iters < 0 || !(rtol >= 0.0))
+    return set_error(TFA_EINVAL, "tfa_gmres: restart must be in 1..62, max_iters >= 0, rtol >= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = (int64_t)NEQ * m->nc;
+  const int mk = restart;
+  if (ctx->krylov.n < (int64_t)(mk + 3) * n) TFA_CUDA(ctx->krylov.alloc((int64_t)(mk + 3) * n));
+  if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
+  double* V = ctx->krylov.p;              // V_0 .. V_mk
+  double* w = V + (int64_t)(mk + 1) * n;  // work vector
+  double* z = w + n;                      // preconditioned vector
+  Gm G{m, bsr_vals, dinv, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}};
+
+  TFA_TRY(G.dots(1, b, n, b));
+  const double bnorm = std::sqrt(G.host[0]);
+  if (bnorm == 0.0) {   // b = 0: x = 0
+    TFA_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+    return 0;
+  }
+  int iters = 0;
+  std::vector<double> H((size_t)(mk + 1) * mk), cs(mk), sn(mk), g(mk + 1), yv(mk);
+  double rel = 0.0;
+  for (;;) {
+    // r = b - A x  (true residual at every restart)
+    G.spmv(x, w);
+    k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, b, -1.0, w, w);
+    TFA_TRY(G.dots(1, w, n, w));
+    const double beta = std::sqrt(G.host[0]);
+    rel = beta / bnorm;
+    if (rel <= rtol || iters >= max_iters || !std::isfinite(beta)) break;
+    k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / beta, w, 0.0, nullptr, V);
+    std::fill(g.begin(), g.end(), 0.0);
+    g[0] = beta;
+    int k = 0;
+    for (; k < mk && iters < max_iters; ++k, ++iters) {
+      G.precond(V + (int64_t)k * n, z);
+      G.spmv(z, w);
+      // classical Gram-Schmidt, applied twice
+      double* h = &H[(size_t)k * (mk + 1)];
+      for (int j = 0; j <= k + 1; ++j) h[j] = 0.0;
+      for (int pass = 0; pass < 2; ++pass) {
+        TFA_TRY(G.dots(k + 1, V, n, w));
+        for (int j = 0; j <= k; ++j) h[j] += G.host[j];
+        TFA_CUDA(cudaMemcpyAsync(G.out, G.host, sizeof(double) * (k + 1), cudaMemcpyHostToDevice, st));
+        k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, G.out, w);
+        TFA_CUDA(cudaStreamSynchronize(st));   // G.host is reused by the next reduction
+      }
+      TFA_TRY(G.dots(1, w, n, w));
+      const double hk1 = std::sqrt(G.host[0]);
+      h[k + 1] = hk1;
+      if (hk1 > 0.0) k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / hk1, w, 0.0, nullptr, V + (int64_t)(k + 1) * n);
+      // Givens rotations on column k of the Hessenberg matrix
+      for (int j = 0; j < k; ++j) {
+        const double t = cs[j] * h[j] + sn[j] * h[j + 1];
+        h[j + 1] = -sn[j] * h[j] + cs[j] * h[j + 1];
+        h[j] = t;
+      }
+      const double den = std::hypot(h[k], h[k + 1]);
+      cs[k] = den > 0.0 ? h[k] / den : 1.0;
+      sn[k] = den > 0.0 ? h[k + 1] / den : 0.0;
+      h[k] = den;
+      h[k + 1] = 0.0;
+      g[k + 1] = -sn[k] * g[k];
+      g[k] = cs[k] * g[k];
+      if (std::fabs(g[k + 1]) <= rtol * bnorm || hk1 == 0.0) {
+        ++k;
+        ++iters;
+        break;
+      }
+    }
+    // y = H^-1 g (upper triangular), u = sum_j y_j V_j, x += M^-1 u
+    for (int i2 = k - 1; i2 >= 0; --i2) {
+      double sacc = g[i2];
+      for (int j = i2 + 1; j < k; ++j) sacc -= H[(size_t)j * (mk + 1) + i2] * yv[j];
+      yv[i2] = sacc / H[(size_t)i2 * (mk + 1) + i2];
+    }
+    if (k > 0) {
+      for (int j = 0; j < k; ++j) G.host[j] = -yv[j];
+      TFA_CUDA(cudaMemcpyAsync(G.out, G.host, sizeof(double) * k, cudaMemcpyHostToDevice, st));
+      TFA_CUDA(cudaMemsetAsync(w, 0, sizeof(double) * n, st));
+      k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k, V, n, G.out, w);   // w = sum_j y_j V_j
+      TFA_CUDA(cudaStreamSynchronize(st));
+      G.precond(w, z);
+      k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, z, 1.0, x, x);
+    }
+  }
+  TFA_CUDA(cudaGetLastError());
+  info[0] = (double)iters;
+  info[1] = rel;
+  return 0;
+}
+
+}  // extern "C"

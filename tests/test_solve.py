@@ -1,0 +1,167 @@
+"""Linear-solve step: oracle pins (-m "not gpu") and GPU parity (-m gpu)."""
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import scipy.sparse.linalg as spl
+
+
+def random_bsr(rng, n, extra=2, diag_boost=6.0):
+    """Random 18x18-block matrix: diagonal blocks plus `extra` off-diagonal blocks per row, columns ascending."""
+    rowptr, col = [0], []
+    for i in range(n):
+        others = rng.choice([j for j in range(n) if j != i], size=min(extra, n - 1), replace=False)
+        cols = sorted(set([i] + [int(j) for j in others]))
+        col += cols
+        rowptr.append(len(col))
+    rowptr, col = np.array(rowptr, dtype=np.int32), np.array(col, dtype=np.int32)
+    vals = rng.normal(size=(len(col), 18, 18))
+    for i in range(n):
+        b = rowptr[i] + int(np.nonzero(col[rowptr[i]:rowptr[i + 1]] == i)[0][0])
+        vals[b] += diag_boost * np.sqrt(18 * (extra + 1)) * np.eye(18)
+    return vals, rowptr, col
+
+
+# ---------------------------------------------------------------------------------------------------
+# oracle pins
+# ---------------------------------------------------------------------------------------------------
+def test_oracle_gmres_equals_the_direct_solution():
+    from oracle import solve
+    rng = np.random.default_rng(1)
+    vals, rp, col = random_bsr(rng, 12)
+    A = solve.bsr_matrix(vals, rp, col)
+    b = rng.normal(size=A.shape[0])
+    xd = spl.spsolve(A.tocsc(), b)
+    for dinv in (None, solve.block_jacobi(vals, rp, col)):
+        x, it, rel, est = solve.gmres(A, b, dinv=dinv, restart=20, max_iters=400, rtol=1e-12)
+        assert rel <= 1e-12 and np.abs(x - xd).max() <= 1e-9 * np.abs(xd).max()
+        # the recurrence's last estimate agrees with the true residual
+        assert abs(est[-1] - rel) <= 1e-3 * rel + 1e-14
+
+
+def test_oracle_full_gmres_terminates_in_n_steps():
+    """Without restart GMRES is exact after at most n steps (n = 36 here)."""
+    from oracle import solve
+    rng = np.random.default_rng(2)
+    vals, rp, col = random_bsr(rng, 2, extra=1, diag_boost=0.3)     # not diagonally dominant
+    A = solve.bsr_matrix(vals, rp, col)
+    b = rng.normal(size=36)
+    x, it, rel, est = solve.gmres(A, b, restart=36, max_iters=36, rtol=1e-13)
+    assert it <= 36 and rel <= 1e-10
+    assert np.abs(A @ x - b).max() <= 1e-9 * np.abs(b).max()
+
+
+def test_oracle_block_jacobi_makes_identity_on_block_diagonal_matrices():
+    from oracle import solve
+    rng = np.random.default_rng(3)
+    vals, rp, col = random_bsr(rng, 6, extra=0)
+    dinv = solve.block_jacobi(vals, rp, col)
+    A = solve.bsr_matrix(vals, rp, col)
+    v = rng.normal(size=A.shape[0])
+    assert np.abs(A @ solve.apply_block_diag(dinv, v) - v).max() <= 1e-12 * np.abs(v).max()
+    x, it, rel, _ = solve.gmres(A, v, dinv=dinv, restart=5, max_iters=5, rtol=1e-12)
+    assert it == 1 and rel <= 1e-12                    # exact preconditioner: one iteration
+
+
+# ---------------------------------------------------------------------------------------------------
+# GPU parity
+# ---------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def system(W):
+    """A real system: BDF2 Jacobian and rhs of the noisy wave (config-1 recipe) on 24 x 12 split quads."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    m = W.split_quad_mesh(24, 12)
+    g = api.Mesh.from_input(m)
+    g.reorder("rcm")
+    P = np.ascontiguousarray(W.wave_state(m.centroids(), seed=3)[g.get("perm")])
+    ctx = api.Context(W.Physics())
+    rhs, vals = ctx.assemble(g, torch.from_numpy(P).cuda(), dt=1e-2)
+    ctx.check()
+    return api, ctx, g, rhs, vals
+
+
+@pytest.mark.gpu
+def test_spmv_parity(system):
+    import torch
+    from oracle import solve
+    api, ctx, g, rhs, vals = system
+    rng = np.random.default_rng(4)
+    x = rng.normal(size=18 * g.n_cells)
+    y = api.bsr_spmv(g, vals, torch.from_numpy(x).cuda()).cpu().numpy()
+    A = solve.bsr_matrix(vals.cpu().numpy(), g.get("bsr_rowptr"), g.get("bsr_col"))
+    ref = A @ x
+    scale = abs(A) @ np.abs(x)                        # sum of |terms| per row
+    assert (np.abs(y - ref) <= 1e-14 * scale * 80).all()
+
+
+@pytest.mark.gpu
+def test_block_jacobi_parity_and_singular_block(system):
+    import torch
+    from oracle import solve
+    api, ctx, g, rhs, vals = system
+    dinv = ctx.block_jacobi(g, vals).cpu().numpy()
+    ctx.check()
+    ref = solve.block_jacobi(vals.cpu().numpy(), g.get("bsr_rowptr"), g.get("bsr_col"))
+    err = np.abs(dinv - ref).max(axis=(1, 2)) / np.abs(ref).max(axis=(1, 2))
+    assert err.max() <= 1e-10, err.max()
+    bad = vals.clone()
+    rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
+    b = rp[5] + int(np.nonzero(col[rp[5]:rp[6]] == 5)[0][0])
+    bad[b] = 0.0
+    ctx.block_jacobi(g, bad)
+    with pytest.raises(api.TfaError) as e:
+        ctx.check()
+    assert e.value.code == -6
+    ctx.check()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precond", [True, False])
+def test_gmres_parity(system, precond):
+    import torch
+    from oracle import solve
+    api, ctx, g, rhs, vals = system
+    rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
+    A = solve.bsr_matrix(vals.cpu().numpy(), rp, col)
+    b = rhs.cpu().numpy().ravel()
+    lu = spl.splu(A.tocsc())
+    xd = lu.solve(b)                                  # external pin: the direct solution
+    inv_op = spl.LinearOperator(A.shape, matvec=lu.solve, rmatvec=lambda v: lu.solve(v, "T"))
+    cond1 = spl.onenormest(A) * spl.onenormest(inv_op)
+    rtol = 1e-10 if precond else 1e-6          # the unpreconditioned iteration is slow on this stiff system
+    dinv_o = solve.block_jacobi(vals.cpu().numpy(), rp, col) if precond else None
+    xo, it_o, rel_o, _ = solve.gmres(A, b, dinv=dinv_o, restart=30, max_iters=600, rtol=rtol)
+    dinv = ctx.block_jacobi(g, vals) if precond else None
+    x, it, rel = ctx.gmres(g, vals, rhs.reshape(-1).contiguous(), dinv=dinv, restart=30, max_iters=600, rtol=rtol)
+    ctx.check()
+    x = x.cpu().numpy()
+    assert rel <= rtol and rel_o <= rtol, (rel, rel_o, it, it_o)
+    # the reported residual is the true one
+    assert abs(np.linalg.norm(b - A @ x) / np.linalg.norm(b) - rel) <= 1e-3 * rel + 1e-15
+    # both iterations stop within the tolerance of the direct solution; counts differ at most by the
+    # rounding of the stopping test (classical Gram-Schmidt twice here, modified Gram-Schmidt in the oracle)
+    tol = 10 * rtol * cond1
+    assert np.abs(x - xd).max() <= tol * np.abs(xd).max() and np.abs(xo - xd).max() <= tol * np.abs(xd).max()
+    assert abs(it - it_o) <= max(2, it_o // 20), (it, it_o)
+    if precond:
+        assert it < 600
+
+
+@pytest.mark.gpu
+def test_gmres_edge_cases(system):
+    import torch
+    api, ctx, g, rhs, vals = system
+    n = 18 * g.n_cells
+    z = torch.zeros(n, dtype=torch.float64, device="cuda")
+    x, it, rel = ctx.gmres(g, vals, z, x=torch.ones_like(z))          # b = 0  ->  x = 0
+    assert it == 0 and float(x.abs().max()) == 0.0
+    b = rhs.reshape(-1).contiguous()
+    x, it, rel = ctx.gmres(g, vals, b, max_iters=0)                    # no iterations allowed
+    assert it == 0 and rel == pytest.approx(1.0)
+    with pytest.raises(api.TfaError):
+        ctx.gmres(g, vals, b, restart=0)
+    # starting from the solution: nothing to do
+    xs, it1, rel1 = ctx.gmres(g, vals, b, dinv=ctx.block_jacobi(g, vals), rtol=1e-9)
+    x2, it2, rel2 = ctx.gmres(g, vals, b, x=xs.clone(), dinv=ctx.block_jacobi(g, vals), rtol=1e-9)
+    assert it2 == 0 and rel2 == pytest.approx(rel1)
