@@ -250,3 +250,73 @@ def test_newton_converges_on_a_bdf2_step_of_the_exact_wave_gpu(W):
     norms, P, Pn = newton_bdf2_step(assemble_fn, g.get("bsr_rowptr"), g.get("bsr_col"), g.n_cells, x, c, mass_ratio, dt)
     ctx.check()
     check_newton(norms, P, Pn, x, c, mass_ratio, dt)
+
+
+@pytest.mark.gpu
+def test_newton_with_device_gmres_on_a_bdf2_step_of_the_exact_wave(W):
+    """The whole implicit step on the device (Eq. 12-14): assembly, block-Jacobi GMRES (the paper's solver
+    configuration, L28, L392), update — no host solver and no oracle; lands on the exact solution."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    c, mass_ratio, dt = 20.0, 25.0, 0.05
+    m = W.split_quad_mesh(32, 16, 0.0, 2.0 * np.pi, 0.0, np.pi)
+    g = api.Mesh.from_input(m)
+    ctx = api.Context(W.Physics(mass_ratio=mass_ratio, c=c))
+    x = m.centroids()[:, 0]
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Pm, Pn = dev(exact_wave(x, 0.3 - dt, c, mass_ratio)[0]), dev(exact_wave(x, 0.3, c, mass_ratio)[0])
+    P = Pn.clone()
+    norms, iters = [], []
+    for _ in range(5):
+        rhs, vals = ctx.assemble(g, P, Pn, Pm, dt)
+        norms.append(float(rhs.abs().max()))
+        dP, it, rel = ctx.gmres(g, vals, rhs.reshape(-1).contiguous(), dinv=ctx.block_jacobi(g, vals), restart=30,
+                                max_iters=300, rtol=1e-9)
+        assert rel <= 1e-9
+        iters.append(it)
+        P = P + dP.reshape(-1, 18)
+    norms.append(float(ctx.assemble(g, P, Pn, Pm, dt, jacobian=False)[0].abs().max()))
+    ctx.check()
+    assert max(iters) < 300
+    check_newton(np.array(norms), P.cpu().numpy(), Pn.cpu().numpy(), x, c, mass_ratio, dt)
+
+
+@pytest.mark.gpu
+def test_wave_propagation_converges_at_second_order_with_the_device_solver(W):
+    """The paper's own validation (section 4.1.1, Fig. 6): the circularly polarised wave advanced with the
+    implicit BDF2 / Newton scheme at CFL > 1 (light-speed CFL 5), L2 error of the perpendicular magnetic field
+    against the exact solution falling at second order or better with the mesh.  Everything on the device:
+    assembly, block-Jacobi GMRES, update."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    c, mass_ratio, tend, cfl = 20.0, 25.0, 1.0, 5.0
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    def l2_error(n):
+        m = W.split_quad_mesh(2 * n, n, 0.0, 2.0 * np.pi, 0.0, np.pi)
+        g = api.Mesh.from_input(m)
+        ctx = api.Context(W.Physics(mass_ratio=mass_ratio, c=c))
+        x = m.centroids()[:, 0]
+        h = 2.0 * np.pi / (2 * n)
+        nsteps = int(np.ceil(tend / (cfl * h / c)))
+        dt = tend / nsteps
+        Pm, Pn = dev(exact_wave(x, -dt, c, mass_ratio)[0]), dev(exact_wave(x, 0.0, c, mass_ratio)[0])
+        for _ in range(nsteps):
+            P = Pn.clone()
+            for _ in range(3):                               # Newton sub-iterations (Eq. 14)
+                rhs, vals = ctx.assemble(g, P, Pn, Pm, dt)
+                dP, it, rel = ctx.gmres(g, vals, rhs.reshape(-1).contiguous(), dinv=ctx.block_jacobi(g, vals),
+                                        restart=30, max_iters=300, rtol=1e-8)
+                assert rel <= 1e-8
+                P = P + dP.reshape(-1, 18)
+            Pm, Pn = Pn, P
+        ctx.check()
+        e = Pn.cpu().numpy() - exact_wave(x, tend, c, mass_ratio)[0]
+        return np.sqrt((e ** 2).mean(axis=0))
+
+    coarse, fine = l2_error(8), l2_error(16)
+    for v in (1, 2, 4, 5, 11, 12, 14, 15):                   # B_perp, E_perp, transverse velocities
+        assert coarse[v] / fine[v] > 3.5, (v, coarse[v], fine[v])
+    assert fine[1] < 1e-2 * ETA                              # 1 % of the wave amplitude on 32 x 16 quads
