@@ -346,9 +346,12 @@ def main():
         torch.cuda.synchronize()
         gm_s = time.perf_counter() - tt
         ctx.check()
+        jv = torch.empty_like(xv)
+        jvp_ms = timed(lambda: ctx.jvp(mesh, P, xv, Pn, Pnm1, wl.dt, eps=1e-7, out=jv), 5)
         spmv_bytes = nnzb * 2592 + 2 * n * 8 + nnzb * 4 + nc * 4
         solve = {"spmv_ms": spmv_ms, "spmv_algorithmic_bytes": spmv_bytes,
                  "spmv_gbs": spmv_bytes / (spmv_ms * 1e-3) / 1e9, "block_jacobi_ms": bj_ms,
+                 "jvp_ms": jvp_ms, "jvp_note": "tfa_jvp: two residual-only assemblies (base + perturbed) and two axpby",
                  "gmres": {"restart": 30, "rtol": 1e-6, "iterations": its, "relative_residual": rel, "seconds": gm_s,
                            "preconditioner": "block-Jacobi (18x18 diagonal blocks)"}}
         del xv, yv, dinv, xs

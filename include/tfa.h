@@ -163,6 +163,18 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
 int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
               double* x, int restart, int max_iters, double rtol, double* info, void* stream);
 
+/* ---- matrix-free operator (the paper's future work, L130): out = (dR~/dP) v by a forward
+ * difference of the residual-only assembly, (R~(P + eps v) - R~(P)) / eps — the full dependence, gradient and
+ * limiter included (the assembled Jacobian freezes them, S8).  eps <= 0: eps = 1e-7 (1 + rms(P)) / rms(v).
+ * DEVICE pointers; synchronises the stream when eps is chosen automatically. */
+int tfa_jvp(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n, const double* state_nm1,
+            double dt, const double* v, double* out, double eps, void* stream);
+/* tfa_gmres with that operator in place of the assembled matrix (no 10 KB/cell Jacobian to write or read); dinv
+ * (optional) is a block-Jacobi preconditioner from an assembled, possibly lagged, Jacobian. */
+int tfa_gmres_jfnk(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                   const double* state_nm1, double dt, const double* dinv, const double* b, double* x, int restart,
+                   int max_iters, double rtol, double* info, void* stream);
+
 /* Per-kernel timing with CUDA events recorded on the launching stream (bench.py's roofline).
  * tfa_timing_enable(ctx, 1): every later tfa_assemble records events before, between and after
  * its two kernels and accumulates their durations at the next tfa_timing_read, which

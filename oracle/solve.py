@@ -81,3 +81,9 @@ def gmres(A, b, x0=None, dinv=None, restart=30, max_iters=300, rtol=1e-8):
                 break
         y = np.linalg.solve(np.triu(H[:k, :k]), g[:k]) if k > 0 else np.zeros(0)
         x = x + Minv(V[:k].T @ y)
+
+
+def jvp(rhs_fn, P, v, eps):
+    """Matrix-free Jacobian action ("Jacobian-free" variant): (R~(P + eps v) - R~(P)) / eps with
+    rhs_fn(P) = -R~(P) the oracle's residual-only assembly (gradient and limiter recomputed, not frozen)."""
+    return -(rhs_fn(P + eps * v) - rhs_fn(P)) / eps

@@ -55,6 +55,8 @@ SYMBOLS = {
     "tfa_bsr_spmv": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "tfa_block_jacobi": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "tfa_gmres": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
+    "tfa_jvp": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _dbl, _vp]),
+    "tfa_gmres_jfnk": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
     "tfa_timing_enable": (_int, [_vp, _int]),
     "tfa_timing_read": (_int, [_vp, C.POINTER(C.c_double), C.POINTER(_int)]),
     "tfa_launches_per_assemble": (_int, [_vp]),

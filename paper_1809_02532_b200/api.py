@@ -181,6 +181,29 @@ class Context:
                                          int(max_iters), float(rtol), info, _stream()))
         return x, int(info[0]), float(info[1])
 
+    def jvp(self, mesh: Mesh, state, v, state_n=None, state_nm1=None, dt=1e-3, eps=0.0, out=None):
+        """tfa_jvp: (dR~/dP) v by a forward difference of the residual (matrix-free)."""
+        state_n = state if state_n is None else state_n
+        state_nm1 = state if state_nm1 is None else state_nm1
+        if out is None:
+            out = torch.empty_like(v)
+        _lib.check(_lib.load().tfa_jvp(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt), _dp(v),
+                                       _dp(out), float(eps), _stream()))
+        return out
+
+    def gmres_jfnk(self, mesh: Mesh, state, b, state_n=None, state_nm1=None, dt=1e-3, x=None, dinv=None, restart=30,
+                   max_iters=300, rtol=1e-8):
+        """tfa_gmres_jfnk: returns (x, iterations, relative residual)."""
+        state_n = state if state_n is None else state_n
+        state_nm1 = state if state_nm1 is None else state_nm1
+        if x is None:
+            x = torch.zeros_like(b)
+        info = (C.c_double * 2)()
+        _lib.check(_lib.load().tfa_gmres_jfnk(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
+                                              _dp(dinv), _dp(b), _dp(x), int(restart), int(max_iters), float(rtol),
+                                              info, _stream()))
+        return x, int(info[0]), float(info[1])
+
     def check(self):
         _lib.check(_lib.load().tfa_check(self._h, _stream()))
 

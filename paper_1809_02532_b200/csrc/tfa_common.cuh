@@ -100,6 +100,8 @@ struct tfa_ctx {
   tfa::DevBuf<int32_t> flags;     // [4] device counters: 0 = non-physical states
   // Krylov workspace of tfa_gmres: (restart + 2) vectors of 18 nc doubles, and reduction scratch
   tfa::DevBuf<double> krylov, red;
+  // matrix-free operator: perturbed state and its residual; the base residual
+  tfa::DevBuf<double> jfnk, jfnk0;
   // staging for tfa_assemble_host
   tfa::DevBuf<double> h_state[3], h_rhs, h_vals;
   int launches = 0;

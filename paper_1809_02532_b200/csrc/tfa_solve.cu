@@ -2,6 +2,7 @@
 // matrix-vector product, block-Jacobi preconditioner, restarted GMRES (the paper's solver configuration,
 // L28, L392).  Kernels are HBM-bound streams; the Hessenberg least-squares problem lives on the host.
 #include <cmath>
+#include <functional>
 #include <vector>
 
 #include "tfa_common.cuh"
@@ -172,9 +173,12 @@ struct Gm {
   cudaStream_t st;
   double *part, *out;   // reduction scratch (device)
   double host[MAXK];
+  std::function<int(const double*, double*)> op;   // y = A x when the matrix is not assembled (JFNK)
 
-  void spmv(const double* x, double* y) const {
+  int spmv(const double* x, double* y) const {
+    if (op) return op(x, y);
     k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, vals, x, y);
+    return 0;
   }
   // z = M^-1 v (block-diagonal product), or a copy without preconditioner
   void precond(const double* v, double* z) const {
@@ -196,40 +200,9 @@ struct Gm {
 
 using namespace tfa;
 
-extern "C" {
-
-int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, double* y, void* stream) {
-  if (!m) return set_error(TFA_EINVAL, "null argument");
-  if (m->nc == 0) return 0;
-  if (!bsr_vals || !x || !y) return set_error(TFA_EINVAL, "null argument");
-  k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, (cudaStream_t)stream>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p,
-                                                                            bsr_vals, x, y);
-  TFA_CUDA(cudaGetLastError());
-  return 0;
-}
-
-int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream) {
-  if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
-  if (m->nc == 0) return 0;
-  if (!bsr_vals || !dinv) return set_error(TFA_EINVAL, "null argument");
-  cudaStream_t st = (cudaStream_t)stream;
-  if (!ctx->flags.p) {
-    TFA_CUDA(ctx->flags.alloc(4));
-    TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
-  }
-  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, bsr_vals, dinv,
-                                                                  ctx->flags.p);
-  TFA_CUDA(cudaGetLastError());
-  return 0;
-}
-
-int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
-              double* x, int restart, int max_iters, double rtol, double* info, void* stream) {
-  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
-  info[0] = 0.0;
-  info[1] = 0.0;
-  if (m->nc == 0) return 0;
-  if (!bsr_vals || !b || !x) return set_error(TFA_EINVAL, "null argument");
+static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv,
+                      std::function<int(const double*, double*)> op, const double* b, double* x, int restart,
+                      int max_iters, double rtol, double* info, void* stream) {
   if (restart < 1 || restart > MAXK - 2 || max_iters < 0 || !(rtol >= 0.0))
     return set_error(TFA_EINVAL, "tfa_gmres: restart must be in 1..62, max_iters >= 0, rtol >= 0");
   cudaStream_t st = (cudaStream_t)stream;
@@ -240,7 +213,7 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
   double* V = ctx->krylov.p;              // V_0 .. V_mk
   double* w = V + (int64_t)(mk + 1) * n;  // work vector
   double* z = w + n;                      // preconditioned vector
-  Gm G{m, bsr_vals, dinv, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}};
+  Gm G{m, bsr_vals, dinv, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, op};
 
   TFA_TRY(G.dots(1, b, n, b));
   const double bnorm = std::sqrt(G.host[0]);
@@ -253,7 +226,7 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
   double rel = 0.0;
   for (;;) {
     // r = b - A x  (true residual at every restart)
-    G.spmv(x, w);
+    TFA_TRY(G.spmv(x, w));
     k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, b, -1.0, w, w);
     TFA_TRY(G.dots(1, w, n, w));
     const double beta = std::sqrt(G.host[0]);
@@ -265,7 +238,7 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
     int k = 0;
     for (; k < mk && iters < max_iters; ++k, ++iters) {
       G.precond(V + (int64_t)k * n, z);
-      G.spmv(z, w);
+      TFA_TRY(G.spmv(z, w));
       // classical Gram-Schmidt, applied twice
       double* h = &H[(size_t)k * (mk + 1)];
       for (int j = 0; j <= k + 1; ++j) h[j] = 0.0;
@@ -321,4 +294,107 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
   return 0;
 }
 
+
+extern "C" {
+
+int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, double* y, void* stream) {
+  if (!m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!bsr_vals || !x || !y) return set_error(TFA_EINVAL, "null argument");
+  k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, (cudaStream_t)stream>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p,
+                                                                            bsr_vals, x, y);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream) {
+  if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!bsr_vals || !dinv) return set_error(TFA_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!ctx->flags.p) {
+    TFA_CUDA(ctx->flags.alloc(4));
+    TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
+  }
+  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, bsr_vals, dinv,
+                                                                  ctx->flags.p);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
+              double* x, int restart, int max_iters, double rtol, double* info, void* stream) {
+  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
+  info[0] = 0.0;
+  info[1] = 0.0;
+  if (m->nc == 0) return 0;
+  if (!bsr_vals || !b || !x) return set_error(TFA_EINVAL, "null argument");
+  return gmres_core(ctx, m, bsr_vals, dinv, nullptr, b, x, restart, max_iters, rtol, info, stream);
+}
+
+// ---- matrix-free operator (the paper's future work, L130) ----
+static int jvp_core(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                    const double* state_nm1, double dt, const double* rhs0, const double* v, double* out, double eps,
+                    double rms_state, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = (int64_t)NEQ * m->nc;
+  if (ctx->jfnk.n < 2 * n) TFA_CUDA(ctx->jfnk.alloc(2 * n));
+  if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
+  double *Pp = ctx->jfnk.p, *rp = Pp + n;
+  if (!(eps > 0.0)) {
+    // eps = 1e-7 (1 + rms(P)) / rms(v)
+    Gm G{m, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
+    TFA_TRY(G.dots(1, v, n, v));
+    const double rv = std::sqrt(G.host[0] / (double)n);
+    if (rv == 0.0) {
+      TFA_CUDA(cudaMemsetAsync(out, 0, sizeof(double) * n, st));
+      return 0;
+    }
+    if (rms_state < 0.0) {
+      TFA_TRY(G.dots(1, state, n, state));
+      rms_state = std::sqrt(G.host[0] / (double)n);
+    }
+    eps = 1e-7 * (1.0 + rms_state) / rv;
+  }
+  k_axpby<<<RED_B, RED_T, 0, st>>>(n, eps, v, 1.0, state, Pp);                                  // P + eps v
+  TFA_TRY(tfa_assemble(ctx, m, Pp, state_n, state_nm1, dt, rp, nullptr, stream));              // rhs = -R~
+  k_axpby<<<RED_B, RED_T, 0, st>>>(n, -1.0 / eps, rp, 1.0 / eps, rhs0, out);                    // (R~' - R~) / eps
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_jvp(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n, const double* state_nm1,
+            double dt, const double* v, double* out, double eps, void* stream) {
+  if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!state || !state_n || !state_nm1 || !v || !out) return set_error(TFA_EINVAL, "null argument");
+  const int64_t n = (int64_t)NEQ * m->nc;
+  if (ctx->jfnk0.n < n) TFA_CUDA(ctx->jfnk0.alloc(n));
+  TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream));
+  return jvp_core(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, v, out, eps, -1.0, stream);
+}
+
+int tfa_gmres_jfnk(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                   const double* state_nm1, double dt, const double* dinv, const double* b, double* x, int restart,
+                   int max_iters, double rtol, double* info, void* stream) {
+  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
+  info[0] = 0.0;
+  info[1] = 0.0;
+  if (m->nc == 0) return 0;
+  if (!state || !state_n || !state_nm1 || !b || !x) return set_error(TFA_EINVAL, "null argument");
+  if (!(dt > 0.0)) return set_error(TFA_EINVAL, "dt must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = (int64_t)NEQ * m->nc;
+  if (ctx->jfnk0.n < n) TFA_CUDA(ctx->jfnk0.alloc(n));
+  if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
+  // the base residual and the state's size, once per solve
+  TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream));
+  Gm G{m, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
+  TFA_TRY(G.dots(1, state, n, state));
+  const double rms_state = std::sqrt(G.host[0] / (double)n);
+  auto op = [=](const double* xin, double* yout) -> int {
+    return jvp_core(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, xin, yout, 0.0, rms_state, stream);
+  };
+  return gmres_core(ctx, m, nullptr, dinv, op, b, x, restart, max_iters, rtol, info, stream);
+}
 }  // extern "C"

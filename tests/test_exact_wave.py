@@ -320,3 +320,36 @@ def test_wave_propagation_converges_at_second_order_with_the_device_solver(W):
     for v in (1, 2, 4, 5, 11, 12, 14, 15):                   # B_perp, E_perp, transverse velocities
         assert coarse[v] / fine[v] > 3.5, (v, coarse[v], fine[v])
     assert fine[1] < 1e-2 * ETA                              # 1 % of the wave amplitude on 32 x 16 quads
+
+
+@pytest.mark.gpu
+def test_newton_jfnk_contracts_faster_than_the_frozen_jacobian(W):
+    """Matrix-free Newton (the paper's future work, L130) on the same BDF2 step: the operator carries the
+    gradient / limiter dependence the assembled Jacobian freezes (S8), so Newton contracts much faster."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    c, mass_ratio, dt = 20.0, 25.0, 0.05
+    m = W.split_quad_mesh(32, 16, 0.0, 2.0 * np.pi, 0.0, np.pi)
+    g = api.Mesh.from_input(m)
+    ctx = api.Context(W.Physics(mass_ratio=mass_ratio, c=c))
+    x = m.centroids()[:, 0]
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Pm, Pn = dev(exact_wave(x, 0.3 - dt, c, mass_ratio)[0]), dev(exact_wave(x, 0.3, c, mass_ratio)[0])
+    P = Pn.clone()
+    norms = []
+    for _ in range(3):
+        rhs, vals = ctx.assemble(g, P, Pn, Pm, dt)
+        norms.append(float(rhs.abs().max()))
+        dP, it, rel = ctx.gmres_jfnk(g, P, rhs.reshape(-1).contiguous(), Pn, Pm, dt, dinv=ctx.block_jacobi(g, vals),
+                                     restart=30, max_iters=300, rtol=1e-5)   # inexact Newton; FD operator noise ~1e-8
+        assert rel <= 1e-5 and it < 300
+        P = P + dP.reshape(-1, 18)
+    norms.append(float(ctx.assemble(g, P, Pn, Pm, dt, jacobian=False)[0].abs().max()))
+    ctx.check()
+    norms = np.array(norms)
+    # frozen Jacobian: factor 0.04 .. 0.3 per iteration
+    assert norms[1] < 0.02 * norms[0] and norms[2] < 0.02 * norms[1] and norms[3] < 1e-6 * norms[0], norms
+    Pex = exact_wave(x, 0.3 + dt, c, mass_ratio)[0]
+    err, change = np.abs(P.cpu().numpy() - Pex).max(axis=0), np.abs(Pn.cpu().numpy() - Pex).max(axis=0)
+    assert (err[[1, 2, 11, 12]] < 0.06 * change[[1, 2, 11, 12]]).all()

@@ -165,3 +165,85 @@ def test_gmres_edge_cases(system):
     xs, it1, rel1 = ctx.gmres(g, vals, b, dinv=ctx.block_jacobi(g, vals), rtol=1e-9)
     x2, it2, rel2 = ctx.gmres(g, vals, b, x=xs.clone(), dinv=ctx.block_jacobi(g, vals), rtol=1e-9)
     assert it2 == 0 and rel2 == pytest.approx(rel1)
+
+
+# ---------------------------------------------------------------------------------------------------
+# matrix-free operator
+# ---------------------------------------------------------------------------------------------------
+def _wave_case(W, orc):
+    m = W.split_quad_mesh(12, 8)
+    P = W.wave_state(m.centroids(), seed=7)
+    o = orc.OracleMesh.from_input(m)
+    pc = orc.physics_c(W.Physics())
+    nu = orc.default_numerics(pc)
+    return m, P, o, pc, nu
+
+
+def test_oracle_jvp_against_central_differences(orc, W):
+    """Forward difference of the oracle residual against the central one with a larger step (brute force)."""
+    from oracle import solve
+    m, P, o, pc, nu = _wave_case(W, orc)
+    rhs_fn = lambda Q: orc.assemble(o, pc, nu, Q, P, P, 1e-2, jacobian=False)[0]
+    rng = np.random.default_rng(8)
+    v = rng.normal(size=P.shape) * np.maximum(np.abs(P), 1e-2)
+    fwd = solve.jvp(rhs_fn, P, v, 1e-7)
+    h = 1e-5
+    cen = -(rhs_fn(P + h * v) - rhs_fn(P - h * v)) / (2 * h)
+    assert np.abs(fwd - cen).max() <= 2e-4 * np.abs(cen).max()
+
+
+@pytest.mark.gpu
+def test_jvp_parity(W, orc):
+    import torch
+    from oracle import solve
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    m, P, o, pc, nu = _wave_case(W, orc)
+    g = api.Mesh.from_input(m)
+    ctx = api.Context(W.Physics())
+    rng = np.random.default_rng(9)
+    v = rng.normal(size=P.shape) * np.maximum(np.abs(P), 1e-2)
+    eps = 1e-6
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = ctx.jvp(g, dev(P), dev(v).reshape(-1), dt=1e-2, eps=eps).cpu().numpy().reshape(-1, 18)
+    ctx.check()
+    rhs_fn = lambda Q: orc.assemble(o, pc, nu, Q, P, P, 1e-2, jacobian=False)[0]
+    ref = solve.jvp(rhs_fn, P, v, eps)
+    scale = orc.assemble(o, pc, nu, P, P, P, 1e-2, jacobian=False)[1]      # sum of |terms| of the residual
+    # two residuals, each within 1e-12 of its scale (S18; measured 4e-16), differenced and divided by eps
+    assert (np.abs(out - ref).max(axis=0) <= 2e-14 / eps * scale.max(axis=0)).all()
+    # automatic step: same operator up to the O(eps) truncation of the forward difference
+    auto = ctx.jvp(g, dev(P), dev(v).reshape(-1), dt=1e-2).cpu().numpy().reshape(-1, 18)
+    assert np.abs(auto - ref).max() <= 1e-3 * np.abs(ref).max()
+
+
+@pytest.mark.gpu
+def test_gmres_jfnk_solves_the_newton_system(W, orc):
+    """Matrix-free GMRES (block-Jacobi from the assembled, frozen Jacobian as preconditioner) against the same
+    solve done on the host with the oracle's matrix-free operator; and against the assembled-matrix solve, from
+    which it differs only by the frozen-gradient terms."""
+    import torch
+    from oracle import solve
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    m, P, o, pc, nu = _wave_case(W, orc)
+    g = api.Mesh.from_input(m)
+    ctx = api.Context(W.Physics())
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Pd = dev(P)
+    rhs, vals = ctx.assemble(g, Pd, dt=1e-2)
+    dinv = ctx.block_jacobi(g, vals)
+    b = rhs.reshape(-1).contiguous()
+    # (the forward difference leaves operator noise of about 1e-9 relative: 1e-6 is a reachable tolerance)
+    x, it, rel = ctx.gmres_jfnk(g, Pd, b, dt=1e-2, dinv=dinv, restart=40, max_iters=400, rtol=1e-6)
+    ctx.check()
+    assert rel <= 1e-6 and it < 400
+    # the solution satisfies the matrix-free system as the oracle sees it
+    rhs_fn = lambda Q: orc.assemble(o, pc, nu, Q, P, P, 1e-2, jacobian=False)[0]
+    xs = x.cpu().numpy().reshape(-1, 18)
+    eps = 1e-7 * (1.0 + np.sqrt((P ** 2).mean())) / np.sqrt((xs ** 2).mean())
+    r = rhs.cpu().numpy() - solve.jvp(rhs_fn, P, xs, eps)
+    assert np.linalg.norm(r) <= 1e-4 * np.linalg.norm(rhs.cpu().numpy())
+    # and is close to the frozen-Jacobian solution
+    xa, _, _ = ctx.gmres(g, vals, b, dinv=dinv, restart=40, max_iters=400, rtol=1e-8)
+    assert float((x - xa).norm() / xa.norm()) < 0.5
