@@ -20,8 +20,7 @@
 //    (8x8, 5x5, 5x5), the source (Eq. 4/6) couples the blocks on the diagonal block only.
 //  * 18x18 blocks are staged in shared memory (their structural zeros are written once per CTA)
 //    and leave the SM as 2592-byte TMA bulk stores (cp.async.bulk.global.shared::cta).
-//  * The TFA_ASM_* switches below select variants that were measured and rejected;
-//    the defaults are the measured best.
+//  * The TFA_ASM_* constants below were tuned by measurement (DESIGN.md 6.3 lists what was tried).
 #include <cstdlib>
 
 #include "tfa_common.cuh"
@@ -30,12 +29,6 @@
 #ifndef TFA_ASM_EARLY2
 #define TFA_ASM_EARLY2 1   // bit 0: AUSM lanes, bit 1: Maxwell lanes evaluate all three faces before the first barrier
 #endif
-#ifndef TFA_ASM_VEC3
-#define TFA_ASM_VEC3 0     // AUSM lanes evaluate their three faces through ausm_flux_n<3>
-#endif
-#ifndef TFA_ASM_L2HINT
-#define TFA_ASM_L2HINT 0   // bit 0: bulk stores evict_first, bit 1: bulk loads evict_last
-#endif
 #ifndef TFA_ASM_BLKP
 #define TFA_ASM_BLKP 330   // doubles between staged blocks (324 = dense)
 #endif
@@ -43,7 +36,7 @@
 #define TFA_ASM_T 10      // cells per tile (multiple of 5)
 #endif
 #ifndef TFA_ASM_NM
-#define TFA_ASM_NM 2   // mirror staging buffers per tile (1..3): fewer CTA barriers against more shared memory
+#define TFA_ASM_NM 2   // mirror staging buffers per tile (the barrier sequence is written for 2)
 #endif
 
 namespace tfa {
@@ -55,17 +48,8 @@ constexpr int BLKP = TFA_ASM_BLKP;
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void bulk_store(void* gdst, const void* ssrc, uint32_t bytes) {
   const uint32_t s = (uint32_t)__cvta_generic_to_shared(ssrc);
-#if TFA_ASM_L2HINT & 1
-  // the Jacobian is written once and not read again by this kernel: first in line for eviction from L2
-  uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst), "r"(s),
-               "r"(bytes), "l"(pol)
-               : "memory");
-#else
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(s), "r"(bytes)
                : "memory");
-#endif
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 // all bulk stores of this thread have finished READING shared memory (the staging may be reused)
@@ -95,21 +79,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   } while (!done);
 }
 __device__ __forceinline__ void bulk_load(void* sdst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
-#if TFA_ASM_L2HINT & 2
-  // face states are read twice (by the cell and by its neighbour): keep them in L2 against the write stream
-  uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
-          smem_u32(sdst)),
-      "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
-      : "memory");
-#else
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
                    smem_u32(sdst)),
                "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
-#endif
 }
 // pull one 128-byte line towards L2 ahead of use (read latency under the Jacobian's write stream is long)
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -423,69 +396,10 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     constexpr bool EARLY2 = TFA_ASM_EARLY2 & (ROLE == 2 ? 2 : 1);   // evaluate face 2 together with faces 0, 1
 
     double d0[NV], d1[NV], d2[NV];
-    bool bnd0, bnd1, bnd2 = false;
-    if (ROLE != 2 && EARLY2 && TFA_ASM_VEC3) {
-      // AUSM lanes: VF faces through one face-vectorised flux call (interleaved dependency chains)
-      constexpr int VF = TFA_ASM_VEC3 >= 3 ? 3 : 2;
-      double own[VF][5], oth[VF][5], nrm[VF][2], H[VF][5];
-      bool bn[VF], okf[VF];
-#pragma unroll
-      for (int k = 0; k < VF; ++k) {
-        const int32_t nf = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);
-        bn[k] = nf < 0;
-        const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);
-        nrm[k][0] = g01.x;
-        nrm[k][1] = g01.y;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          own[k][q] = in.fo[ca][k][vidx<ROLE>(q)] + me[q];
-          oth[k][q] = in.fx[ca][k][vidx<ROLE>(q)];
-        }
-      }
-      bool anyb = false;
-#pragma unroll
-      for (int k = 0; k < VF; ++k) anyb |= bn[k];
-      if (__any_sync(0xffffffffu, anyb)) {
-        // boundary face: P_R := P_L, so the perturbation moves both arguments (S9)
-#pragma unroll
-        for (int k = 0; k < VF; ++k)
-          if (bn[k]) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) oth[k][q] = own[k][q];
-          }
-      }
-      if (run) {
-        ausm_flux_n<VF>(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nrm, H, okf);
-        bool okall = true;
-#pragma unroll
-        for (int k = 0; k < VF; ++k) okall &= okf[k];
-        if (!pert && act) nonphys |= !okall;
-      } else {
-#pragma unroll
-        for (int k = 0; k < VF; ++k)
-#pragma unroll
-          for (int q = 0; q < 5; ++q) H[k][q] = 0.0;
-      }
-#pragma unroll
-      for (int k = 0; k < VF; ++k) {
-        const double len = cg[8 * k + 2];
-        const double f = pert ? len * inv_e : len;
-        double* d = k == 0 ? d0 : (k == 1 ? d1 : d2);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const double hb = __shfl_sync(0xffffffffu, H[k][q], base_lane);
-          d[q] = __dmul_rn(__fma_rn(-hb, pm, H[k][q]), f);
-        }
-      }
-      bnd0 = bn[0];
-      bnd1 = bn[1];
-      if (VF == 3) bnd2 = bn[VF - 1];
-      else bnd2 = face(2, d2);
-    } else {
-      bnd0 = face(0, d0);
-      bnd1 = face(1, d1);
-      if (EARLY2) bnd2 = face(2, d2);
-    }
+    const bool bnd0 = face(0, d0);
+    const bool bnd1 = face(1, d1);
+    bool bnd2 = false;
+    if (EARLY2) bnd2 = face(2, d2);
     // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
     // them.  This barrier also publishes S.rs / S.s0 of the tile.
     if (ROLE == 0 && tid < T) bulk_wait_read();

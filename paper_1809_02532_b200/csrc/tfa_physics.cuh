@@ -166,81 +166,6 @@ __device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, doubl
   return ok;
 }
 
-// The same scheme for NF faces at once, every statement written across the faces, so that the
-// NF dependency chains (square roots and divisions of ~20 dependent instructions each) interleave
-// and hide each other's latency.  L, R: [NF][5]; n: [NF][2]; H: [NF][5].  Same arithmetic per face
-// as ausm_flux.
-template <int NF>
-__device__ __forceinline__ void ausm_flux_n(double Rs, double gR, double cp, double Minf2, const Consts& K,
-                                            const double (*L)[5], const double (*R)[5], const double (*n)[2],
-                                            double (*H)[5], bool* ok) {
-  double aL[NF], aR[NF], pL[NF], pR[NF], unL[NF], unR[NF], HtL[NF], HtR[NF], a12[NF], ia[NF], ML[NF], MR[NF],
-      Mb2[NF], Mo[NF], fa[NF], M12[NF], mdot[NF], p12[NF];
-#pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    ok[f] = (L[f][0] > 0.0) & (R[f][0] > 0.0) & (L[f][4] > 0.0) & (R[f][4] > 0.0);
-    aL[f] = gR * L[f][4];
-    aR[f] = gR * R[f][4];
-  }
-#pragma unroll
-  for (int f = 0; f < NF; ++f) aL[f] = sqrt(aL[f]);
-#pragma unroll
-  for (int f = 0; f < NF; ++f) aR[f] = sqrt(aR[f]);
-#pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    pL[f] = L[f][0] * Rs * L[f][4];
-    pR[f] = R[f][0] * Rs * R[f][4];
-    unL[f] = L[f][1] * n[f][0] + L[f][2] * n[f][1];
-    unR[f] = R[f][1] * n[f][0] + R[f][2] * n[f][1];
-    HtL[f] = cp * L[f][4] + 0.5 * (L[f][1] * L[f][1] + L[f][2] * L[f][2] + L[f][3] * L[f][3]);
-    HtR[f] = cp * R[f][4] + 0.5 * (R[f][1] * R[f][1] + R[f][2] * R[f][2] + R[f][3] * R[f][3]);
-    a12[f] = 0.5 * (aL[f] + aR[f]);
-  }
-#pragma unroll
-  for (int f = 0; f < NF; ++f) ia[f] = 1.0 / a12[f];
-#pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    ML[f] = unL[f] * ia[f];
-    MR[f] = unR[f] * ia[f];
-    Mb2[f] = 0.5 * (unL[f] * unL[f] + unR[f] * unR[f]) * (ia[f] * ia[f]);
-    Mo[f] = fmin(1.0, fmax(Mb2[f], Minf2));
-  }
-#pragma unroll
-  for (int f = 0; f < NF; ++f) Mo[f] = sqrt(Mo[f]);
-  double P5p[NF], P5m[NF], den[NF], num[NF];
-#pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    fa[f] = Mo[f] * (2.0 - Mo[f]);
-    const double al16 = 3.0 * (5.0 * fa[f] * fa[f] - 4.0);
-    const double m2pL = 0.25 * (ML[f] + 1.0) * (ML[f] + 1.0), m2mL = -0.25 * (ML[f] - 1.0) * (ML[f] - 1.0);
-    const double m2pR = 0.25 * (MR[f] + 1.0) * (MR[f] + 1.0), m2mR = -0.25 * (MR[f] - 1.0) * (MR[f] - 1.0);
-    const bool supL = fabs(ML[f]) >= 1.0, supR = fabs(MR[f]) >= 1.0;
-    const double M4p = supL ? fmax(ML[f], 0.0) : m2pL * (1.0 - K.beta16 * m2mL);
-    const double M4m = supR ? fmin(MR[f], 0.0) : m2mR * (1.0 + K.beta16 * m2pR);
-    P5p[f] = supL ? (ML[f] > 0.0 ? 1.0 : 0.0) : m2pL * ((2.0 - ML[f]) - al16 * ML[f] * m2mL);
-    P5m[f] = supR ? (MR[f] < 0.0 ? 1.0 : 0.0) : m2mR * ((-2.0 - MR[f]) + al16 * MR[f] * m2pR);
-    M12[f] = M4p + M4m;
-    num[f] = -K.Kp * fmax(1.0 - K.sigma * Mb2[f], 0.0) * (pR[f] - pL[f]) * (ia[f] * ia[f]);
-    den[f] = fa[f] * 0.5 * (L[f][0] + R[f][0]);
-  }
-#pragma unroll
-  for (int f = 0; f < NF; ++f) num[f] = num[f] / den[f];
-#pragma unroll
-  for (int f = 0; f < NF; ++f) {
-    M12[f] = M12[f] + num[f];
-    const bool up = M12[f] > 0.0;
-    mdot[f] = a12[f] * M12[f] * (up ? L[f][0] : R[f][0]);
-    const double pu = -K.Ku * P5p[f] * P5m[f] * (L[f][0] + R[f][0]) * (fa[f] * a12[f]) * (unR[f] - unL[f]);
-    p12[f] = P5p[f] * pL[f] + P5m[f] * pR[f] + pu;
-    const bool upm = mdot[f] > 0.0;
-    H[f][0] = mdot[f];
-    H[f][1] = mdot[f] * (upm ? L[f][1] : R[f][1]) + p12[f] * n[f][0];
-    H[f][2] = mdot[f] * (upm ? L[f][2] : R[f][2]) + p12[f] * n[f][1];
-    H[f][3] = mdot[f] * (upm ? L[f][3] : R[f][3]);
-    H[f][4] = mdot[f] * (upm ? HtL[f] : HtR[f]);
-  }
-}
-
 // Two-fluid source (Eq. 4, Eq. 6; charge density rho_s q_s/m_s, S5; eps0 = 1/c^2)
 __device__ __forceinline__ void source_terms(const Consts& K, const double* P, double* S) {
   const double qi = K.qm[0] * P[8], qe = K.qm[1] * P[9];   // q_s n_s
