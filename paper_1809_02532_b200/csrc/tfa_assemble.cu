@@ -150,13 +150,13 @@ __device__ __forceinline__ void cons5(double cv, const double* Q, double* U) {
 
 // ------------------------------------------------------------------------------------------------
 // Non-flux part of the residual of one (cell, group): source (Alg. 1) and BDF2 term (Eq. 13).
-// grp 0 = field rows 0..7, 1 = ion rows, 2 = electron rows.  Writes S.rs (all rows) and S.s0.
+// grp 0 = field rows 0..7, 1 = ion rows, 2 = electron rows.  P, Pn, Pm: the cell's 18 values at the three time
+// levels.  Writes the group's rows of rs[18] and (species) its four entries of s0[8].
 // ------------------------------------------------------------------------------------------------
-template <int T, int NM>
-__device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts& K, int c, int grp, int64_t i,
-                                                const double* __restrict__ P,
-                                                const double* __restrict__ state_n,
-                                                const double* __restrict__ state_nm1, double vol, double inv2dt) {
+__device__ __forceinline__ void cell_group_rest(const int grp, const Consts& K, const double* __restrict__ P,
+                                                const double* __restrict__ Pn, const double* __restrict__ Pm,
+                                                double vol, double inv2dt, double* __restrict__ rs,
+                                                double* __restrict__ s0) {
   const bool do_src = K.mask & 2, do_time = K.mask & 4;
   const double ft = vol * inv2dt;
   if (grp == 0) {
@@ -172,8 +172,8 @@ __device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts&
     for (int r = 0; r < 8; ++r) {
       double a = 0.0;
       if (do_src) a -= Sf[r] * vol;
-      if (do_time) a += ft * (3.0 * P[r] - 4.0 * state_n[NEQ * i + r] + state_nm1[NEQ * i + r]);
-      S.rs[c][r] = a;
+      if (do_time) a += ft * (3.0 * P[r] - 4.0 * Pn[r] + Pm[r]);
+      rs[r] = a;
     }
   } else {
     const int s = grp - 1;
@@ -182,8 +182,8 @@ __device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts&
 #pragma unroll
     for (int r = 0; r < 5; ++r) {
       Q[r] = P[rows[r]];
-      Qn[r] = state_n[NEQ * i + rows[r]];
-      Qm[r] = state_nm1[NEQ * i + rows[r]];
+      Qn[r] = Pn[rows[r]];
+      Qm[r] = Pm[rows[r]];
     }
 #pragma unroll
     for (int r = 0; r < 3; ++r) { B[r] = P[r]; E[r] = P[3 + r]; }
@@ -198,12 +198,12 @@ __device__ __forceinline__ void cell_group_rest(AsmSmem<T, NM>& S, const Consts&
       double a = 0.0;
       if (do_src) a -= S5[r] * vol;
       if (do_time) a += ft * (3.0 * U[r] - 4.0 * Un[r] + Um[r]);
-      S.rs[c][rows[r]] = a;
+      rs[rows[r]] = a;
     }
-    S.s0[c][3 * s] = S5[1];
-    S.s0[c][3 * s + 1] = S5[2];
-    S.s0[c][3 * s + 2] = S5[3];
-    S.s0[c][6 + s] = S5[4];
+    s0[3 * s] = S5[1];
+    s0[3 * s + 1] = S5[2];
+    s0[3 * s + 2] = S5[3];
+    s0[6 + s] = S5[4];
   }
 }
 
@@ -279,8 +279,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     if (ROLE == 2 && tid >= C::NT - 3 * T) {
       const int q = tid - (C::NT - 3 * T);
       const int c = q / 3, grp = q - 3 * c;
-      if (c < ncell)
-        cell_group_rest<T, NM>(S, K, c, grp, cell0 + c, in.st[c], state_n, state_nm1, in.cg[c][7], inv2dt);
+      if (c < ncell) {
+        const double* Pn_ = state_n + NEQ * (cell0 + c);
+        const double* Pm_ = state_nm1 + NEQ * (cell0 + c);
+        cell_group_rest(grp, K, in.st[c], Pn_, Pm_, in.cg[c][7], inv2dt, S.rs[c], S.s0[c]);
+      }
     }
     // the next tile of this CTA: its packed neighbours (needed to request its inputs after face 0), and
     // the lines its non-TMA reads touch, towards L2
@@ -532,8 +535,7 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
   using C = AsmCfg<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   AsmSmem<T, NM>& S = *reinterpret_cast<AsmSmem<T, NM>*>(smem_raw);
-  // one instantiation serves both calls, so that the residual does not depend on whether the
-  // Jacobian is asked for (same instructions on the base lanes)
+  // (residual-only calls go to k_residual; the JAC = false path here is kept for completeness)
   const bool JAC = vals != nullptr;
   const int warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) {
@@ -561,6 +563,65 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     role_loop<T, NM, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
   else
     role_loop<T, NM, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
+}
+
+// ================================================================================================
+// Residual only (tfa_assemble with bsr_vals = NULL; the matrix-free operator's evaluations): no Jacobian, so
+// no staging, no perturbed lanes — thread = (cell, group), one warp per 32 cells and group (ions, electrons,
+// fields), the three faces in sequence, face states straight from the gradient kernel's array.
+// ================================================================================================
+constexpr int RES_CELLS = 32;
+template <int ROLE>
+__device__ __forceinline__ void residual_rows(const int64_t i, const Consts& K, const double* __restrict__ state,
+                                              const double* __restrict__ state_n, const double* __restrict__ state_nm1,
+                                              const double inv2dt, const double* __restrict__ fown,
+                                              const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
+                                              double* __restrict__ rhs, bool& nonphys) {
+  constexpr int NV = ROLE == 2 ? 8 : 5;
+  constexpr int SPC = ROLE == 2 ? 0 : ROLE;
+  const double* __restrict__ cg = cgeo + CGEO * i;
+  double acc[NV];
+#pragma unroll
+  for (int q = 0; q < NV; ++q) acc[q] = 0.0;
+  if (K.mask & 1) {
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {
+      const int32_t nf = nbrf[3 * i + k];
+      const double nx = cg[8 * k], ny = cg[8 * k + 1], len = cg[8 * k + 2];
+      const double* __restrict__ fo = fown + (3 * i + k) * NEQ;
+      const double* __restrict__ fx = nf < 0 ? fo : fown + (3 * (int64_t)(nf >> 2) + (nf & 3)) * NEQ;
+      double own[NV], oth[NV], H[NV];
+#pragma unroll
+      for (int q = 0; q < NV; ++q) {
+        own[q] = fo[vidx<ROLE>(q)];
+        oth[q] = fx[vidx<ROLE>(q)];
+      }
+      if (ROLE == 2) maxwell_flux(K, own, oth, nx, ny, H);
+      else nonphys |= !ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nx, ny, H);
+#pragma unroll
+      for (int q = 0; q < NV; ++q) acc[q] = __dadd_rn(acc[q], __dmul_rn(H[q], len));
+    }
+  }
+  double rs[NEQ], s0[8];
+  cell_group_rest(ROLE == 2 ? 0 : ROLE + 1, K, state + NEQ * i, state_n + NEQ * i, state_nm1 + NEQ * i, cg[7], inv2dt,
+                  rs, s0);
+#pragma unroll
+  for (int q = 0; q < NV; ++q) rhs[NEQ * i + vidx<ROLE>(q)] = -(acc[q] + rs[vidx<ROLE>(q)]);
+}
+
+__global__ void __launch_bounds__(3 * RES_CELLS) k_residual(
+    const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
+    const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
+    const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
+    double* __restrict__ rhs, int32_t* __restrict__ flags) {
+  const int role = threadIdx.x >> 5;   // warp 0 ions, 1 electrons, 2 fields
+  const int64_t i = blockIdx.x * (int64_t)RES_CELLS + (threadIdx.x & 31);
+  if (i >= nc) return;
+  bool nonphys = false;
+  if (role == 0) residual_rows<0>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, rhs, nonphys);
+  else if (role == 1) residual_rows<1>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, rhs, nonphys);
+  else residual_rows<2>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, rhs, nonphys);
+  if (nonphys) atomicAdd(flags, 1);
 }
 
 // ================================================================================================
@@ -595,6 +656,12 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
                     const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
                     int32_t* flags, cudaStream_t st) {
   if (m.nc == 0) return 0;
+  if (!vals) {
+    k_residual<<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, 1.0 / (2.0 * dt), fown,
+                                                             m.cgeo.p, m.nbrf.p, rhs, flags);
+    TFA_CUDA(cudaGetLastError());
+    return 0;
+  }
   return launch_nm<TFA_ASM_T, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
 }
 

@@ -254,7 +254,7 @@ def test_reordered_assembly(api, orc, W):
     assert er < RES_TOL and ej < JAC_TOL, (er, ej)
 
 
-def test_run_to_run_determinism_and_no_memset_needed(api, W):
+def test_run_to_run_determinism_and_no_memset_needed(api, orc, W):
     """S21: two assemblies of the same input are bit-identical, whatever the output held before."""
     import torch
     mi = small_meshes(W)["delaunay"]
@@ -270,9 +270,16 @@ def test_run_to_run_determinism_and_no_memset_needed(api, W):
     torch.cuda.synchronize()
     assert torch.equal(rhs1, rhs2) and torch.equal(vals1, vals2)
     assert torch.isfinite(vals1).all()
-    # residual-only evaluation gives the same rhs
+    # the residual-only call (its own kernel: no staging, no perturbed lanes) is deterministic as well and
+    # meets the residual tolerance against the oracle; the two kernels' residuals agree to rounding
     rhs3, none = ctx.assemble(g, P, jacobian=False)
-    assert none is None and torch.equal(rhs1, rhs3)
+    rhs4, _ = ctx.assemble(g, P, jacobian=False)
+    assert none is None and torch.equal(rhs3, rhs4)
+    o = orc.OracleMesh.from_input(mi)
+    ph_o = orc.physics_c()
+    rhs_o, sc_o, _ = orc.assemble(o, ph_o, orc.default_numerics(ph_o), W.gem_state(mi.centroids()), jacobian=False)
+    assert residual_error(rhs3.cpu().numpy(), rhs_o, sc_o) < RES_TOL
+    assert residual_error(rhs3.cpu().numpy(), rhs1.cpu().numpy(), sc_o) < 1e-14
     assert ctx.launches_per_assemble == 2
 
 
