@@ -276,10 +276,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     const double* __restrict__ sO = in.st[ca];
 
     // ---- the non-flux part of the residual, one thread per (cell, group) ----
-    if (ROLE == 2 && tid >= C::NT - 3 * T) {
-      const int q = tid - (C::NT - 3 * T);
-      const int c = q / 3, grp = q - 3 * c;
-      if (c < ncell) {
+    // (two paths, fields and species: one warp each, so that neither warp runs both)
+    if (ROLE == 2 && warp >= C::AW + C::MW - 2) {
+      const bool fields = warp == C::AW + C::MW - 1;
+      const int c = fields ? lane : lane >> 1, grp = fields ? 0 : 1 + (lane & 1);
+      if (lane < (fields ? T : 2 * T) && c < ncell) {
         const double* Pn_ = state_n + NEQ * (cell0 + c);
         const double* Pm_ = state_nm1 + NEQ * (cell0 + c);
         cell_group_rest(grp, K, in.st[c], Pn_, Pm_, in.cg[c][7], inv2dt, S.rs[c], S.s0[c]);
