@@ -32,6 +32,9 @@
 #ifndef TFA_ASM_BLKP
 #define TFA_ASM_BLKP 330   // doubles between staged blocks (324 = dense)
 #endif
+#ifndef TFA_ASM_WB
+#define TFA_ASM_WB 4   // warp issuing the end-of-tile bulk stores: the first Maxwell warp (slack at the top of the next tile)
+#endif
 #ifndef TFA_ASM_T
 #define TFA_ASM_T 10      // cells per tile (multiple of 5)
 #endif
@@ -244,6 +247,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
   constexpr int GL = NV + 1;              // lanes per group: base + NV perturbed
   constexpr int NG = ROLE == 2 ? 3 : 5;   // groups per warp
   constexpr int SPC = ROLE == 2 ? 0 : ROLE;
+  constexpr int WB = TFA_ASM_WB;   // warp issuing the end-of-tile bulk stores
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool do_flux = K.mask & 1, do_src = K.mask & 2, do_time = K.mask & 4;
   const int64_t ntiles = (nc + T - 1) / T;
@@ -316,7 +320,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     int4 b4 = make_int4(-1, -1, -1, -1);
     // bulk stores are issued by lane c (cell c) of warp 0 for the faces 0, 1 and of warp 1 for the diagonal block
     // and face 2, so that neither warp carries all 4 T requests of a tile (about 70 cycles each)
-    const bool issuer = JAC && warp < 2 && lane < ncell;
+    const bool issuer = JAC && (warp == 0 || warp == WB) && lane < ncell;
     if (issuer) b4 = *reinterpret_cast<const int4*>(blk4 + 4 * (cell0 + lane));
 
     // eps_k = delta * max(|P_cell,k|, ref_k), made representable (S7)
@@ -409,7 +413,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     if (EARLY2) bnd2 = face(2, d2);
     // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
     // them.  This barrier also publishes S.rs / S.s0 of the tile.
-    if (warp < 2 && lane < T) bulk_wait_read();
+    if ((warp == 0 || warp == WB) && lane < T) bulk_wait_read();
     cta_sync();   // A
     stage_mirror(0, d0, bnd0);
     stage_mirror(1, d1, bnd1);
@@ -519,13 +523,13 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     stage_mirror(0, d2, bnd2);
     fence_async_smem();
     cta_sync();   // B: every block of the tile is staged
-    if (issuer && warp == 1) {
+    if (issuer && warp == WB) {
       bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[lane][0], BLK * 8);
       if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[0][lane][0], BLK * 8);
       bulk_commit();
     }
   }
-  if (JAC && warp < 2 && lane < T) bulk_wait_all();
+  if (JAC && (warp == 0 || warp == WB) && lane < T) bulk_wait_all();
   if (nonphys) atomicAdd(flags, 1);
 }
 
