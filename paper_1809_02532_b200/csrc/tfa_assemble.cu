@@ -411,17 +411,17 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     const bool bnd1 = face(1, d1);
     bool bnd2 = false;
     if (EARLY2) bnd2 = face(2, d2);
+    if (loader && nN > 0) {
+      // request the next tile's inputs into the other stage (every read of that stage ended before the
+      // previous tile's closing barrier) — here, while this Maxwell warp would wait for the AUSM warps
+      stage_inputs<T>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo);
+    }
     // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
     // them.  This barrier also publishes S.rs / S.s0 of the tile.
     if ((warp == 0 || warp == WB) && lane < T) bulk_wait_read();
     cta_sync();   // A
     stage_mirror(0, d0, bnd0);
     stage_mirror(1, d1, bnd1);
-    if (loader && nN > 0) {
-      // request the next tile's inputs into the other stage: every read of that stage ended before
-      // the previous tile's closing barrier
-      stage_inputs<T>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo);
-    }
     fence_async_smem();
     cta_sync();   // 1
     // a7: each block leaves the SM as one 2592-byte bulk store
