@@ -32,9 +32,6 @@
 #ifndef TFA_ASM_BLKP
 #define TFA_ASM_BLKP 330   // doubles between staged blocks (324 = dense)
 #endif
-#ifndef TFA_ASM_WB
-#define TFA_ASM_WB 4   // warp issuing the end-of-tile bulk stores: the first Maxwell warp (slack at the top of the next tile)
-#endif
 #ifndef TFA_ASM_T
 #define TFA_ASM_T 10      // cells per tile (multiple of 5)
 #endif
@@ -247,7 +244,10 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
   constexpr int GL = NV + 1;              // lanes per group: base + NV perturbed
   constexpr int NG = ROLE == 2 ? 3 : 5;   // groups per warp
   constexpr int SPC = ROLE == 2 ? 0 : ROLE;
-  constexpr int WB = TFA_ASM_WB;   // warp issuing the end-of-tile bulk stores
+  // warp issuing the end-of-tile bulk stores: the first Maxwell warp (it has slack at the top of the next tile;
+  // measured against warp 1 and the last warp)
+  constexpr int WB = C::AW;
+  static_assert(T <= 32, "one issuing lane per tile cell");
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool do_flux = K.mask & 1, do_src = K.mask & 2, do_time = K.mask & 4;
   const int64_t ntiles = (nc + T - 1) / T;
