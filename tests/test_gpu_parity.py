@@ -388,3 +388,38 @@ def test_flux_sqrt_and_reciprocal_error_bound(api):
     es = np.abs(s - np.sqrt(x)) / np.spacing(np.sqrt(x))
     er = np.abs(r - 1.0 / x) / np.spacing(1.0 / x)
     assert es.max() <= 1.0 and er.max() <= 1.0, (es.max(), er.max())
+
+
+def test_gpu_invariants_free_stream_and_telescoping(api, W):
+    """north_star's first two oracle invariants, checked on the CUDA path itself (no oracle involved):
+    a uniform state gives a zero convective residual on any mesh, boundary cells included (free-stream
+    preservation, L85 consistency); on a periodic mesh the face fluxes telescope to a zero domain sum per
+    equation.  Each cell evaluates its faces in its own outward frame, so the two sides of a
+    face agree to rounding, not bit for bit: the sums are zero to rounding of the largest term."""
+    import torch
+    rng = np.random.default_rng(11)
+    ctx = api.Context()
+    nu = api.default_numerics(ctx.physics)
+    nu.term_mask = 1                                   # convective fluxes only
+    ctx.set_numerics(nu)
+    # free stream: one random physical state everywhere, on a mesh with boundaries and on a Delaunay mesh
+    for mi in (W.split_quad_mesh(9, 6, *W.GEM_DOMAIN, periodic_x=True, periodic_y=False),
+               W.delaunay_mesh(23, 17, *W.GEM_DOMAIN, jitter=0.3, seed=4, shuffle_cells=True)):
+        g = api.Mesh.from_input(mi)
+        P1 = random_state(rng, 1)
+        P = np.repeat(P1, g.n_cells, axis=0)
+        rhs, vals = ctx.assemble(g, dev(P))
+        ctx.check()
+        # scale of one face term: |F(U).n| Sigma <= c^2 |U| h
+        scale = 400.0 * np.abs(P1).max() * np.sqrt(g.get("volume").max())
+        assert float(rhs.abs().max()) <= 1e-12 * scale
+    # telescoping: noisy wave on the periodic mesh of config 1
+    w = W.make_workload("c1")
+    g = api.Mesh.from_input(w.mesh)
+    rhs, _ = ctx.assemble(g, dev(w.state), jacobian=False)
+    rhs2, _ = ctx.assemble(g, dev(w.state))
+    ctx.check()
+    for r in (rhs, rhs2):
+        tot = r.sum(dim=0).abs().cpu().numpy()
+        mag = r.abs().sum(dim=0).cpu().numpy()
+        assert (tot <= 1e-12 * np.maximum(mag, 1e-300) + 1e-13).all(), (tot, mag)
