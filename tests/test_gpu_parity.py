@@ -6,7 +6,7 @@ sum-of-|terms| scale; Jacobian 1e-8 of the row-maximum magnitude; connectivity b
 import numpy as np
 import pytest
 
-from conftest import random_state
+from conftest import random_state, rot18
 from helpers import (RES_TOL, JAC_TOL, residual_error, jacobian_error_rows, bsr_to_rows,
                      check_connectivity_against_brute)
 
@@ -423,3 +423,29 @@ def test_gpu_invariants_free_stream_and_telescoping(api, W):
         tot = r.sum(dim=0).abs().cpu().numpy()
         mag = r.abs().sum(dim=0).cpu().numpy()
         assert (tot <= 1e-12 * np.maximum(mag, 1e-300) + 1e-13).all(), (tot, mag)
+
+
+@pytest.mark.parametrize("theta,K", [(0.7, 1e9), (np.pi / 2, 1.0)])
+def test_gpu_rotation_covariance_of_the_wave(api, W, theta, K):
+    """north_star's fourth invariant (S19) on the CUDA path itself: rotate the mesh and the in-plane vector
+    components; the rhs rows rotate with them, the Jacobian blocks are conjugated (up to the forward-difference
+    truncation, the step sizes depending on the components).  Arbitrary angle with the limiter off, 90 degrees
+    with it on."""
+    mi = W.split_quad_mesh(6, 6)
+    ctx = api.Context()
+    nu = api.default_numerics(ctx.physics)
+    nu.venkat_K = K
+    ctx.set_numerics(nu)
+    P = W.wave_state(mi.centroids(), seed=3)
+    Q = rot18(theta)
+    g0, g1 = api.Mesh.from_input(mi), api.Mesh.from_input(mi.rotated(theta))
+    assert np.array_equal(g0.get("face_cells"), g1.get("face_cells"))
+    rhs0, v0 = ctx.assemble(g0, dev(P))
+    rhs1, v1 = ctx.assemble(g1, dev(P @ Q.T))
+    ctx.check()
+    rhs0, v0, rhs1, v1 = (t.cpu().numpy() for t in (rhs0, v0, rhs1, v1))
+    # scale of the residual's terms: time term Omega 3U/(2 dt) dominates at dt = 1e-3
+    scale = np.abs(v0).max() * np.abs(P).max()
+    assert np.abs(rhs1 - rhs0 @ Q.T).max() < 1e-11 * scale
+    J0rot = np.einsum("ab,nbc,dc->nad", Q, v0, Q)
+    assert np.abs(v1 - J0rot).max() < 2e-5 * np.abs(v0).max()
