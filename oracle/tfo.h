@@ -18,6 +18,9 @@
  *   residual      : free-stream preservation, periodic telescoping, rotation covariance
  *   Jacobian      : brute-force central differences of the oracle's own frozen residual;
  *                   Maxwell sub-block against the closed-form matrix; time term vs dU/dP by FD
+ *   against the paper (tests/test_exact_wave.py): the exact circularly polarised wave of Eq. 15-18 makes the
+ *                   spatial residual converge at second order; Newton on a BDF2 step of it contracts and lands
+ *                   on the exact solution; Harris-sheet total force balance and Ampere's law (GEM set-up)
  * Unpinned (no independent value available):
  *   |A_n| vs ref. [4] of the paper (S3), AUSM+-up constants / a_1/2 choice vs COOLFluiD (S4),
  *   LS weight exponent (S12), Venkatakrishnan eps^2=(K h)^3 (S13).
