@@ -151,7 +151,9 @@ def run_reference(args, wl):
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl_description(args.workload, wl), "sample_rows": min(args.cpu_rows, wl.mesh.n_cells)},
+            "config": {"workload": wl_description(args.workload, wl), "n_cells": wl.mesh.n_cells,
+                       "parallelism": "host cores (oracle)", "dt": wl.dt, "reorder": wl.reorder,
+                       "sample_rows": min(args.cpu_rows, wl.mesh.n_cells)},
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
