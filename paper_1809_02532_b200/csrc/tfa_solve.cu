@@ -43,32 +43,40 @@ __global__ void __launch_bounds__(SV_T) k_bsr_spmv(int64_t nc, const int32_t* __
 }
 
 // ------------------------------------------------------------------------------------------------
-// Inverse of each diagonal block: one warp per cell, Gauss-Jordan with partial pivoting on [A | I] in
-// shared memory (lane l < 18 owns row l).
+// Inverse of each diagonal block: one warp per cell, in-place Gauss-Jordan with partial pivoting in shared
+// memory.  Per pivot the 18 x 18 update is swept by all 32 lanes (11 elements each) instead of row by row;
+// the row interchanges are undone as column interchanges at the end.
 // ------------------------------------------------------------------------------------------------
-constexpr int BJ_WARPS = 4;
+constexpr int BJ_WARPS = 8;
+constexpr int BJ_LD = NEQ + 1;   // padded row length (bank spread)
 __global__ void __launch_bounds__(32 * BJ_WARPS) k_block_jacobi(int64_t nc, const int32_t* __restrict__ rowptr,
                                                                const int32_t* __restrict__ col,
                                                                const double* __restrict__ vals,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
-  __shared__ double M[BJ_WARPS][NEQ][2 * NEQ + 1];
+  __shared__ double M[BJ_WARPS][NEQ * BJ_LD];
+  __shared__ double colk[BJ_WARPS][NEQ];
+  __shared__ int piv[BJ_WARPS][NEQ];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
   if (i >= nc) return;
   int64_t bd = -1;
   for (int32_t b = rowptr[i]; b < rowptr[i + 1]; ++b)
     if (col[b] == (int32_t)i) bd = b;
-  double(*A)[2 * NEQ + 1] = M[w];
-  for (int e = lane; e < BLK; e += 32) {
-    const int r = e / NEQ, c = e - NEQ * r;
-    A[r][c] = vals[bd * BLK + e];
-    A[r][NEQ + c] = r == c ? 1.0 : 0.0;
+  double* A = M[w];
+  // element e = lane + 32 u of the block, u < 11: its row / column are the same for every pivot
+  int er[11], ec[11];
+#pragma unroll
+  for (int u = 0; u < 11; ++u) {
+    const int e = lane + 32 * u;
+    er[u] = e / NEQ;
+    ec[u] = e - NEQ * er[u];
+    if (e < BLK) A[er[u] * BJ_LD + ec[u]] = vals[bd * BLK + e];
   }
   __syncwarp();
   bool singular = false;
   for (int k = 0; k < NEQ; ++k) {
     // pivot: largest |A[r][k]| over r >= k (ties: smallest r)
-    double best = lane >= k && lane < NEQ ? fabs(A[lane][k]) : -1.0;
+    double best = lane >= k && lane < NEQ ? fabs(A[lane * BJ_LD + k]) : -1.0;
     int arg = lane;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -77,21 +85,25 @@ __global__ void __launch_bounds__(32 * BJ_WARPS) k_block_jacobi(int64_t nc, cons
       if (ob > best || (ob == best && oa < arg)) { best = ob; arg = oa; }
     }
     if (!(best > 0.0) || !isfinite(best)) { singular = true; break; }
-    if (arg != k) {   // swap rows k and arg
-      for (int c = lane; c < 2 * NEQ; c += 32) {
-        const double t = A[k][c];
-        A[k][c] = A[arg][c];
-        A[arg][c] = t;
-      }
-      __syncwarp();
+    if (lane == 0) piv[w][k] = arg;
+    if (arg != k && lane < NEQ) {   // swap rows k and arg
+      const double t = A[k * BJ_LD + lane];
+      A[k * BJ_LD + lane] = A[arg * BJ_LD + lane];
+      A[arg * BJ_LD + lane] = t;
     }
-    const double ip = 1.0 / A[k][k];
     __syncwarp();
-    for (int c = lane; c < 2 * NEQ; c += 32) A[k][c] *= ip;
+    const double ip = 1.0 / A[k * BJ_LD + k];
+    if (lane < NEQ) colk[w][lane] = A[lane * BJ_LD + k];   // column k before it is overwritten
     __syncwarp();
-    if (lane < NEQ && lane != k) {
-      const double f = A[lane][k];
-      for (int c = 0; c < 2 * NEQ; ++c) A[lane][c] = fma(-f, A[k][c], A[lane][c]);
+    if (lane < NEQ) A[k * BJ_LD + lane] = lane == k ? ip : A[k * BJ_LD + lane] * ip;   // pivot row of the inverse
+    __syncwarp();
+#pragma unroll
+    for (int u = 0; u < 11; ++u) {
+      const int r = er[u], c = ec[u];
+      if (lane + 32 * u < BLK && r != k) {
+        const double base = c == k ? 0.0 : A[r * BJ_LD + c];
+        A[r * BJ_LD + c] = fma(-colk[w][r], A[k * BJ_LD + c], base);
+      }
     }
     __syncwarp();
   }
@@ -100,7 +112,19 @@ __global__ void __launch_bounds__(32 * BJ_WARPS) k_block_jacobi(int64_t nc, cons
     for (int e = lane; e < BLK; e += 32) dinv[i * BLK + e] = 0.0;
     return;
   }
-  for (int e = lane; e < BLK; e += 32) dinv[i * BLK + e] = A[e / NEQ][NEQ + e % NEQ];
+  // inverse of the row-permuted matrix -> inverse of the matrix: column interchanges in reverse order
+  for (int k = NEQ - 1; k >= 0; --k) {
+    const int p = piv[w][k];
+    if (p != k && lane < NEQ) {
+      const double t = A[lane * BJ_LD + k];
+      A[lane * BJ_LD + k] = A[lane * BJ_LD + p];
+      A[lane * BJ_LD + p] = t;
+    }
+    __syncwarp();
+  }
+#pragma unroll
+  for (int u = 0; u < 11; ++u)
+    if (lane + 32 * u < BLK) dinv[i * BLK + lane + 32 * u] = A[er[u] * BJ_LD + ec[u]];
 }
 
 // ------------------------------------------------------------------------------------------------
