@@ -10,7 +10,7 @@ int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, 
                     double* grad, double* phi, cudaStream_t st);
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
                     const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
-                    int32_t* flags, cudaStream_t st);
+                    int32_t* flags, int* resident_ctas, cudaStream_t st);
 int launch_probe_dfma(int grid, int iters, double* sink, cudaStream_t st);
 int launch_probe_copy(const double* src, double* dst, int64_t n, cudaStream_t st);
 int launch_probe_math(const double* x, double* s, double* r, int64_t n, cudaStream_t st);
@@ -126,7 +126,8 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
   }
   TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
-  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, rhs, bsr_vals, ctx->flags.p, st));
+  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, rhs, bsr_vals, ctx->flags.p,
+                          &ctx->asm_resident_ctas, st));
   if (ev) {
     TFA_CUDA(cudaEventRecord(ev[2], st));
     ++ctx->timed;

@@ -637,21 +637,20 @@ namespace {
 template <int T, int NM>
 int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
               const double* state_nm1, double dt, const double* fown, double* rhs, double* vals, int32_t* flags,
-              cudaStream_t st) {
+              int* resident_ctas, cudaStream_t st) {
   using C = AsmCfg<T>;
-  static int ctas_per_sm = 0, n_sm = 0;
   const int smem = (int)sizeof(AsmSmem<T, NM>);
-  if (!ctas_per_sm) {
+  if (*resident_ctas <= 0) {   // once per context (= per device): CTAs that fit the GPU at once
     TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    int dev = 0, occ = 0;
+    int dev = 0, occ = 0, n_sm = 0;
     TFA_CUDA(cudaGetDevice(&dev));
     TFA_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, NM>, C::NT, smem));
     if (occ < 1) return set_error(TFA_ECUDA, "k_assemble does not fit on an SM");
-    ctas_per_sm = occ;
+    *resident_ctas = n_sm * occ;
   }
   const int64_t ntiles = (m.nc + T - 1) / T;
-  const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)n_sm * ctas_per_sm);
+  const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)*resident_ctas);
   const double inv2dt = 1.0 / (2.0 * dt);
   k_assemble<T, NM><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
                                                m.nbrf.p, m.blk4.p, rhs, vals, flags);
@@ -662,7 +661,7 @@ int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const dou
 
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
                     const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
-                    int32_t* flags, cudaStream_t st) {
+                    int32_t* flags, int* resident_ctas, cudaStream_t st) {
   if (m.nc == 0) return 0;
   if (!vals) {
     k_residual<<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, 1.0 / (2.0 * dt), fown,
@@ -670,7 +669,7 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
     TFA_CUDA(cudaGetLastError());
     return 0;
   }
-  return launch_nm<TFA_ASM_T, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, st);
+  return launch_nm<TFA_ASM_T, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, resident_ctas, st);
 }
 
 }  // namespace tfa

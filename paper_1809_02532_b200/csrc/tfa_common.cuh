@@ -105,6 +105,7 @@ struct tfa_ctx {
   // staging for tfa_assemble_host
   tfa::DevBuf<double> h_state[3], h_rhs, h_vals;
   int launches = 0;
+  int asm_resident_ctas = 0;      // persistent grid of k_assemble on this context's device (0 = not queried yet)
   // optional per-kernel timing (tfa_timing_enable): a ring of event triples
   static constexpr int kMaxTimed = 64;
   bool timing = false;
