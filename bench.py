@@ -343,10 +343,12 @@ def main():
         dinv = torch.empty((nc, 18, 18), dtype=torch.float64, device="cuda")
         bj_ms = timed(lambda: ctx.block_jacobi(mesh, vals, dinv), 3)
         bvec = rhs.reshape(-1).contiguous()
-        tt = time.perf_counter()
-        xs, its, rel = ctx.gmres(mesh, vals, bvec, dinv=dinv, restart=30, max_iters=300, rtol=1e-6)
-        torch.cuda.synchronize()
-        gm_s = time.perf_counter() - tt
+        for _ in range(2):   # the first solve allocates the Krylov workspace; the second is the timed one
+            torch.cuda.synchronize()
+            tt = time.perf_counter()
+            xs, its, rel = ctx.gmres(mesh, vals, bvec, dinv=dinv, restart=30, max_iters=300, rtol=1e-6)
+            torch.cuda.synchronize()
+            gm_s = time.perf_counter() - tt
         ctx.check()
         jv = torch.empty_like(xv)
         jvp_ms = timed(lambda: ctx.jvp(mesh, P, xv, Pn, Pnm1, wl.dt, eps=1e-7, out=jv), 5)

@@ -155,7 +155,7 @@ int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, dou
 int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream);
 /* Solve A x = b by right-preconditioned GMRES(restart): A M^-1 u = b, x = x0 + M^-1 u, M^-1 = dinv (block
  * diagonal; NULL = no preconditioner).  x holds the initial guess on entry and the solution on return.
- * Orthogonalisation: classical Gram-Schmidt applied twice; the small Hessenberg problem is solved on the host
+ * Orthogonalisation: classical Gram-Schmidt, repeated once when it cancelled more than a factor sqrt(2); the small Hessenberg problem is solved on the host
  * with Givens rotations (each iteration synchronises the stream).  Stops when the true residual norm
  * ||b - A x|| <= rtol * ||b|| (checked at every restart; the recurrence's estimate ends a cycle) or after
  * max_iters iterations.  info[0] = iterations done, info[1] = ||b - A x|| / ||b|| on return.

@@ -161,12 +161,15 @@ __global__ void __launch_bounds__(RED_T) k_dots(int64_t n, int k, const double* 
     }
   }
 }
-__global__ void k_dots_final(int k, int nblocks, const double* __restrict__ part, double* __restrict__ out) {
-  const int j = threadIdx.x;
-  if (j >= k) return;
+// one warp per dot product: lane l adds the partial sums l, l + 32, ... in order, then a fixed shuffle tree
+__global__ void __launch_bounds__(32) k_dots_final(int nblocks, const double* __restrict__ part,
+                                                   double* __restrict__ out) {
+  const int j = blockIdx.x;
   double s = 0.0;
-  for (int b = 0; b < nblocks; ++b) s += part[(int64_t)b * MAXK + j];
-  out[j] = s;
+  for (int b = threadIdx.x; b < nblocks; b += 32) s += part[(int64_t)b * MAXK + j];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (threadIdx.x == 0) out[j] = s;
 }
 // w -= sum_j h[j] V_j
 __global__ void __launch_bounds__(RED_T) k_sub_combination(int64_t n, int k, const double* __restrict__ V, int64_t ld,
@@ -212,7 +215,7 @@ struct Gm {
   // host[j] = V_j . w for j < k (synchronises)
   int dots(int k, const double* V, int64_t ld, const double* w) {
     k_dots<<<RED_B, RED_T, 0, st>>>(n, k, V, ld, w, part);
-    k_dots_final<<<1, MAXK, 0, st>>>(k, RED_B, part, out);
+    k_dots_final<<<k, 32, 0, st>>>(RED_B, part, out);
     TFA_CUDA(cudaMemcpyAsync(host, out, sizeof(double) * k, cudaMemcpyDeviceToHost, st));
     TFA_CUDA(cudaStreamSynchronize(st));
     return 0;
@@ -263,18 +266,23 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
     for (; k < mk && iters < max_iters; ++k, ++iters) {
       G.precond(V + (int64_t)k * n, z);
       TFA_TRY(G.spmv(z, w));
-      // classical Gram-Schmidt, applied twice
+      // classical Gram-Schmidt (all projections from one pass over the basis), repeated when it cancelled
+      // more than a factor sqrt(2) of the vector (the Daniel-Gragg-Kaufman-Stewart test): "twice is enough"
       double* h = &H[(size_t)k * (mk + 1)];
       for (int j = 0; j <= k + 1; ++j) h[j] = 0.0;
+      TFA_TRY(G.dots(1, w, n, w));
+      double before = std::sqrt(G.host[0]), hk1 = 0.0;
       for (int pass = 0; pass < 2; ++pass) {
         TFA_TRY(G.dots(k + 1, V, n, w));
         for (int j = 0; j <= k; ++j) h[j] += G.host[j];
         TFA_CUDA(cudaMemcpyAsync(G.out, G.host, sizeof(double) * (k + 1), cudaMemcpyHostToDevice, st));
         k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, G.out, w);
         TFA_CUDA(cudaStreamSynchronize(st));   // G.host is reused by the next reduction
+        TFA_TRY(G.dots(1, w, n, w));
+        hk1 = std::sqrt(G.host[0]);
+        if (hk1 > 0.7071067811865476 * before) break;
+        before = hk1;
       }
-      TFA_TRY(G.dots(1, w, n, w));
-      const double hk1 = std::sqrt(G.host[0]);
       h[k + 1] = hk1;
       if (hk1 > 0.0) k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / hk1, w, 0.0, nullptr, V + (int64_t)(k + 1) * n);
       // Givens rotations on column k of the Hessenberg matrix
