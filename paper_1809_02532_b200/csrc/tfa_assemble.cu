@@ -243,7 +243,9 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
   constexpr int NV = ROLE == 2 ? 8 : 5;   // variables (= rows) of the role's group
   constexpr int GL = NV + 1;              // lanes per group: base + NV perturbed
   constexpr int NG = ROLE == 2 ? 3 : 5;   // groups per warp
-  constexpr int SPC = ROLE == 2 ? 0 : ROLE;
+  // AUSM lanes: one code path for both species (halves the kernel's hot code), the species at run time
+  const int SPC = ROLE == 2 ? 0 : ((threadIdx.x >> 5) & 1);
+  auto vx = [&](const int q) { return ROLE == 2 ? q : (q == 0 ? 8 + SPC : (q == 4 ? 16 + SPC : 9 + 3 * SPC + q)); };
   // warp issuing the end-of-tile bulk stores: the first Maxwell warp (it has slack at the top of the next tile;
   // measured against warp 1 and the last warp)
   constexpr int WB = C::AW;
@@ -259,7 +261,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
   const int base_lane = GL * g;
   const bool pert = p != 0;
   const int pj = p - 1;   // perturbed variable of the group; -1 on the base lane
-  const int v = ROLE == 2 ? max(pj, 0) : (pj <= 0 ? 8 + ROLE : (pj == 4 ? 16 + ROLE : 9 + 3 * ROLE + pj));
+  const int v = ROLE == 2 ? max(pj, 0) : (pj <= 0 ? 8 + SPC : (pj == 4 ? 16 + SPC : 9 + 3 * SPC + pj));
   const bool run = do_flux && (JAC || !pert);
   const double pm = pert ? 1.0 : 0.0;
   bool nonphys = false;
@@ -366,8 +368,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
         } else {
 #pragma unroll
           for (int q = 0; q < NV; ++q) {
-            own[q] = fo[vidx<ROLE>(q)] + me[q];
-            oth[q] = fx[vidx<ROLE>(q)];
+            own[q] = fo[vx(q)] + me[q];
+            oth[q] = fx[vx(q)];
           }
         }
         if (any_bnd) {
@@ -400,7 +402,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     auto stage_mirror = [&](const int buf, const double* __restrict__ d, const bool bnd) {
       if (JAC && pert && act && !bnd) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) S.mir[buf][cl][vidx<ROLE>(q) * NEQ + v] = -d[q];
+        for (int q = 0; q < NV; ++q) S.mir[buf][cl][vx(q) * NEQ + v] = -d[q];
       }
     };
     static_assert(NM == 2, "the barrier sequence below is written for two mirror buffers");
@@ -437,7 +439,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     // ---- residual, source Jacobian (L245-253), BDF2 diagonal (Eq. 13), diagonal block ----
     if (act && !pert) {
 #pragma unroll
-      for (int q = 0; q < NV; ++q) rhs[NEQ * i + vidx<ROLE>(q)] = -(acc[q] + S.rs[cl][vidx<ROLE>(q)]);
+      for (int q = 0; q < NV; ++q) rhs[NEQ * i + vx(q)] = -(acc[q] + S.rs[cl][vx(q)]);
     }
     if (JAC) {
       if (act && pert) {
@@ -475,7 +477,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
           double Q[5], Qp[5], E[3], B[3];
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            Q[q] = sO[vidx<ROLE>(q)];
+            Q[q] = sO[vx(q)];
             Qp[q] = q == pj ? tv : Q[q];
           }
 #pragma unroll
@@ -508,7 +510,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
             acc[4] -= (S1[3] - S.s0[cl][6 + SPC]) * fs;
           }
 #pragma unroll
-          for (int q = 0; q < 5; ++q) S.diag[cl][vidx<ROLE>(q) * NEQ + v] = acc[q];
+          for (int q = 0; q < 5; ++q) S.diag[cl][vx(q) * NEQ + v] = acc[q];
           // S_E = -c^2 sum_s q_s n_s u_s and S_Phi = c^2 sum_s q_s n_s: only this species' term moves
 #pragma unroll
           for (int r = 0; r < 3; ++r)
@@ -567,8 +569,6 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
   __syncthreads();   // the prologue's neighbour table (plain stores) is visible
   if (warp >= C::AW)
     role_loop<T, NM, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
-  else if (warp & 1)
-    role_loop<T, NM, 1>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
   else
     role_loop<T, NM, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
 }
