@@ -123,6 +123,11 @@ __device__ __forceinline__ double nrcp(double d) {
   return fma(y, e, y);
 }
 
+// max / min as one compare and one select (fmax / fmin cost several instructions for their NaN rules; a NaN
+// here can only come from a non-physical state, which is reported separately)
+__device__ __forceinline__ double sel_max(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double sel_min(double a, double b) { return a < b ? a : b; }
+
 // Multi-fluid AUSM+-up for one species (Eq. 10; Liou's scheme = ref. [30]; S4).
 // L, R = (rho, u, v, w, T).  Returns true if the states are physical.
 // Rs, gR, cp, Minf2: the species' constants (K.Rs[s], ...), passed in registers (warp uniform).
@@ -139,19 +144,19 @@ __device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, doubl
   const double ia = TFA_RCP(a12);
   const double ML = unL * ia, MR = unR * ia;
   const double Mb2 = 0.5 * (unL * unL + unR * unR) * (ia * ia);
-  const double Mo = TFA_SQRT(fmin(1.0, fmax(Mb2, Minf2)));
+  const double Mo = TFA_SQRT(sel_min(1.0, sel_max(Mb2, Minf2)));
   const double fa = Mo * (2.0 - Mo);
   const double al16 = 3.0 * (5.0 * fa * fa - 4.0);             // 16 alpha, alpha = 3/16 (-4 + 5 fa^2)
   // split Mach numbers and pressures; for |M| >= 1:  M4+ = max(M,0), P5+ = (M > 0), etc.
   const double m2pL = 0.25 * (ML + 1.0) * (ML + 1.0), m2mL = -0.25 * (ML - 1.0) * (ML - 1.0);
   const double m2pR = 0.25 * (MR + 1.0) * (MR + 1.0), m2mR = -0.25 * (MR - 1.0) * (MR - 1.0);
   const bool supL = fabs(ML) >= 1.0, supR = fabs(MR) >= 1.0;
-  const double M4p = supL ? fmax(ML, 0.0) : m2pL * (1.0 - K.beta16 * m2mL);
-  const double M4m = supR ? fmin(MR, 0.0) : m2mR * (1.0 + K.beta16 * m2pR);
+  const double M4p = supL ? sel_max(ML, 0.0) : m2pL * (1.0 - K.beta16 * m2mL);
+  const double M4m = supR ? sel_min(MR, 0.0) : m2mR * (1.0 + K.beta16 * m2pR);
   const double P5p = supL ? (ML > 0.0 ? 1.0 : 0.0) : m2pL * ((2.0 - ML) - al16 * ML * m2mL);
   const double P5m = supR ? (MR < 0.0 ? 1.0 : 0.0) : m2mR * ((-2.0 - MR) + al16 * MR * m2pR);
   const double rsum = rL + rR;
-  const double Mp = -K.Kp * fmax(1.0 - K.sigma * Mb2, 0.0) * (pR - pL) * (ia * ia) * TFA_RCP(fa * 0.5 * rsum);
+  const double Mp = -K.Kp * sel_max(1.0 - K.sigma * Mb2, 0.0) * (pR - pL) * (ia * ia) * TFA_RCP(fa * 0.5 * rsum);
   const double M12 = M4p + M4m + Mp;
   const bool up = M12 > 0.0;
   const double mdot = a12 * M12 * (up ? rL : rR);
