@@ -120,7 +120,8 @@ struct __align__(128) AsmSmem {
   double s0[T][8];       // Lorentz-force and Joule-heating rows of S(P_i): equations 10..17
 };
 
-// roles: 0 = ion AUSM lanes, 1 = electron AUSM lanes, 2 = Maxwell lanes.
+// roles: 0 = ion AUSM lanes, 1 = electron AUSM lanes, 2 = Maxwell lanes (k_residual; k_assemble runs both
+// species through the role-0 code with the species at run time, which keeps its hot code small).
 // index of the q-th variable of the role's group inside the 18-vector
 template <int ROLE>
 __device__ __forceinline__ constexpr int vidx(int q) {
