@@ -193,6 +193,30 @@ def gem_state(centroids: np.ndarray, mass_ratio: float = 25.0, lam: float = 0.5,
     return P
 
 
+def gem_double_state(centroids: np.ndarray, mass_ratio: float = 25.0, lam: float = 0.5,
+                     Lx: float = 25.6, Ly: float = 25.6, psi0: float = 0.1) -> np.ndarray:
+    """Double current sheet on the periodic square [-Lx/2, Lx/2] x [-Ly/2, Ly/2] ("a square, where
+    a double current sheet is simulated ... periodic boundary conditions in all sides"): two Harris sheets of
+    opposite current at y = -+Ly/4, each the set-up of gem_state, each seeded with an X point at x = 0."""
+    x, y = centroids[:, 0], centroids[:, 1]
+    n = centroids.shape[0]
+    P = np.zeros((n, NEQ), dtype=np.float64)
+    ya, yb = (y + 0.25 * Ly) / lam, (y - 0.25 * Ly) / lam
+    sa, sb = 1.0 / np.cosh(ya) ** 2, 1.0 / np.cosh(yb) ** 2
+    dens = sa + sb + 0.2
+    kx, ky = 2 * np.pi / Lx, 2 * np.pi / Ly
+    # psi = psi0 cos(kx x) sin(ky y) (+-1 on the two sheets); Bx = Bx0 - dpsi/dy, By = dpsi/dx
+    P[:, IB + 0] = np.tanh(ya) - np.tanh(yb) - 1.0 - psi0 * ky * np.cos(kx * x) * np.cos(ky * y)
+    P[:, IB + 1] = -psi0 * kx * np.sin(kx * x) * np.sin(ky * y)
+    P[:, IRHOI] = dens
+    P[:, IRHOE] = dens / mass_ratio
+    P[:, ITI] = 5.0 / 12.0
+    P[:, ITE] = 1.0 / 12.0
+    Jz = -(sa - sb) / lam
+    P[:, IUE + 2] = Jz / (-1.0 * dens)
+    return P
+
+
 def perturb(state: np.ndarray, seed: int, amp: float) -> np.ndarray:
     """State perturbation between consecutive assemblies (BASELINE config 2)."""
     rng = np.random.default_rng(seed)
