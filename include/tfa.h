@@ -151,7 +151,8 @@ int tfa_probe_math(const double* x, double* sqrt_out, double* rcp_out, int64_t n
 /* y = A x for A = bsr_vals in the mesh's BSR pattern. */
 int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, double* y, void* stream);
 /* dinv [n_cells][18][18] = inverses of the diagonal blocks (Gauss-Jordan with partial pivoting, one warp per
- * block).  A singular block (pivot 0 or not finite) gets a zero inverse and is reported by tfa_check as TFA_ESINGULAR. */
+ * block; the pivot is the largest remaining entry of the column up to 2^-20 relative).  A singular block (pivot 0,
+ * subnormal or not finite) gets a zero inverse and is reported by tfa_check as TFA_ESINGULAR. */
 int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream);
 /* Solve A x = b by right-preconditioned GMRES(restart): A M^-1 u = b, x = x0 + M^-1 u, M^-1 = dinv (block
  * diagonal; NULL = no preconditioner).  x holds the initial guess on entry and the solution on return.

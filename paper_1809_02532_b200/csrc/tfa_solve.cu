@@ -43,88 +43,89 @@ __global__ void __launch_bounds__(SV_T) k_bsr_spmv(int64_t nc, const int32_t* __
 }
 
 // ------------------------------------------------------------------------------------------------
-// Inverse of each diagonal block: one warp per cell, in-place Gauss-Jordan with partial pivoting in shared
-// memory.  Per pivot the 18 x 18 update is swept by all 32 lanes (11 elements each) instead of row by row;
-// the row interchanges are undone as column interchanges at the end.
+// Inverse of each diagonal block: one warp per cell, Gauss-Jordan with partial pivoting.  Lane r keeps row r in
+// registers; rows are never moved (the pivot of step k is the largest |a[r][k]| among the rows not yet used,
+// p_k); the pivot row goes through a double-buffered 18-double row of shared memory, one __syncwarp per step.  With P the permutation (PA)[k] = A[p_k], the in-place result S = (PA)^-1 sits as row k in lane p_k and
+// A^-1[k][p_c] = S[k][c]; it is put in order in shared memory and written out coalesced.
+// (First version: the block in shared memory, every lane sweeping 11 elements per step; 3 loads and a store
+// per element made it shared-memory-bandwidth bound, 9.8 ms at 1M cells.)
 // ------------------------------------------------------------------------------------------------
 constexpr int BJ_WARPS = 8;
-constexpr int BJ_LD = NEQ + 1;   // padded row length (bank spread)
-__global__ void __launch_bounds__(32 * BJ_WARPS) k_block_jacobi(int64_t nc, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ rowptr,
                                                                const int32_t* __restrict__ col,
                                                                const double* __restrict__ vals,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
-  __shared__ double M[BJ_WARPS][NEQ * BJ_LD];
-  __shared__ double colk[BJ_WARPS][NEQ];
-  __shared__ int piv[BJ_WARPS][NEQ];
+  __shared__ __align__(16) double rowbuf[BJ_WARPS][2][NEQ];
+  __shared__ __align__(16) double outb[BJ_WARPS][BLK];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
   if (i >= nc) return;
   int64_t bd = -1;
   for (int32_t b = rowptr[i]; b < rowptr[i + 1]; ++b)
     if (col[b] == (int32_t)i) bd = b;
-  double* A = M[w];
-  // element e = lane + 32 u of the block, u < 11: its row / column are the same for every pivot
-  int er[11], ec[11];
+  const bool has = lane < NEQ;
+  double a[NEQ];
 #pragma unroll
-  for (int u = 0; u < 11; ++u) {
-    const int e = lane + 32 * u;
-    er[u] = e / NEQ;
-    ec[u] = e - NEQ * er[u];
-    if (e < BLK) A[er[u] * BJ_LD + ec[u]] = vals[bd * BLK + e];
+  for (int c = 0; c < NEQ; ++c) a[c] = 0.0;
+  if (has) {
+    const double2* __restrict__ src = reinterpret_cast<const double2*>(vals + bd * BLK + lane * NEQ);
+#pragma unroll
+    for (int c = 0; c < NEQ; c += 2) {
+      const double2 t = src[c / 2];
+      a[c] = t.x;
+      a[c + 1] = t.y;
+    }
   }
-  __syncwarp();
-  bool singular = false;
+  bool used = !has, singular = false;
+  int myk = 0;
+  int pk[NEQ];
+#pragma unroll
+  for (int k = 0; k < NEQ; ++k) pk[k] = 0;
+#pragma unroll
   for (int k = 0; k < NEQ; ++k) {
-    // pivot: largest |A[r][k]| over r >= k (ties: smallest r)
-    double best = lane >= k && lane < NEQ ? fabs(A[lane * BJ_LD + k]) : -1.0;
-    int arg = lane;
+    // pivot: the largest |a[r][k]| over the rows not used yet, compared on the high word (sign, exponent, 20
+    // mantissa bits: any entry within 2^-20 of the largest serves partial pivoting equally well) with one warp
+    // reduction; ties go to the smallest r.  NaN / Inf sort above every finite number and end the inversion.
+    const unsigned key = used ? 0u : (unsigned)(__double2hiint(a[k]) & 0x7fffffff);
+    const unsigned mx = __reduce_max_sync(0xffffffffu, key);
+    if (mx == 0u || mx >= 0x7ff00000u) singular = true;   // warp-uniform: zero / subnormal / not finite
+    if (!singular) {
+      const int arg = __ffs(__ballot_sync(0xffffffffu, key == mx)) - 1;
+      pk[k] = arg;
+      double2* __restrict__ rb = reinterpret_cast<double2*>(rowbuf[w][k & 1]);
+      const bool mine = lane == arg;
+      if (mine) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      const double ob = __shfl_xor_sync(0xffffffffu, best, o);
-      const int oa = __shfl_xor_sync(0xffffffffu, arg, o);
-      if (ob > best || (ob == best && oa < arg)) { best = ob; arg = oa; }
-    }
-    if (!(best > 0.0) || !isfinite(best)) { singular = true; break; }
-    if (lane == 0) piv[w][k] = arg;
-    if (arg != k && lane < NEQ) {   // swap rows k and arg
-      const double t = A[k * BJ_LD + lane];
-      A[k * BJ_LD + lane] = A[arg * BJ_LD + lane];
-      A[arg * BJ_LD + lane] = t;
-    }
-    __syncwarp();
-    const double ip = 1.0 / A[k * BJ_LD + k];
-    if (lane < NEQ) colk[w][lane] = A[lane * BJ_LD + k];   // column k before it is overwritten
-    __syncwarp();
-    if (lane < NEQ) A[k * BJ_LD + lane] = lane == k ? ip : A[k * BJ_LD + lane] * ip;   // pivot row of the inverse
-    __syncwarp();
+        for (int c = 0; c < NEQ; c += 2) rb[c / 2] = make_double2(a[c], a[c + 1]);
+        used = true;
+        myk = k;
+      }
+      __syncwarp();
+      // one code path for all rows: a[c] <- m t[c] + z with (m, z) = (1/t[k], 0) on the pivot row (its own row
+      // is t) and (-a[k]/t[k], a[c]) elsewhere; column k becomes the inverse's: 1/t[k] and -a[k]/t[k]
+      const double ip = 1.0 / rowbuf[w][k & 1][k];
+      const double m = mine ? ip : -(a[k] * ip);
 #pragma unroll
-    for (int u = 0; u < 11; ++u) {
-      const int r = er[u], c = ec[u];
-      if (lane + 32 * u < BLK && r != k) {
-        const double base = c == k ? 0.0 : A[r * BJ_LD + c];
-        A[r * BJ_LD + c] = fma(-colk[w][r], A[k * BJ_LD + c], base);
+      for (int c = 0; c < NEQ; c += 2) {
+        const double2 t = rb[c / 2];
+        a[c] = c == k ? m : fma(m, t.x, mine ? 0.0 : a[c]);
+        a[c + 1] = c + 1 == k ? m : fma(m, t.y, mine ? 0.0 : a[c + 1]);
       }
     }
-    __syncwarp();
   }
   if (singular) {
     if (lane == 0) atomicAdd(flags + 1, 1);
     for (int e = lane; e < BLK; e += 32) dinv[i * BLK + e] = 0.0;
     return;
   }
-  // inverse of the row-permuted matrix -> inverse of the matrix: column interchanges in reverse order
-  for (int k = NEQ - 1; k >= 0; --k) {
-    const int p = piv[w][k];
-    if (p != k && lane < NEQ) {
-      const double t = A[lane * BJ_LD + k];
-      A[lane * BJ_LD + k] = A[lane * BJ_LD + p];
-      A[lane * BJ_LD + p] = t;
-    }
-    __syncwarp();
-  }
+  if (has) {
 #pragma unroll
-  for (int u = 0; u < 11; ++u)
-    if (lane + 32 * u < BLK) dinv[i * BLK + lane + 32 * u] = A[er[u] * BJ_LD + ec[u]];
+    for (int c = 0; c < NEQ; ++c) outb[w][myk * NEQ + pk[c]] = a[c];
+  }
+  __syncwarp();
+  const double2* __restrict__ ob2 = reinterpret_cast<const double2*>(outb[w]);
+  double2* __restrict__ dst = reinterpret_cast<double2*>(dinv + i * BLK);
+  for (int e = lane; e < BLK / 2; e += 32) dst[e] = ob2[e];
 }
 
 // ------------------------------------------------------------------------------------------------

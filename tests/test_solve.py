@@ -117,6 +117,42 @@ def test_block_jacobi_parity_and_singular_block(system):
 
 
 @pytest.mark.gpu
+def test_block_jacobi_needs_its_pivoting(system):
+    """Diagonal blocks the assembled Jacobian never produces: dense random blocks with a zero diagonal,
+    signed permutation matrices, rows of very different scale.  Every pivot step moves (implicitly) a row, so
+    the permutation bookkeeping of the kernel is exercised; A A^-1 = I is the check, numpy's inverse the oracle."""
+    import torch
+    api, ctx, g, rhs, vals = system
+    rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
+    n = g.n_cells
+    diag = np.array([rp[i] + int(np.nonzero(col[rp[i]:rp[i + 1]] == i)[0][0]) for i in range(n)])
+    rng = np.random.default_rng(7)
+    blocks = rng.standard_normal((n, 18, 18))
+    blocks[:, np.arange(18), np.arange(18)] = 0.0                       # no usable diagonal pivot
+    for i in range(0, n, 3):                                            # signed, scaled permutations
+        blocks[i] = 0.0
+        blocks[i, np.arange(18), rng.permutation(18)] = rng.choice([-1.0, 1.0], 18) * 10.0 ** rng.integers(-6, 7, 18)
+    blocks[1::3] *= (10.0 ** rng.integers(-8, 9, (len(blocks[1::3]), 18)))[:, :, None]   # badly scaled rows
+    v = vals.clone()
+    v[torch.from_numpy(diag).cuda()] = torch.from_numpy(blocks).cuda()
+    dinv = ctx.block_jacobi(g, v).cpu().numpy()
+    ctx.check()
+    ref = np.linalg.inv(blocks)
+    prod = np.einsum("nij,njk->nik", blocks, dinv)
+    cond = np.linalg.cond(blocks, 1)
+    assert (np.abs(prod - np.eye(18)).max(axis=(1, 2)) <= 1e-13 * cond).all()
+    assert (np.abs(dinv - ref).max(axis=(1, 2)) <= 1e-13 * cond * np.abs(ref).max(axis=(1, 2))).all()
+    # the inverse of a scaled signed permutation has the transposed pattern, exactly
+    assert np.array_equal(dinv[0] != 0.0, (blocks[0] != 0.0).T)
+    # a NaN in a diagonal block is reported, not propagated silently
+    v[int(diag[2]), 4, 4] = float("nan")
+    ctx.block_jacobi(g, v)
+    with pytest.raises(api.TfaError) as e:
+        ctx.check()
+    assert e.value.code == -6
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("precond", [True, False])
 def test_gmres_parity(system, precond):
     import torch
