@@ -44,10 +44,12 @@ __global__ void k_lsq_coef(int64_t nc, const int32_t* __restrict__ st_ptr, const
 
 // Thread = (cell, pair of variables): 16-byte loads of the states; index and coefficient loads shared by the two
 // variables (measured against one variable per thread: 0.39 against 0.48 ms at 1M cells).  9 threads per cell,
-// 32 cells per CTA; 9 consecutive lanes read one neighbour state (144 contiguous bytes).
+// 32 cells per CTA; 9 consecutive lanes read one neighbour state (144 contiguous bytes).  Four CTAs per SM
+// (56 registers: 32-bit stencil indices, the cell's geometry read after the stencil walk): 0.364 against 0.384 ms
+// with three CTAs at 72 registers; five CTAs spill into the walk (0.57-0.60 ms).
 constexpr int GP_CELLS = 32;
 constexpr int GP_T = GP_CELLS * (NEQ / 2);   // 288 threads
-__global__ void __launch_bounds__(GP_T) k_gradient_limiter(
+__global__ void __launch_bounds__(GP_T, 4) k_gradient_limiter(
     int64_t nc, const double* __restrict__ state, const int32_t* __restrict__ st_ptr,
     const int32_t* __restrict__ st_idx, const double* __restrict__ coef, const double* __restrict__ cgeo,
     double venkK, double* __restrict__ fown, double* __restrict__ grad_out, double* __restrict__ phi_out) {
@@ -55,14 +57,6 @@ __global__ void __launch_bounds__(GP_T) k_gradient_limiter(
   const int64_t i = blockIdx.x * (int64_t)GP_CELLS + threadIdx.x / (NEQ / 2);
   if (i >= nc) return;
   const double2 Pi = *reinterpret_cast<const double2*>(state + NEQ * i + v);
-  const double* g = cgeo + CGEO * i;
-  double ox[3], oy[3];
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    ox[k] = g[8 * k + 3];
-    oy[k] = g[8 * k + 4];
-  }
-  const double sqrt_vol = g[15];
   double gx[2] = {0.0, 0.0}, gy[2] = {0.0, 0.0}, dmax[2] = {0.0, 0.0}, dmin[2] = {0.0, 0.0};
   const int32_t b = st_ptr[i], e = st_ptr[i + 1];
   const double2* __restrict__ coef2 = reinterpret_cast<const double2*>(coef);
@@ -80,14 +74,14 @@ __global__ void __launch_bounds__(GP_T) k_gradient_limiter(
   };
   auto batch = [&](auto nu) {
     constexpr int NU = decltype(nu)::value;
-    int64_t j[NU];
+    int32_t j[NU];
     double2 c[NU], Pj[NU];
 #pragma unroll
     for (int u = 0; u < NU; ++u) j[u] = st_idx[q + u];
 #pragma unroll
     for (int u = 0; u < NU; ++u) c[u] = coef2[q + u];
 #pragma unroll
-    for (int u = 0; u < NU; ++u) Pj[u] = *reinterpret_cast<const double2*>(state + NEQ * j[u] + v);
+    for (int u = 0; u < NU; ++u) Pj[u] = *reinterpret_cast<const double2*>(state + NEQ * (int64_t)j[u] + v);
 #pragma unroll
     for (int u = 0; u < NU; ++u) add(c[u], Pj[u]);
     q += NU;
@@ -95,6 +89,16 @@ __global__ void __launch_bounds__(GP_T) k_gradient_limiter(
   while (q + 8 <= e) batch(std::integral_constant<int, 8>{});
   if (q + 4 <= e) batch(std::integral_constant<int, 4>{});
   for (; q < e; ++q) add(coef2[q], *reinterpret_cast<const double2*>(state + NEQ * (int64_t)st_idx[q] + v));
+  // the cell's own geometry is read here, not before the walk (volatile keeps the compiler from hoisting the loads
+  // and holding 14 more registers across it)
+  const volatile double* g = cgeo + CGEO * i;
+  double ox[3], oy[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    ox[k] = g[8 * k + 3];
+    oy[k] = g[8 * k + 4];
+  }
+  const double sqrt_vol = g[15];
   const double Kh = venkK * sqrt_vol;
   const double eps2 = Kh * Kh * Kh;
   double phi[2], f[3][2];
