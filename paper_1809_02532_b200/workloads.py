@@ -143,6 +143,23 @@ class Physics:
     rusanov_alpha: float = 1.0
 
 
+def fan_mesh(n: int, radius: float = 1.0, seed: int = 0, jitter: float = 0.2) -> MeshInput:
+    """``n`` triangles around one hub node (a closed fan, all rim faces on the boundary): every cell meets every
+    other cell at the hub, so each vertex-neighbour stencil has n - 1 entries -- the long-stencil case of step a2.
+    Rim radii and angles are jittered so that the least-squares systems are generic."""
+    if n < 3:
+        raise ValueError("a closed fan needs at least 3 triangles")
+    rng = np.random.default_rng(seed)
+    ang = 2.0 * np.pi * (np.arange(n) + rng.uniform(-jitter, jitter, n)) / n
+    rad = radius * (1.0 + rng.uniform(-jitter, jitter, n))
+    node_xy = np.zeros((n + 1, 2))
+    node_xy[1:, 0] = rad * np.cos(ang)
+    node_xy[1:, 1] = rad * np.sin(ang)
+    k = np.arange(n)
+    cell_nodes = np.stack([np.zeros(n, dtype=np.int64), 1 + k, 1 + (k + 1) % n], axis=1).astype(np.int32)
+    return MeshInput(node_xy, cell_nodes, np.ascontiguousarray(node_xy[cell_nodes]), f"fan{n}")
+
+
 def wave_state(centroids: np.ndarray, seed: int | None, noise: float = 1e-3,
                mass_ratio: float = 25.0) -> np.ndarray:
     """Circularly polarised wave (BASELINE config 1-2; Eq. 16-17 for the shape)."""

@@ -151,6 +151,27 @@ def test_gradients_parity(api, orc, W, name, K, p):
     assert h > 0
 
 
+@pytest.mark.parametrize("n", [3, 4, 13, 40, 75])
+def test_long_stencils_fan(api, orc, W, n):
+    """Closed fans: every stencil has n - 1 entries (2, 3, 12, 39, 74): the stencil walk's batches of eight, its
+    batch of four and its tail entries in every combination; connectivity, gradients and assembly."""
+    mi = W.fan_mesh(n, seed=n)
+    g, o = api.Mesh.from_input(mi), orc.OracleMesh.from_input(mi)
+    for item in INT_ITEMS:
+        np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
+    assert g.n_stencil == n * (n - 1)
+    P = random_state(np.random.default_rng(n), n)
+    ctx = api.Context()
+    grad, phi = ctx.gradients(g, dev(P))
+    go, po = orc.gradients(o, orc.default_numerics(), P)
+    np.testing.assert_allclose(grad.cpu().numpy(), go, rtol=0, atol=1e-12 * np.abs(go).max())
+    np.testing.assert_allclose(phi.cpu().numpy(), po, rtol=0, atol=1e-11)
+    Pg = W.gem_state(mi.centroids()) + np.random.default_rng(1).uniform(-1e-3, 1e-3, (n, 18))
+    er, ej, _ = compare_assembly(api, orc, mi, Pg, W.perturb(Pg, 11, 1e-4), W.perturb(Pg, 12, 1e-4))
+    assert er < RES_TOL, er
+    assert ej < JAC_TOL, ej
+
+
 # ------------------------------------------------------------------------------------------
 # a3..a7: residual + Jacobian
 # ------------------------------------------------------------------------------------------

@@ -103,3 +103,34 @@ def test_mesh_errors(orc, W):
         orc.OracleMesh(mi.node_xy, bad, None)
     with pytest.raises(RuntimeError):      # periodic direction only 2 cells wide
         orc.OracleMesh.from_input(W.split_quad_mesh(2, 4))
+
+
+@pytest.mark.parametrize("n", [3, 4, 13, 40])
+def test_fan_stencil_is_everyone_else(orc, W, n):
+    """Closed fan of n triangles around a hub: the vertex-neighbour stencil of every cell is all other cells, the
+    face neighbours are the two adjacent ones (brute force on the definition)."""
+    mi = W.fan_mesh(n, seed=n)
+    m = orc.OracleMesh.from_input(mi)
+    assert (m.n_cells, m.n_faces, m.nnzb, m.n_stencil) == (n, 2 * n, 3 * n, n * (n - 1))
+    sp, si = m.get("stencil_ptr"), m.get("stencil_idx")
+    rp, col = m.get("bsr_rowptr"), m.get("bsr_col")
+    for c in range(n):
+        assert list(si[sp[c]:sp[c + 1]]) == [j for j in range(n) if j != c]
+        assert list(col[rp[c]:rp[c + 1]]) == sorted({(c - 1) % n, c, (c + 1) % n})
+    check_connectivity_against_brute(m.get, _sizes(m), mi.cell_nodes)
+    assert (m.get("volume") > 0).all()
+
+
+def test_fan_gradient_is_exact_for_linear_fields(orc, W):
+    """Least squares over a 39-entry stencil reproduces a linear field's gradient; the limiter leaves it alone when
+    K is huge (S12, S13)."""
+    mi = W.fan_mesh(40, seed=3)
+    m = orc.OracleMesh.from_input(mi)
+    cen = mi.centroids()
+    a = np.linspace(-1.0, 1.0, 18)
+    b = np.linspace(0.5, -0.7, 18)
+    P = 2.0 + a[None, :] * cen[:, :1] + b[None, :] * cen[:, 1:2]
+    grad, phi = orc.gradients(m, orc.default_numerics(venkat_K=1e9), P)
+    np.testing.assert_allclose(grad[:, :, 0], np.broadcast_to(a, (40, 18)), atol=1e-11)
+    np.testing.assert_allclose(grad[:, :, 1], np.broadcast_to(b, (40, 18)), atol=1e-11)
+    np.testing.assert_allclose(phi, 1.0, atol=1e-9)
