@@ -100,6 +100,48 @@ def test_limiter_closed_forms(orc, W):
     assert (phi > 0).all() and (phi <= 1).all()       # K > 0: phi in (0, 1]
 
 
+@pytest.mark.parametrize("K", [1.0, 0.3, 2.5])
+def test_limiter_finite_K_closed_form_on_a_linear_field(orc, W, K):
+    """Pins eps^2 = (K sqrt(Omega))^3 (L208, S13) at finite K.  On a linear field the
+    least-squares gradient is the exact slope g, so every quantity of Venkatakrishnan's function is known in
+    closed form: Delta2 = g . (x_f - x_i), Delta1 = (max or min over the cell and its vertex neighbours) - P_i,
+        phi_f = (Delta1^2 + eps^2 + 2 Delta1 Delta2) / (Delta1^2 + 2 Delta2^2 + Delta1 Delta2 + eps^2),
+    phi_i = min(1, min_f phi_f).  Omega comes from the shoelace formula here.  The slope is sized so that eps^2 and
+    Delta^2 are comparable: another exponent (h^2), h = Omega instead of sqrt(Omega), or K outside the cube
+    changes phi by far more than the tolerance (asserted below)."""
+    mi = meshes(W)["delaunay"]
+    m = orc.OracleMesh.from_input(mi)
+    cen = mi.centroids()
+    X = mi.cell_xy
+    area = 0.5 * ((X[:, 1, 0] - X[:, 0, 0]) * (X[:, 2, 1] - X[:, 0, 1]) - (X[:, 1, 1] - X[:, 0, 1]) * (X[:, 2, 0] - X[:, 0, 0]))
+    g = np.array([1.7, -1.1]) * K ** 1.5
+    lin = cen @ g + 0.3
+    grad, phi = orc.gradients(m, orc.default_numerics(venkat_K=K), np.tile(lin[:, None], (1, 18)))
+    sp, si = m.get("stencil_ptr"), m.get("stencil_idx")
+
+    def expected(i, eps2):
+        js = si[sp[i]:sp[i + 1]]
+        umax, umin = max(lin[js].max(), lin[i]), min(lin[js].min(), lin[i])
+        out = 1.0
+        for k in range(3):
+            d2 = (0.5 * (X[i, k] + X[i, (k + 1) % 3]) - cen[i]) @ g
+            if d2 == 0:
+                continue
+            d1 = (umax if d2 > 0 else umin) - lin[i]
+            out = min(out, (d1 * d1 + eps2 + 2 * d1 * d2) / (d1 * d1 + 2 * d2 * d2 + d1 * d2 + eps2))
+        return out
+
+    exp = np.array([expected(i, (K * np.sqrt(area[i])) ** 3) for i in range(m.n_cells)])
+    np.testing.assert_allclose(phi[:, 0], exp, rtol=0, atol=1e-11)
+    np.testing.assert_allclose(phi, np.tile(exp[:, None], (1, 18)), rtol=0, atol=1e-11)
+    assert (exp < 0.999).sum() >= 5                       # the limiter is active (hull cells: no neighbour beyond the face)
+    # the plausible mistakes are far outside the tolerance
+    for wrong in (lambda a: (K * np.sqrt(a)) ** 2, lambda a: (K * a) ** 3, lambda a: K * np.sqrt(a) ** 3 if K != 1.0
+                  else (K * np.sqrt(a)) ** 3 * 1.5, lambda a: 0.0):
+        bad = np.array([expected(i, wrong(area[i])) for i in range(m.n_cells)])
+        assert np.abs(bad - exp).max() > 1e-3
+
+
 # ------------------------------------------------------------------------------------------
 # residual
 # ------------------------------------------------------------------------------------------

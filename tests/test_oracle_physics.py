@@ -158,6 +158,80 @@ def test_ausm_contact_and_signs(orc, s):
     assert (H[1] * nx + H[2] * ny) > p
 
 
+@pytest.mark.parametrize("s", [0, 1])
+@pytest.mark.parametrize("Kp,sigma,minf", [(0.25, 1.0, 0.1), (0.4, 0.7, 0.3), (0.25, 1.0, 1.0)])
+def test_ausm_pressure_diffusion_magnitude_at_rest(orc, s, Kp, sigma, minf):
+    """Magnitude of M_p (Liou's AUSM+-up, ref. [30] via L99).  Both fluids at rest with
+    different pressure, density and temperature: M_L = M_R = 0, the split Mach numbers cancel
+    (M4+(0) + M4-(0) = 3/8 - 3/8), Mbar = 0 so M_o = M_inf, f_a = M_inf (2 - M_inf), and the whole mass flux is the
+    pressure-diffusion term:
+        mdot = a12 M_p rho_up,  M_p = -(K_p / f_a) (p_R - p_L) / (rho12 a12^2),
+    with a12 = (a_L + a_R)/2, rho12 = (rho_L + rho_R)/2 and rho_up the side the flow comes from.  p_u vanishes
+    (u_nR = u_nL), P5+-(0) = 1/2, so the interface pressure is the mean.  A wrong power of a12, a dropped 1/f_a,
+    rho_L for rho12 or a geometric mean for a12 all fail."""
+    ph = orc.physics_c()
+    nu = orc.default_numerics(ph, ausm_Kp=Kp, ausm_sigma=sigma, ausm_Minf=[minf, minf])
+    Rs = 1.0 if s == 0 else ph.mass_ratio
+    g = ph.gamma_gas
+    nx, ny = np.cos(1.1), np.sin(1.1)
+    for rhoL, TL, rhoR, TR in [(1.0, 0.5, 1.7, 0.9), (1.3, 0.8, 0.6, 0.35), (0.9, 0.4, 0.9, 0.45)]:
+        rhoL, rhoR = rhoL / (1.0 if s == 0 else 25.0), rhoR / (1.0 if s == 0 else 25.0)
+        L, R = np.array([rhoL, 0, 0, 0, TL]), np.array([rhoR, 0, 0, 0, TR])
+        pL, pR = rhoL * Rs * TL, rhoR * Rs * TR
+        a12 = 0.5 * (np.sqrt(g * Rs * TL) + np.sqrt(g * Rs * TR))
+        fa = minf * (2.0 - minf)
+        Mp = -(Kp / fa) * (pR - pL) / (0.5 * (rhoL + rhoR) * a12 ** 2)
+        up_rho, up_T = (rhoL, TL) if Mp > 0 else (rhoR, TR)
+        mdot = a12 * Mp * up_rho
+        p12 = 0.5 * (pL + pR)
+        Ht = g * Rs / (g - 1.0) * up_T                       # total enthalpy of a fluid at rest
+        expect = np.array([mdot, p12 * nx, p12 * ny, 0.0, mdot * Ht])
+        H = orc.flux_ausm(ph, nu, s, L, R, nx, ny)
+        np.testing.assert_allclose(H, expect, rtol=1e-13, atol=1e-15 * p12)
+        assert abs(mdot) > 1e-3 * up_rho * a12                # the term is not negligible in this test
+
+
+@pytest.mark.parametrize("s", [0, 1])
+@pytest.mark.parametrize("Ku,minf", [(0.75, 0.1), (0.5, 0.4)])
+def test_ausm_velocity_diffusion_magnitude_symmetric_streams(orc, s, Ku, minf):
+    """Magnitude of p_u.  Symmetric receding (or approaching) streams, u_nL = -u, u_nR = +u,
+    equal rho and T, M = u/a: M4+(-M) + M4-(M) = 0 and p_R = p_L, so mdot = 0 and the flux is (0, p12 n, 0) with
+        p12 = (P5+(-M) + P5-(M)) p - K_u P5+(-M) P5-(M) (rho_L + rho_R) (f_a a) (u_nR - u_nL),
+    Mbar^2 = M^2, M_o = sqrt(min(1, max(M^2, M_inf^2))), f_a = M_o (2 - M_o), alpha = 3/16 (-4 + 5 f_a^2).
+    P5 is taken in Liou's published monomial form P5+-(M) = 1/4 (M +- 1)^2 (2 -+ M) +- alpha M (M^2 - 1)^2 (the
+    oracle nests it differently); as a second route, the pressure-split part is measured from the oracle itself
+    with K_u = 0 and only the difference is compared with the closed form of p_u."""
+    ph = orc.physics_c()
+    Rs = 1.0 if s == 0 else ph.mass_ratio
+    g = ph.gamma_gas
+    nu = orc.default_numerics(ph, ausm_Ku=Ku, ausm_Minf=[minf, minf])
+    nu0 = orc.default_numerics(ph, ausm_Ku=0.0, ausm_Minf=[minf, minf])
+    nx, ny = np.cos(-0.4), np.sin(-0.4)
+    rho, T = 1.2 / (1.0 if s == 0 else 25.0), 0.6
+    a, p = np.sqrt(g * Rs * T), rho * Rs * T
+    for M in (0.05, 0.3, 0.7, -0.3, -0.7):                    # M > 0 receding, M < 0 approaching
+        u = M * a
+        L = np.array([rho, -u * nx, -u * ny, 0.3, T])
+        R = np.array([rho, +u * nx, +u * ny, -0.2, T])
+        Mo = np.sqrt(min(1.0, max(M * M, minf * minf)))
+        fa = Mo * (2.0 - Mo)
+        alpha = 3.0 / 16.0 * (-4.0 + 5.0 * fa * fa)
+        P5p = lambda m: 0.25 * (m + 1) ** 2 * (2 - m) + alpha * m * (m * m - 1) ** 2
+        P5m = lambda m: 0.25 * (m - 1) ** 2 * (2 + m) - alpha * m * (m * m - 1) ** 2
+        Pp, Pm = P5p(-M), P5m(M)
+        assert abs(Pp - Pm) < 1e-15                            # symmetry of the set-up
+        pu = -Ku * Pp * Pm * (2 * rho) * (fa * a) * (2 * u)
+        H = orc.flux_ausm(ph, nu, s, L, R, nx, ny)
+        H0 = orc.flux_ausm(ph, nu0, s, L, R, nx, ny)
+        assert abs(H[0]) < 1e-15 * rho * a and abs(H[3]) < 1e-15 * p and abs(H[4]) < 1e-14 * p * a
+        p12, p12_0 = H[1] * nx + H[2] * ny, H0[1] * nx + H0[2] * ny
+        np.testing.assert_allclose(p12, (Pp + Pm) * p + pu, rtol=1e-13)
+        # second route: P from the K_u = 0 evaluation, p_u from the difference
+        P_meas = p12_0 / (2 * p)
+        np.testing.assert_allclose(p12 - p12_0, -Ku * P_meas ** 2 * (2 * rho) * (fa * a) * (2 * u), rtol=1e-11)
+        assert abs(pu) > 1e-3 * p * abs(M)                     # the term matters here
+
+
 def test_ausm_split_functions(orc):
     """Liou's polynomials: beta = 1/8 puts an inflection of M4+ at M = 0; alpha = 3/16 makes P5+
     twice differentiable at M = 1; M4+ + M4- = M and P5+ + P5- = 1 for any alpha, beta;
