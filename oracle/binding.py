@@ -26,7 +26,9 @@ class Numerics(C.Structure):
 MESH_ITEMS = dict(face_cells=(0, np.int32), cell_faces=(1, np.int32), stencil_ptr=(2, np.int32),
                   stencil_idx=(3, np.int32), bsr_rowptr=(4, np.int32), bsr_col=(5, np.int32),
                   perm=(6, np.int32), volume=(7, np.float64), face_normal_len=(8, np.float64),
-                  centroid=(9, np.float64), face_nodes=(10, np.int32))
+                  centroid=(9, np.float64), face_nodes=(10, np.int32), bfaces=(12, np.int32),
+                  bc_tags=(13, np.int32))
+BC_TRANSMISSIVE, BC_GHOST, BC_WALL = 0, 1, 2
 
 
 def build(force: bool = False) -> str:
@@ -53,6 +55,11 @@ def lib():
         dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.c_void_p
         L.tfo_last_error.restype = C.c_char_p
         L.tfo_mesh_create.argtypes = [C.POINTER(vp), C.c_int64, vp, C.c_int64, vp, vp]
+        L.tfo_mesh_create_poly.argtypes = [C.POINTER(vp), C.c_int64, vp, C.c_int64, vp, vp, vp]
+        L.tfo_mesh_info.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
+        L.tfo_mesh_set_bc.argtypes = [vp, vp, vp]
+        L.tfo_wall_ghost.argtypes = [vp, C.c_double, C.c_double, vp]
+        L.tfo_wall_ghost.restype = None
         L.tfo_mesh_reorder.argtypes = [vp, C.c_int, vp]
         L.tfo_mesh_sizes.argtypes = [vp] + [C.POINTER(C.c_int64)] * 4
         L.tfo_mesh_get.argtypes = [vp, C.c_int, vp, C.c_int64]
@@ -123,23 +130,41 @@ def num_threads() -> int:
 
 
 class OracleMesh:
-    def __init__(self, node_xy, cell_nodes, cell_xy=None):
+    def __init__(self, node_xy, cell_nodes, cell_xy=None, cell_ptr=None):
+        """Triangles: cell_nodes [nc][3].  Mixed triangles / quadrilaterals: cell_ptr [nc+1] and flat cell_nodes,
+        cell_xy [cell_ptr[nc]][2]."""
         self._h = C.c_void_p()
         node_xy = _f64(node_xy)
         cell_nodes = np.ascontiguousarray(cell_nodes, dtype=np.int32)
         cxy = None if cell_xy is None else _f64(cell_xy)
-        _chk(lib().tfo_mesh_create(C.byref(self._h), node_xy.shape[0], _p(node_xy), cell_nodes.shape[0],
-                                   _p(cell_nodes), _p(cxy)))
+        if cell_ptr is None:
+            _chk(lib().tfo_mesh_create(C.byref(self._h), node_xy.shape[0], _p(node_xy), cell_nodes.shape[0],
+                                       _p(cell_nodes), _p(cxy)))
+        else:
+            cp = np.ascontiguousarray(cell_ptr, dtype=np.int32)
+            _chk(lib().tfo_mesh_create_poly(C.byref(self._h), node_xy.shape[0], _p(node_xy), cp.shape[0] - 1,
+                                            _p(cp), _p(cell_nodes), _p(cxy)))
         self._sizes()
 
     @classmethod
     def from_input(cls, mi) -> "OracleMesh":
-        return cls(mi.node_xy, mi.cell_nodes, mi.cell_xy)
+        return cls(mi.node_xy, mi.cell_nodes, mi.cell_xy, getattr(mi, "cell_ptr", None))
 
     def _sizes(self):
         v = [C.c_int64() for _ in range(4)]
         _chk(lib().tfo_mesh_sizes(self._h, *[C.byref(x) for x in v]))
         self.n_cells, self.n_faces, self.nnzb, self.n_stencil = [int(x.value) for x in v]
+        mf, nb = C.c_int32(), C.c_int64()
+        _chk(lib().tfo_mesh_info(self._h, C.byref(mf), C.byref(nb)))
+        self.max_faces, self.n_bfaces = int(mf.value), int(nb.value)
+
+    def set_bc(self, tags, ghost=None):
+        """tags [n_bfaces] in the order of get("bfaces"); ghost [n_bfaces][18] for the BC_GHOST faces."""
+        tags = np.ascontiguousarray(tags, dtype=np.int32)
+        assert tags.shape == (self.n_bfaces,)
+        gh = None if ghost is None else _f64(ghost)
+        assert gh is None or gh.shape == (self.n_bfaces, NEQ)
+        _chk(lib().tfo_mesh_set_bc(self._h, _p(tags), _p(gh)))
 
     def reorder(self, kind: str = "rcm", perm=None):
         k = {"none": 0, "rcm": 1, "user": 2}[kind]
@@ -149,14 +174,14 @@ class OracleMesh:
 
     def get(self, name: str) -> np.ndarray:
         which, dt = MESH_ITEMS[name]
-        n = dict(face_cells=2 * self.n_faces, face_nodes=2 * self.n_faces, cell_faces=3 * self.n_cells,
+        n = dict(face_cells=2 * self.n_faces, face_nodes=2 * self.n_faces, cell_faces=self.max_faces * self.n_cells,
                  stencil_ptr=self.n_cells + 1, stencil_idx=self.n_stencil, bsr_rowptr=self.n_cells + 1,
                  bsr_col=self.nnzb, perm=self.n_cells, volume=self.n_cells, face_normal_len=3 * self.n_faces,
-                 centroid=2 * self.n_cells)[name]
+                 centroid=2 * self.n_cells, bfaces=self.n_bfaces, bc_tags=self.n_bfaces)[name]
         out = np.empty(n, dtype=dt)
         _chk(lib().tfo_mesh_get(self._h, which, _p(out), out.nbytes))
-        shape = dict(face_cells=(-1, 2), face_nodes=(-1, 2), cell_faces=(-1, 3), face_normal_len=(-1, 3),
-                     centroid=(-1, 2)).get(name)
+        shape = dict(face_cells=(-1, 2), face_nodes=(-1, 2), cell_faces=(-1, self.max_faces),
+                     face_normal_len=(-1, 3), centroid=(-1, 2)).get(name)
         return out.reshape(shape) if shape else out
 
     def close(self):
@@ -181,7 +206,8 @@ def gradients(mesh: OracleMesh, nu: Numerics, state):
 
 def assemble(mesh: OracleMesh, ph: PhysicsC, nu: Numerics, state, state_n=None, state_nm1=None, dt=1e-3,
              rows=None, jacobian=True):
-    """Returns (rhs, scale, vals).  rows=None: vals[nnzb][18][18]; else compact vals[n_rows][4][18][18]."""
+    """Returns (rhs, scale, vals).  rows=None: vals[nnzb][18][18]; else compact, zero-padded
+    vals[n_rows][max_faces + 1][18][18]."""
     state = _f64(state)
     state_n = state if state_n is None else _f64(state_n)
     state_nm1 = state if state_nm1 is None else _f64(state_nm1)
@@ -192,7 +218,7 @@ def assemble(mesh: OracleMesh, ph: PhysicsC, nu: Numerics, state, state_n=None, 
     else:
         rr = np.ascontiguousarray(rows, dtype=np.int32)
         n = nr = rr.shape[0]
-        vals = np.empty((n, 4, NEQ, NEQ)) if jacobian else None
+        vals = np.empty((n, mesh.max_faces + 1, NEQ, NEQ)) if jacobian else None
     rhs = np.empty((n, NEQ))
     scale = np.empty((n, NEQ))
     _chk(lib().tfo_assemble(mesh._h, C.byref(ph), C.byref(nu), _p(state), _p(state_n), _p(state_nm1),
@@ -237,6 +263,13 @@ def phys_flux(ph, P, nx, ny):
     F = np.empty(NEQ)
     lib().tfo_phys_flux(C.byref(ph), _p(P), nx, ny, _p(F))
     return F
+
+
+def wall_ghost(P, nx, ny):
+    P = _f64(P)
+    G = np.empty(NEQ)
+    lib().tfo_wall_ghost(_p(P), float(nx), float(ny), _p(G))
+    return G
 
 
 def source(ph, P):

@@ -42,12 +42,14 @@ inline double qm_s(const tfo_physics& ph, int s) { return s == 0 ? 1.0 : -ph.mas
 
 struct tfo_mesh {
   int64_t nn = 0, nc = 0, nf = 0;
+  int maxf = 3;                      // largest number of faces of a cell (3 triangles only, 4 with quadrilaterals)
   std::vector<double> node_xy;       // [nn][2]
-  std::vector<int32_t> cell_nodes;   // [nc][3]
-  std::vector<double> cell_xy;       // [nc][3][2]
+  std::vector<int32_t> cptr;         // [nc+1]: corners (= local faces) of cell i are cptr[i] .. cptr[i+1]-1
+  std::vector<int32_t> cell_nodes;   // [cptr[nc]], counter-clockwise
+  std::vector<double> cell_xy;       // [cptr[nc]][2]
   std::vector<int32_t> face_nodes;   // [nf][2] (lo, hi)
   std::vector<int32_t> face_cells;   // [nf][2] (L, R or -1)
-  std::vector<int32_t> cell_faces;   // [nc][3]
+  std::vector<int32_t> cell_faces;   // [cptr[nc]]: face of local edge k = (corner k -> corner k+1)
   std::vector<int32_t> st_ptr, st_idx;
   std::vector<double> st_d;          // [nst][2] displacement centroid_j - centroid_i (S9)
   std::vector<int32_t> bsr_rowptr, bsr_col;
@@ -55,9 +57,15 @@ struct tfo_mesh {
   // geometry, per cell from its own corners
   std::vector<double> cen;           // [nc][2]
   std::vector<double> vol;           // [nc]
-  std::vector<double> fmid_off;      // [nc][3][2]  midpoint of local edge k minus centroid
-  std::vector<double> fnrm;          // [nc][3][2]  outward unit normal of local edge k
-  std::vector<double> flen;          // [nc][3]
+  std::vector<double> fmid_off;      // [cptr[nc]][2]  midpoint of local edge k minus centroid
+  std::vector<double> fnrm;          // [cptr[nc]][2]  outward unit normal of local edge k
+  std::vector<double> flen;          // [cptr[nc]]
+  // boundary conditions (L260: a separate loop over the boundary faces; S9, S24)
+  std::vector<int32_t> bfaces;       // boundary faces (R = -1) in ascending face id
+  std::vector<int32_t> bface_of;     // [nf] index into bfaces, -1 for interior faces
+  std::vector<int32_t> bc_tag;       // [nb] TFO_BC_*
+  std::vector<double> ghost;         // [nb][18] ghost states of the TFO_BC_GHOST faces (empty = none given)
+  int nv(int64_t i) const { return cptr[i + 1] - cptr[i]; }
 };
 
 namespace {
@@ -67,52 +75,87 @@ namespace {
 // ------------------------------------------------------------------------------------------
 int build(tfo_mesh& m) {
   const int64_t nc = m.nc;
+  const int64_t ncorn = nc ? m.cptr[nc] : 0;
+  m.maxf = 3;
   // geometry per cell
   m.cen.assign(2 * nc, 0.0);
   m.vol.assign(nc, 0.0);
-  m.fmid_off.assign(6 * nc, 0.0);
-  m.fnrm.assign(6 * nc, 0.0);
-  m.flen.assign(3 * nc, 0.0);
+  m.fmid_off.assign(2 * ncorn, 0.0);
+  m.fnrm.assign(2 * ncorn, 0.0);
+  m.flen.assign(ncorn, 0.0);
   for (int64_t i = 0; i < nc; ++i) {
-    const double* X = &m.cell_xy[6 * i];
-    double cx = (X[0] + X[2] + X[4]) / 3.0, cy = (X[1] + X[3] + X[5]) / 3.0;
-    double area = 0.5 * ((X[2] - X[0]) * (X[5] - X[1]) - (X[3] - X[1]) * (X[4] - X[0]));
-    if (!(area > 0.0)) return fail(-2, "cell " + std::to_string(i) + " is not counter-clockwise");
+    const int nv = m.nv(i);
+    const int64_t c0 = m.cptr[i];
+    if (nv < 3 || nv > TFO_MAXV) return fail(-2, "cell " + std::to_string(i) + " must have 3 or 4 corners");
+    m.maxf = std::max(m.maxf, nv);
+    const double* X = &m.cell_xy[2 * c0];
+    double cx, cy, area;
+    if (nv == 3) {
+      cx = (X[0] + X[2] + X[4]) / 3.0;
+      cy = (X[1] + X[3] + X[5]) / 3.0;
+      area = 0.5 * ((X[2] - X[0]) * (X[5] - X[1]) - (X[3] - X[1]) * (X[4] - X[0]));
+      if (!(area > 0.0)) return fail(-2, "cell " + std::to_string(i) + " is not counter-clockwise");
+    } else {
+      // polygon: shoelace area and area centroid, taken relative to corner 0 (no cancellation against the
+      // cell's position in the domain); every corner must turn left (convex, counter-clockwise)
+      double a2 = 0.0, sx = 0.0, sy = 0.0;
+      for (int k = 1; k + 1 < nv; ++k) {
+        const double ax = X[2 * k] - X[0], ay = X[2 * k + 1] - X[1];
+        const double bx = X[2 * k + 2] - X[0], by = X[2 * k + 3] - X[1];
+        const double cr = ax * by - ay * bx;   // twice the area of the triangle (corner 0, k, k+1)
+        a2 += cr;
+        sx += cr * (ax + bx);                  // times three times that triangle's centroid offset
+        sy += cr * (ay + by);
+      }
+      area = 0.5 * a2;
+      for (int k = 0; k < nv; ++k) {
+        const int k1 = (k + 1) % nv, k2 = (k + 2) % nv;
+        const double ux = X[2 * k1] - X[2 * k], uy = X[2 * k1 + 1] - X[2 * k + 1];
+        const double vx = X[2 * k2] - X[2 * k1], vy = X[2 * k2 + 1] - X[2 * k1 + 1];
+        if (!(ux * vy - uy * vx > 0.0))
+          return fail(-2, "cell " + std::to_string(i) + " is not a convex counter-clockwise polygon");
+      }
+      if (!(area > 0.0)) return fail(-2, "cell " + std::to_string(i) + " is not counter-clockwise");
+      cx = X[0] + sx / (3.0 * a2);
+      cy = X[1] + sy / (3.0 * a2);
+    }
     m.cen[2 * i] = cx;
     m.cen[2 * i + 1] = cy;
     m.vol[i] = area;
-    for (int k = 0; k < 3; ++k) {
-      int k1 = (k + 1) % 3;
+    for (int k = 0; k < nv; ++k) {
+      int k1 = (k + 1) % nv;
       double ax = X[2 * k], ay = X[2 * k + 1], bx = X[2 * k1], by = X[2 * k1 + 1];
       double dx = bx - ax, dy = by - ay;
       double len = std::sqrt(dx * dx + dy * dy);
-      m.flen[3 * i + k] = len;
-      m.fnrm[6 * i + 2 * k] = dy / len;        // outward for a CCW cell: (dy, -dx)/len
-      m.fnrm[6 * i + 2 * k + 1] = -dx / len;
-      m.fmid_off[6 * i + 2 * k] = 0.5 * (ax + bx) - cx;
-      m.fmid_off[6 * i + 2 * k + 1] = 0.5 * (ay + by) - cy;
+      m.flen[c0 + k] = len;
+      m.fnrm[2 * (c0 + k)] = dy / len;        // outward for a CCW cell: (dy, -dx)/len
+      m.fnrm[2 * (c0 + k) + 1] = -dx / len;
+      m.fmid_off[2 * (c0 + k)] = 0.5 * (ax + bx) - cx;
+      m.fmid_off[2 * (c0 + k) + 1] = 0.5 * (ay + by) - cy;
     }
-    const int32_t* cn = &m.cell_nodes[3 * i];
-    if (cn[0] == cn[1] || cn[1] == cn[2] || cn[0] == cn[2])
-      return fail(-2, "cell " + std::to_string(i) + " repeats a node (periodic direction too narrow)");
-    for (int k = 0; k < 3; ++k)
+    const int32_t* cn = &m.cell_nodes[c0];
+    for (int a = 0; a < nv; ++a)
+      for (int b = a + 1; b < nv; ++b)
+        if (cn[a] == cn[b])
+          return fail(-2, "cell " + std::to_string(i) + " repeats a node (periodic direction too narrow)");
+    for (int k = 0; k < nv; ++k)
       if (cn[k] < 0 || cn[k] >= m.nn) return fail(-2, "node id out of range");
   }
   // faces = unique node pairs, sorted by (lo, hi) (S10)
   struct Edge { int64_t key; int32_t cell, k; };
-  std::vector<Edge> edges(3 * nc);
+  std::vector<Edge> edges(ncorn);
   for (int64_t i = 0; i < nc; ++i)
-    for (int k = 0; k < 3; ++k) {
-      int32_t a = m.cell_nodes[3 * i + k], b = m.cell_nodes[3 * i + (k + 1) % 3];
+    for (int k = 0; k < m.nv(i); ++k) {
+      int32_t a = m.cell_nodes[m.cptr[i] + k], b = m.cell_nodes[m.cptr[i] + (k + 1) % m.nv(i)];
       int64_t lo = std::min(a, b), hi = std::max(a, b);
-      edges[3 * i + k] = {lo * (int64_t)m.nn + hi, (int32_t)i, k};
+      edges[m.cptr[i] + k] = {lo * (int64_t)m.nn + hi, (int32_t)i, k};
     }
   std::sort(edges.begin(), edges.end(), [](const Edge& x, const Edge& y) {
     return x.key != y.key ? x.key < y.key : (x.cell != y.cell ? x.cell < y.cell : x.k < y.k);
   });
   m.face_nodes.clear();
   m.face_cells.clear();
-  m.cell_faces.assign(3 * nc, -1);
+  m.cell_faces.assign(ncorn, -1);
   for (size_t e = 0; e < edges.size();) {
     size_t e2 = e;
     while (e2 < edges.size() && edges[e2].key == edges[e].key) ++e2;
@@ -124,38 +167,38 @@ int build(tfo_mesh& m) {
     m.face_cells.push_back(e2 - e == 2 ? edges[e + 1].cell : -1);
     if (e2 - e == 2 && edges[e].cell == edges[e + 1].cell)
       return fail(-2, "a cell is its own neighbour (periodic direction too narrow)");
-    for (size_t q = e; q < e2; ++q) m.cell_faces[3 * edges[q].cell + edges[q].k] = f;
+    for (size_t q = e; q < e2; ++q) m.cell_faces[m.cptr[edges[q].cell] + edges[q].k] = f;
     e = e2;
   }
   m.nf = (int64_t)m.face_cells.size() / 2;
   // vertex-neighbour stencil (L74: "all face-vertex cell neighbors"), ascending, unique, no self
   std::vector<std::vector<int32_t>> node_cells(m.nn);
   for (int64_t i = 0; i < nc; ++i)
-    for (int k = 0; k < 3; ++k) node_cells[m.cell_nodes[3 * i + k]].push_back((int32_t)i);
+    for (int k = 0; k < m.nv(i); ++k) node_cells[m.cell_nodes[m.cptr[i] + k]].push_back((int32_t)i);
   m.st_ptr.assign(nc + 1, 0);
   m.st_idx.clear();
   m.st_d.clear();
   for (int64_t i = 0; i < nc; ++i) {
     std::vector<int32_t> s;
-    for (int k = 0; k < 3; ++k)
-      for (int32_t j : node_cells[m.cell_nodes[3 * i + k]])
+    for (int k = 0; k < m.nv(i); ++k)
+      for (int32_t j : node_cells[m.cell_nodes[m.cptr[i] + k]])
         if (j != i) s.push_back(j);
     std::sort(s.begin(), s.end());
     s.erase(std::unique(s.begin(), s.end()), s.end());
     for (int32_t j : s) {
       // displacement through the smallest shared node id (S9, S22)
       int32_t v = INT32_MAX;
-      for (int a = 0; a < 3; ++a)
-        for (int b = 0; b < 3; ++b)
-          if (m.cell_nodes[3 * i + a] == m.cell_nodes[3 * j + b]) v = std::min(v, m.cell_nodes[3 * i + a]);
+      for (int a = 0; a < m.nv(i); ++a)
+        for (int b = 0; b < m.nv(j); ++b)
+          if (m.cell_nodes[m.cptr[i] + a] == m.cell_nodes[m.cptr[j] + b]) v = std::min(v, m.cell_nodes[m.cptr[i] + a]);
       int ai = 0, bj = 0;
-      for (int a = 0; a < 3; ++a) {
-        if (m.cell_nodes[3 * i + a] == v) ai = a;
-        if (m.cell_nodes[3 * j + a] == v) bj = a;
-      }
-      double dx = (m.cen[2 * j] - m.cell_xy[6 * j + 2 * bj]) - (m.cen[2 * i] - m.cell_xy[6 * i + 2 * ai]);
-      double dy = (m.cen[2 * j + 1] - m.cell_xy[6 * j + 2 * bj + 1]) -
-                  (m.cen[2 * i + 1] - m.cell_xy[6 * i + 2 * ai + 1]);
+      for (int a = 0; a < m.nv(i); ++a)
+        if (m.cell_nodes[m.cptr[i] + a] == v) ai = a;
+      for (int a = 0; a < m.nv(j); ++a)
+        if (m.cell_nodes[m.cptr[j] + a] == v) bj = a;
+      double dx = (m.cen[2 * j] - m.cell_xy[2 * (m.cptr[j] + bj)]) - (m.cen[2 * i] - m.cell_xy[2 * (m.cptr[i] + ai)]);
+      double dy = (m.cen[2 * j + 1] - m.cell_xy[2 * (m.cptr[j] + bj) + 1]) -
+                  (m.cen[2 * i + 1] - m.cell_xy[2 * (m.cptr[i] + ai) + 1]);
       m.st_idx.push_back(j);
       m.st_d.push_back(dx);
       m.st_d.push_back(dy);
@@ -167,8 +210,8 @@ int build(tfo_mesh& m) {
   m.bsr_col.clear();
   for (int64_t i = 0; i < nc; ++i) {
     std::vector<int32_t> cols{(int32_t)i};
-    for (int k = 0; k < 3; ++k) {
-      int32_t f = m.cell_faces[3 * i + k];
+    for (int k = 0; k < m.nv(i); ++k) {
+      int32_t f = m.cell_faces[m.cptr[i] + k];
       int32_t j = m.face_cells[2 * f] == i ? m.face_cells[2 * f + 1] : m.face_cells[2 * f];
       if (j >= 0) cols.push_back(j);
     }
@@ -177,6 +220,19 @@ int build(tfo_mesh& m) {
       return fail(-2, "two faces of a cell lead to the same neighbour (periodic direction too narrow)");
     for (int32_t j : cols) m.bsr_col.push_back(j);
     m.bsr_rowptr[i + 1] = (int32_t)m.bsr_col.size();
+  }
+  // boundary faces in ascending face id.  Faces are numbered by their node pair, so neither this list nor the
+  // tags attached to it change when the cells are reordered.
+  m.bfaces.clear();
+  m.bface_of.assign(m.nf, -1);
+  for (int64_t f = 0; f < m.nf; ++f)
+    if (m.face_cells[2 * f + 1] < 0) {
+      m.bface_of[f] = (int32_t)m.bfaces.size();
+      m.bfaces.push_back((int32_t)f);
+    }
+  if (m.bc_tag.size() != m.bfaces.size()) {
+    m.bc_tag.assign(m.bfaces.size(), TFO_BC_TRANSMISSIVE);
+    m.ghost.clear();
   }
   return 0;
 }
@@ -429,8 +485,8 @@ void grad_cell(const tfo_mesh& m, const tfo_numerics& nu, const double* P, int64
     const double Kh = nu.venkat_K * h;
     const double eps2 = Kh * Kh * Kh;
     double ph_i = 1.0;
-    for (int k = 0; k < 3; ++k) {
-      const double d2 = gx * m.fmid_off[6 * i + 2 * k] + gy * m.fmid_off[6 * i + 2 * k + 1];
+    for (int k = 0; k < m.nv(i); ++k) {
+      const double d2 = gx * m.fmid_off[2 * (m.cptr[i] + k)] + gy * m.fmid_off[2 * (m.cptr[i] + k) + 1];
       double pf = 1.0;
       if (d2 != 0.0) {
         const double d1 = d2 > 0.0 ? umax - Pi : umin - Pi;
@@ -449,9 +505,42 @@ inline void extrapolate(const double* Pc, const double* g, const double* phi, do
 }
 
 inline int local_face(const tfo_mesh& m, int64_t cell, int32_t f) {
-  for (int k = 0; k < 3; ++k)
-    if (m.cell_faces[3 * cell + k] == f) return k;
+  for (int k = 0; k < m.nv(cell); ++k)
+    if (m.cell_faces[m.cptr[cell] + k] == f) return k;
   return -1;
+}
+
+// Ghost state of a perfectly conducting slip wall (reading S24): the mirror image of the inner state, so that
+// the face mean has B.n = 0, E_tangential = 0 and u_s.n = 0.  Vectors that must vanish normally flip their
+// normal component (B, u_s); E flips its tangential components (z included); of each cleaning pair
+// (B_n, Psi), (E_n, Phi) one member flips and the other is kept; rho_s and T_s are kept.
+void wall_ghost(const double* P, double nx, double ny, double* G) {
+  for (int v = 0; v < NEQ; ++v) G[v] = P[v];
+  const double Bn = P[0] * nx + P[1] * ny;
+  G[0] = P[0] - 2.0 * Bn * nx;
+  G[1] = P[1] - 2.0 * Bn * ny;
+  const double En = P[3] * nx + P[4] * ny;
+  G[3] = -P[3] + 2.0 * En * nx;
+  G[4] = -P[4] + 2.0 * En * ny;
+  G[5] = -P[5];
+  G[7] = -P[7];
+  for (int s = 0; s < 2; ++s) {
+    const double un = P[i_u(s)] * nx + P[i_u(s) + 1] * ny;
+    G[i_u(s)] = P[i_u(s)] - 2.0 * un * nx;
+    G[i_u(s) + 1] = P[i_u(s) + 1] - 2.0 * un * ny;
+  }
+}
+
+// The boundary loop of L260: the state on the far side of boundary face f, given the reconstructed inner state.
+//   TFO_BC_TRANSMISSIVE  P_R := P_L                                        (S9)
+//   TFO_BC_GHOST         P_R := the caller's ghost state of that face      (does not move with P_L)
+//   TFO_BC_WALL          P_R := wall_ghost(P_L, n)                         (S24)
+void boundary_state(const tfo_mesh& m, int32_t f, const double* PL, double nx, double ny, double* PR) {
+  const int32_t b = m.bface_of[f];
+  const int tag = m.bc_tag[b];
+  if (tag == TFO_BC_GHOST) for (int v = 0; v < NEQ; ++v) PR[v] = m.ghost[(size_t)NEQ * b + v];
+  else if (tag == TFO_BC_WALL) wall_ghost(PL, nx, ny, PR);
+  else for (int v = 0; v < NEQ; ++v) PR[v] = PL[v];
 }
 
 // perturbation size (S7): eps_k = delta * max(|P_cell,k|, ref_k), made representable
@@ -468,7 +557,7 @@ struct GradSource {
   const double* phi = nullptr;    // [nc][18]
 };
 
-// One row of Alg. 1 for cell i.  rhs_row[18], scale_row[18], blocks: up to 4 [18][18] in BSR order.
+// One row of Alg. 1 for cell i.  rhs_row[18], scale_row[18], blocks: the row's [18][18] blocks in BSR order.
 void assemble_row(const tfo_mesh& m, const tfo_physics& ph, const tfo_numerics& nu, const double* P,
                   const double* Pn, const double* Pnm1, double dt, int64_t i, const double* g_all,
                   const double* phi_all, const int32_t* gmap /*cell -> slot in g_all or NULL*/,
@@ -490,21 +579,22 @@ void assemble_row(const tfo_mesh& m, const tfo_physics& ph, const tfo_numerics& 
 
   // ---- loop over the faces of the cell (L230-244) ----
   if (do_flux)
-    for (int k = 0; k < 3; ++k) {
-      const int32_t f = m.cell_faces[3 * i + k];
+    for (int k = 0; k < m.nv(i); ++k) {
+      const int32_t f = m.cell_faces[m.cptr[i] + k];
       const int64_t cL = m.face_cells[2 * f], cR = m.face_cells[2 * f + 1];
       const bool own_is_L = (cL == i);
       const double s_if = own_is_L ? 1.0 : -1.0;
       const int kL = local_face(m, cL, f);
       // normal, length and midpoint offset from the L cell; R's offset from R's own corners
-      const double nx = m.fnrm[6 * cL + 2 * kL], ny = m.fnrm[6 * cL + 2 * kL + 1];
-      const double len = m.flen[3 * cL + kL];
-      const double dLx = m.fmid_off[6 * cL + 2 * kL], dLy = m.fmid_off[6 * cL + 2 * kL + 1];
+      const int64_t eL = m.cptr[cL] + kL;
+      const double nx = m.fnrm[2 * eL], ny = m.fnrm[2 * eL + 1];
+      const double len = m.flen[eL];
+      const double dLx = m.fmid_off[2 * eL], dLy = m.fmid_off[2 * eL + 1];
       double dRx = 0, dRy = 0;
       if (cR >= 0) {
-        const int kR = local_face(m, cR, f);
-        dRx = m.fmid_off[6 * cR + 2 * kR];
-        dRy = m.fmid_off[6 * cR + 2 * kR + 1];
+        const int64_t eR = m.cptr[cR] + local_face(m, cR, f);
+        dRx = m.fmid_off[2 * eR];
+        dRy = m.fmid_off[2 * eR + 1];
       }
       const double* gL = g_all + slot(cL) * NEQ * 2;
       const double* phL = phi_all + slot(cL) * NEQ;
@@ -513,7 +603,7 @@ void assemble_row(const tfo_mesh& m, const tfo_physics& ph, const tfo_numerics& 
       double PL[NEQ], PR[NEQ], H[NEQ];
       extrapolate(P + NEQ * cL, gL, phL, dLx, dLy, PL);
       if (cR >= 0) extrapolate(P + NEQ * cR, gR, phR, dRx, dRy, PR);
-      else for (int v = 0; v < NEQ; ++v) PR[v] = PL[v];           // boundary: P_R := P_L (S9)
+      else boundary_state(m, f, PL, nx, ny, PR);                  // boundary face (L260; S9, S24)
       face_flux(ph, nu, PL, PR, nx, ny, H);
       for (int r = 0; r < NEQ; ++r) {
         Rt[r] += s_if * H[r] * len;
@@ -532,7 +622,7 @@ void assemble_row(const tfo_mesh& m, const tfo_physics& ph, const tfo_numerics& 
           if (side == 0) {
             extrapolate(Pc, gL, phL, dLx, dLy, PLp);
             if (cR >= 0) for (int q = 0; q < NEQ; ++q) PRp[q] = PR[q];
-            else for (int q = 0; q < NEQ; ++q) PRp[q] = PLp[q];   // boundary: both arguments move
+            else boundary_state(m, f, PLp, nx, ny, PRp);          // boundary: the far side follows its rule
           } else {
             for (int q = 0; q < NEQ; ++q) PLp[q] = PL[q];
             extrapolate(Pc, gR, phR, dRx, dRy, PRp);
@@ -624,19 +714,29 @@ void tfo_default_numerics(tfo_numerics* n, const tfo_physics* p) {
   n->pad_ = 0;
 }
 
-int tfo_mesh_create(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
-                    const int32_t* cell_nodes, const double* cell_xy) {
+static int create_common(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                         const int32_t* cell_ptr /*NULL: triangles*/, const int32_t* cell_nodes,
+                         const double* cell_xy) {
   if (!out || !cell_nodes || n_cells < 0 || n_nodes < 0 || (!node_xy && !cell_xy))
     return fail(-1, "tfo_mesh_create: bad argument");
   tfo_mesh* m = new tfo_mesh;
   m->nn = n_nodes;
   m->nc = n_cells;
+  m->cptr.resize(n_cells + 1);
+  for (int64_t i = 0; i <= n_cells; ++i) m->cptr[i] = cell_ptr ? cell_ptr[i] : (int32_t)(3 * i);
+  if (m->cptr[0] != 0) { delete m; return fail(-1, "cell_ptr must start at 0"); }
+  for (int64_t i = 0; i < n_cells; ++i)
+    if (m->cptr[i + 1] - m->cptr[i] < 3 || m->cptr[i + 1] - m->cptr[i] > TFO_MAXV) {
+      delete m;
+      return fail(-2, "cell " + std::to_string(i) + " must have 3 or 4 corners");
+    }
+  const int64_t ncorn = m->cptr[n_cells];
   if (node_xy) m->node_xy.assign(node_xy, node_xy + 2 * n_nodes);
-  m->cell_nodes.assign(cell_nodes, cell_nodes + 3 * n_cells);
-  if (cell_xy) m->cell_xy.assign(cell_xy, cell_xy + 6 * n_cells);
+  m->cell_nodes.assign(cell_nodes, cell_nodes + ncorn);
+  if (cell_xy) m->cell_xy.assign(cell_xy, cell_xy + 2 * ncorn);
   else {
-    m->cell_xy.resize(6 * n_cells);
-    for (int64_t i = 0; i < 3 * n_cells; ++i) {
+    m->cell_xy.resize(2 * ncorn);
+    for (int64_t i = 0; i < ncorn; ++i) {
       int32_t v = cell_nodes[i];
       if (v < 0 || v >= n_nodes) { delete m; return fail(-2, "node id out of range"); }
       m->cell_xy[2 * i] = node_xy[2 * v];
@@ -649,6 +749,17 @@ int tfo_mesh_create(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int6
   if (rc) { delete m; return rc; }
   *out = m;
   return 0;
+}
+
+int tfo_mesh_create(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                    const int32_t* cell_nodes, const double* cell_xy) {
+  return create_common(out, n_nodes, node_xy, n_cells, nullptr, cell_nodes, cell_xy);
+}
+
+int tfo_mesh_create_poly(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                         const int32_t* cell_ptr, const int32_t* cell_nodes, const double* cell_xy) {
+  if (!cell_ptr) return fail(-1, "tfo_mesh_create_poly: cell_ptr missing");
+  return create_common(out, n_nodes, node_xy, n_cells, cell_ptr, cell_nodes, cell_xy);
 }
 
 int tfo_mesh_reorder(tfo_mesh* m, int kind, const int32_t* user_perm) {
@@ -665,17 +776,47 @@ int tfo_mesh_reorder(tfo_mesh* m, int kind, const int32_t* user_perm) {
       hit[p[i]] = 1;
     }
   } else return fail(-1, "unknown reorder kind");
-  std::vector<int32_t> cn(3 * m->nc), pm(m->nc);
-  std::vector<double> cx(6 * m->nc);
+  std::vector<int32_t> cp(m->nc + 1, 0), cn, pm(m->nc);
+  std::vector<double> cx;
+  cn.reserve(m->cell_nodes.size());
+  cx.reserve(m->cell_xy.size());
   for (int64_t i = 0; i < m->nc; ++i) {
-    for (int k = 0; k < 3; ++k) cn[3 * i + k] = m->cell_nodes[3 * (int64_t)p[i] + k];
-    for (int k = 0; k < 6; ++k) cx[6 * i + k] = m->cell_xy[6 * (int64_t)p[i] + k];
-    pm[i] = m->perm[p[i]];
+    const int64_t o = p[i];
+    for (int32_t q = m->cptr[o]; q < m->cptr[o + 1]; ++q) {
+      cn.push_back(m->cell_nodes[q]);
+      cx.push_back(m->cell_xy[2 * q]);
+      cx.push_back(m->cell_xy[2 * q + 1]);
+    }
+    cp[i + 1] = (int32_t)cn.size();
+    pm[i] = m->perm[o];
   }
+  m->cptr.swap(cp);
   m->cell_nodes.swap(cn);
   m->cell_xy.swap(cx);
   m->perm.swap(pm);
-  return build(*m);
+  return build(*m);   // faces keep their ids (they are numbered by node pair), so the boundary tags stay valid
+}
+
+int tfo_mesh_info(const tfo_mesh* m, int32_t* max_faces, int64_t* n_bfaces) {
+  if (!m) return fail(-1, "null mesh");
+  if (max_faces) *max_faces = m->maxf;
+  if (n_bfaces) *n_bfaces = (int64_t)m->bfaces.size();
+  return 0;
+}
+
+int tfo_mesh_set_bc(tfo_mesh* m, const int32_t* tags, const double* ghost) {
+  if (!m || !tags) return fail(-1, "null argument");
+  const size_t nb = m->bfaces.size();
+  bool need_ghost = false;
+  for (size_t b = 0; b < nb; ++b) {
+    if (tags[b] < 0 || tags[b] > TFO_BC_WALL) return fail(-1, "unknown boundary tag");
+    need_ghost |= tags[b] == TFO_BC_GHOST;
+  }
+  if (need_ghost && !ghost) return fail(-1, "ghost states missing for TFO_BC_GHOST faces");
+  m->bc_tag.assign(tags, tags + nb);
+  if (ghost) m->ghost.assign(ghost, ghost + (size_t)NEQ * nb);
+  else m->ghost.clear();
+  return 0;
 }
 
 int tfo_mesh_sizes(const tfo_mesh* m, int64_t* n_cells, int64_t* n_faces, int64_t* nnzb, int64_t* n_stencil) {
@@ -692,10 +833,20 @@ int tfo_mesh_get(const tfo_mesh* m, int which, void* dst, int64_t bytes) {
   const void* src = nullptr;
   int64_t n = 0;
   std::vector<double> tmp;
+  std::vector<int32_t> itmp;
   switch (which) {
     case TFO_FACE_CELLS: src = m->face_cells.data(); n = m->face_cells.size() * 4; break;
     case TFO_FACE_NODES: src = m->face_nodes.data(); n = m->face_nodes.size() * 4; break;
-    case TFO_CELL_FACES: src = m->cell_faces.data(); n = m->cell_faces.size() * 4; break;
+    case TFO_CELL_FACES: {   // [nc][maxf], -1 where a cell has fewer faces
+      itmp.assign((size_t)m->nc * m->maxf, -1);
+      for (int64_t i = 0; i < m->nc; ++i)
+        for (int k = 0; k < m->nv(i); ++k) itmp[(size_t)i * m->maxf + k] = m->cell_faces[m->cptr[i] + k];
+      src = itmp.data();
+      n = itmp.size() * 4;
+      break;
+    }
+    case TFO_BFACES: src = m->bfaces.data(); n = m->bfaces.size() * 4; break;
+    case TFO_BC_TAGS: src = m->bc_tag.data(); n = m->bc_tag.size() * 4; break;
     case TFO_STENCIL_PTR: src = m->st_ptr.data(); n = m->st_ptr.size() * 4; break;
     case TFO_STENCIL_IDX: src = m->st_idx.data(); n = m->st_idx.size() * 4; break;
     case TFO_BSR_ROWPTR: src = m->bsr_rowptr.data(); n = m->bsr_rowptr.size() * 4; break;
@@ -708,9 +859,9 @@ int tfo_mesh_get(const tfo_mesh* m, int which, void* dst, int64_t bytes) {
       for (int64_t f = 0; f < m->nf; ++f) {
         int64_t cL = m->face_cells[2 * f];
         int k = local_face(*m, cL, (int32_t)f);
-        tmp[3 * f] = m->fnrm[6 * cL + 2 * k];
-        tmp[3 * f + 1] = m->fnrm[6 * cL + 2 * k + 1];
-        tmp[3 * f + 2] = m->flen[3 * cL + k];
+        tmp[3 * f] = m->fnrm[2 * (m->cptr[cL] + k)];
+        tmp[3 * f + 1] = m->fnrm[2 * (m->cptr[cL] + k) + 1];
+        tmp[3 * f + 2] = m->flen[m->cptr[cL] + k];
       }
       src = tmp.data();
       n = tmp.size() * 8;
@@ -766,8 +917,9 @@ int tfo_assemble(const tfo_mesh* m, const tfo_physics* ph, const tfo_numerics* n
     grad_cell(*m, *nu, state, need[q], &g[2 * NEQ * q], &phi[NEQ * q]);
 #pragma omp parallel for schedule(static)
   for (int64_t r = 0; r < n_rows; ++r) {
-    double* blk = vals ? vals + r * 4 * NEQ * NEQ : nullptr;
-    if (blk) for (int q = 0; q < 4 * NEQ * NEQ; ++q) blk[q] = 0.0;
+    const int64_t nb = (int64_t)(m->maxf + 1) * NEQ * NEQ;   // blocks per row, zero padded
+    double* blk = vals ? vals + r * nb : nullptr;
+    if (blk) for (int64_t q = 0; q < nb; ++q) blk[q] = 0.0;
     assemble_row(*m, *ph, *nu, state, state_n, state_nm1, dt, rows[r], g.data(), phi.data(), gmap.data(),
                  rhs + NEQ * r, scale ? scale + NEQ * r : nullptr, blk);
   }
@@ -819,6 +971,7 @@ void tfo_ausm_split(double M, double alpha, double beta, double* o) {
   o[2] = P5p(M, alpha);
   o[3] = P5m(M, alpha);
 }
+void tfo_wall_ghost(const double* P18, double nx, double ny, double* G18) { wall_ghost(P18, nx, ny, G18); }
 void tfo_source(const tfo_physics* ph, const double* P18, double* S18) { source(*ph, P18, S18); }
 void tfo_cons(const tfo_physics* ph, const double* P18, double* U18) { cons(*ph, P18, U18); }
 void tfo_dcons_dprim(const tfo_physics* ph, const double* P18, double* D) { dcons_dprim(*ph, P18, D); }

@@ -9,21 +9,35 @@
  * readings S1..S23 listed in DESIGN.md.  No blocking, fusion or reordering beyond what
  * Algorithm 1 (L221-256) states.  All pointers are HOST pointers.
  *
+ * Cells are triangles or convex quadrilaterals, mixed freely (the paper's meshes are Cartesian
+ * quadrilaterals, L433, L559); boundary faces follow one of three rules (L260; S9, S24).
+ *
  * Pins (tests/test_oracle_*.py, -m "not gpu"):
- *   connectivity  : Euler counts, tests/golden/ hand-worked 2x2 mesh, brute-force O(n^2) adjacency
- *   gradient      : exact for linear fields; limiter closed forms (phi=1 const field, 0.75 point)
+ *   connectivity  : Euler counts, tests/golden/ hand-worked 2x2 meshes (triangles, quadrilaterals),
+ *                   brute-force O(n^2) adjacency, independent serial RCM
+ *   geometry      : Green's-theorem area and centroid, both diagonal splits of a quadrilateral, closed normals
+ *   gradient      : exact for linear fields; on Cartesian quads equal to the weighted central differences;
+ *                   limiter closed forms: phi = 1 (constant field), 0.75 point, K = 0 and finite K on a linear
+ *                   field (eps^2 = (K sqrt(Omega))^3)
  *   Maxwell flux  : consistency L85, exact upwind vs numpy eig of A_n, eigenvalues, antisymmetry
- *   AUSM+-up      : consistency L85, antisymmetry, supersonic upwinding, rotation covariance
+ *   AUSM+-up      : consistency L85, antisymmetry, supersonic upwinding, rotation covariance; magnitudes of the
+ *                   pressure-diffusion term M_p (fluid at rest, closed form) and of the velocity-diffusion term
+ *                   p_u (symmetric streams, closed form)
  *   source        : momentum/energy bookkeeping  sum_s S_mom = rho_c E + J x B, sum S_en = J.E
  *   residual      : free-stream preservation, periodic telescoping, rotation covariance
- *   Jacobian      : brute-force central differences of the oracle's own frozen residual;
- *                   Maxwell sub-block against the closed-form matrix; time term vs dU/dP by FD
- *   against the paper (tests/test_exact_wave.py): the exact circularly polarised wave of Eq. 15-18 makes the
- *                   spatial residual converge at second order; Newton on a BDF2 step of it contracts and lands
- *                   on the exact solution; Harris-sheet total force balance and Ampere's law (GEM set-up)
+ *   Jacobian      : brute-force central differences of the oracle's own frozen residual (triangles, quadrilaterals,
+ *                   mixed, with all three boundary rules); Maxwell sub-block linear; time term vs dU/dP by FD
+ *   boundary      : wall mirror state is an involution with B.n = E_t = u.n = 0 at the face and no mass, energy,
+ *                   Psi or tangential flux through it; a ghost-state face fed the neighbour's face state is an
+ *                   interior face (cut-mesh test)
+ *   against the paper (tests/test_exact_wave.py, test_oracle_quads.py): the exact circularly polarised wave of
+ *                   Eq. 15-18 makes the spatial residual converge at second order (split triangles, and the
+ *                   paper's 2N x N quadrilaterals); Newton on a BDF2 step of it contracts and lands on the exact
+ *                   solution; Harris-sheet total force balance and Ampere's law (GEM set-up)
  * Unpinned (no independent value available):
  *   |A_n| vs ref. [4] of the paper (S3), AUSM+-up constants / a_1/2 choice vs COOLFluiD (S4),
- *   LS weight exponent (S12), Venkatakrishnan eps^2=(K h)^3 (S13).
+ *   LS weight exponent (S12: any weight is exact on linear fields), the wall rule's choice of which member of
+ *   each cleaning pair flips (S24).
  */
 #ifndef TFO_H
 #define TFO_H
@@ -56,14 +70,28 @@ typedef struct tfo_numerics {
 
 typedef struct tfo_mesh tfo_mesh;
 
-enum { TFO_FACE_CELLS = 0, TFO_CELL_FACES = 1, TFO_STENCIL_PTR = 2, TFO_STENCIL_IDX = 3,
-       TFO_BSR_ROWPTR = 4, TFO_BSR_COL = 5, TFO_PERM = 6, TFO_VOLUME = 7,
-       TFO_FACE_NORMAL_LEN = 8, TFO_CENTROID = 9, TFO_FACE_NODES = 10 };
+enum { TFO_FACE_CELLS = 0, TFO_CELL_FACES = 1 /* [nc][max_faces], -1 padded */, TFO_STENCIL_PTR = 2,
+       TFO_STENCIL_IDX = 3, TFO_BSR_ROWPTR = 4, TFO_BSR_COL = 5, TFO_PERM = 6, TFO_VOLUME = 7,
+       TFO_FACE_NORMAL_LEN = 8, TFO_CENTROID = 9, TFO_FACE_NODES = 10,
+       TFO_BFACES = 12 /* int32 [n_bfaces]: boundary faces, ascending face id */, TFO_BC_TAGS = 13 };
+
+/* cells are triangles or convex quadrilaterals (the paper's meshes are Cartesian quads, L433, L559) */
+#define TFO_MAXV 4
+/* rule for the far side of a boundary face (the paper's separate boundary loop, L260; readings S9, S24) */
+enum { TFO_BC_TRANSMISSIVE = 0 /* P_R := P_L */, TFO_BC_GHOST = 1 /* P_R := given ghost state, held fixed */,
+       TFO_BC_WALL = 2 /* P_R := mirror image of P_L: perfectly conducting slip wall */ };
 
 /* connectivity + geometry (L74, L230) */
 int  tfo_mesh_create(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
                      const int32_t* cell_nodes, const double* cell_xy);
+/* mixed triangle / quadrilateral mesh: corners of cell i are cell_nodes[cell_ptr[i] .. cell_ptr[i+1]),
+ * counter-clockwise; cell_xy [cell_ptr[n_cells]][2] in the same layout (or NULL) */
+int  tfo_mesh_create_poly(tfo_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                          const int32_t* cell_ptr, const int32_t* cell_nodes, const double* cell_xy);
 int  tfo_mesh_reorder(tfo_mesh* m, int kind /*0 none, 1 RCM, 2 user*/, const int32_t* user_perm);
+int  tfo_mesh_info(const tfo_mesh* m, int32_t* max_faces, int64_t* n_bfaces);
+/* tags [n_bfaces] (order of TFO_BFACES); ghost [n_bfaces][18] (copied; may be NULL without TFO_BC_GHOST faces) */
+int  tfo_mesh_set_bc(tfo_mesh* m, const int32_t* tags, const double* ghost);
 int  tfo_mesh_sizes(const tfo_mesh* m, int64_t* n_cells, int64_t* n_faces, int64_t* nnzb,
                     int64_t* n_stencil);
 int  tfo_mesh_get(const tfo_mesh* m, int which, void* dst, int64_t bytes);
@@ -79,7 +107,7 @@ int tfo_gradients(const tfo_mesh* m, const tfo_numerics* nu, const double* state
 /* steps a3..a7 (Alg. 1; Eq. 8-13).  rows==NULL: all rows, rhs[nc][18], scale[nc][18]
  * (sum of |terms| per entry, may be NULL), vals[nnzb][18][18] (may be NULL -> residual only).
  * rows!=NULL: compact output for the listed rows: rhs[n_rows][18], scale[n_rows][18],
- * vals[n_rows][4][18][18] (the row's blocks in BSR column order, zero padded). */
+ * vals[n_rows][max_faces+1][18][18] (the row's blocks in BSR column order, zero padded). */
 int tfo_assemble(const tfo_mesh* m, const tfo_physics* ph, const tfo_numerics* nu,
                  const double* state, const double* state_n, const double* state_nm1, double dt,
                  double* rhs, double* scale, double* vals, int64_t n_rows, const int32_t* rows);
@@ -97,6 +125,7 @@ void tfo_flux_ausm(const tfo_physics* ph, const tfo_numerics* nu, int species, c
 void tfo_flux_face(const tfo_physics* ph, const tfo_numerics* nu, const double* PL18,
                    const double* PR18, double nx, double ny, double* H18);
 void tfo_phys_flux(const tfo_physics* ph, const double* P18, double nx, double ny, double* F18);
+void tfo_wall_ghost(const double* P18, double nx, double ny, double* G18);   /* S24 */
 void tfo_source(const tfo_physics* ph, const double* P18, double* S18);
 void tfo_cons(const tfo_physics* ph, const double* P18, double* U18);
 void tfo_dcons_dprim(const tfo_physics* ph, const double* P18, double* dUdP /*[18][18]*/);

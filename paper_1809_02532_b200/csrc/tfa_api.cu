@@ -23,13 +23,14 @@ int prepare(tfa_ctx* ctx, const tfa_mesh* m, cudaStream_t st) {
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  if (ctx->ws_mesh == m && ctx->ws_generation == m->generation && ctx->ws_power == ctx->nu.lsq_weight_power)
+  if (ctx->ws_uid == m->uid && ctx->ws_power == ctx->nu.lsq_weight_power && ctx->lsq_coef.n >= 2 * m->nst &&
+      ctx->fown.n >= 3 * NEQ * m->nc)
     return 0;
+  ctx->ws_uid = 0;
   TFA_CUDA(ctx->lsq_coef.alloc(2 * m->nst));
   TFA_CUDA(ctx->fown.alloc(3 * NEQ * m->nc));
   TFA_TRY(launch_lsq_coef(*m, ctx->nu.lsq_weight_power, ctx->lsq_coef.p, st));
-  ctx->ws_mesh = m;
-  ctx->ws_generation = m->generation;
+  ctx->ws_uid = m->uid;
   ctx->ws_power = ctx->nu.lsq_weight_power;
   return 0;
 }
@@ -107,8 +108,13 @@ int tfa_gradients(tfa_ctx* ctx, const tfa_mesh* m, const double* state, double* 
   return launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, nullptr, grad, phi, st);
 }
 
-int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
-                 const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {
+}  // extern "C"
+
+namespace tfa {
+// the two launches of one assembly, with optional per-kernel events (tfa_timing_enable); the matrix-free
+// operator's evaluations call it untimed, so that a long solve never exhausts the event ring
+int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed) {
   if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
   if (m->nc == 0) { ctx->launches = 0; return 0; }   // empty mesh: nothing to write
   if (!state || !state_n || !state_nm1 || !rhs) return set_error(TFA_EINVAL, "null argument");
@@ -117,7 +123,7 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
   TFA_TRY(prepare(ctx, m, st));
   const Consts K = make_consts(ctx->ph, ctx->nu);
   cudaEvent_t* ev = nullptr;
-  if (ctx->timing) {
+  if (timed && ctx->timing) {
     if (ctx->timed >= tfa_ctx::kMaxTimed) return set_error(TFA_EINVAL, "tfa_timing_read must be called every 64 assemblies");
     ev = ctx->ev[ctx->timed];
     for (int q = 0; q < 3; ++q)
@@ -135,6 +141,14 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
   ctx->launches = 2;
   return 0;
 }
+}  // namespace tfa
+
+extern "C" {
+
+int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                 const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {
+  return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream, true);
+}
 
 int tfa_assemble_host(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                       const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {
@@ -144,19 +158,19 @@ int tfa_assemble_host(tfa_ctx* ctx, const tfa_mesh* m, const double* state, cons
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t ns = NEQ * m->nc, nv = (int64_t)BLK * m->nnzb;
   for (int q = 0; q < 3; ++q)
-    if (ctx->h_state[q].n < ns) TFA_CUDA(ctx->h_state[q].alloc(ns));
-  if (ctx->h_rhs.n < ns) TFA_CUDA(ctx->h_rhs.alloc(ns));
-  if (bsr_vals && ctx->h_vals.n < nv) TFA_CUDA(ctx->h_vals.alloc(nv));
+    if (ctx->stage_state[q].n < ns) TFA_CUDA(ctx->stage_state[q].alloc(ns));
+  if (ctx->stage_rhs.n < ns) TFA_CUDA(ctx->stage_rhs.alloc(ns));
+  if (bsr_vals && ctx->stage_vals.n < nv) TFA_CUDA(ctx->stage_vals.alloc(nv));
   const double* src[3] = {state, state_n, state_nm1};
   for (int q = 0; q < 3; ++q) {
     // identical host pointers (P^n = P^{n-1} = P at the first step) are still three copies:
     // the device path is unchanged and the byte count is the honest per-step figure
-    TFA_CUDA(cudaMemcpyAsync(ctx->h_state[q].p, src[q], (size_t)ns * 8, cudaMemcpyHostToDevice, st));
+    TFA_CUDA(cudaMemcpyAsync(ctx->stage_state[q].p, src[q], (size_t)ns * 8, cudaMemcpyHostToDevice, st));
   }
-  TFA_TRY(tfa_assemble(ctx, m, ctx->h_state[0].p, ctx->h_state[1].p, ctx->h_state[2].p, dt, ctx->h_rhs.p,
-                       bsr_vals ? ctx->h_vals.p : nullptr, stream));
-  TFA_CUDA(cudaMemcpyAsync(rhs, ctx->h_rhs.p, (size_t)ns * 8, cudaMemcpyDeviceToHost, st));
-  if (bsr_vals) TFA_CUDA(cudaMemcpyAsync(bsr_vals, ctx->h_vals.p, (size_t)nv * 8, cudaMemcpyDeviceToHost, st));
+  TFA_TRY(tfa_assemble(ctx, m, ctx->stage_state[0].p, ctx->stage_state[1].p, ctx->stage_state[2].p, dt, ctx->stage_rhs.p,
+                       bsr_vals ? ctx->stage_vals.p : nullptr, stream));
+  TFA_CUDA(cudaMemcpyAsync(rhs, ctx->stage_rhs.p, (size_t)ns * 8, cudaMemcpyDeviceToHost, st));
+  if (bsr_vals) TFA_CUDA(cudaMemcpyAsync(bsr_vals, ctx->stage_vals.p, (size_t)nv * 8, cudaMemcpyDeviceToHost, st));
   TFA_CUDA(cudaStreamSynchronize(st));
   return 0;
 }

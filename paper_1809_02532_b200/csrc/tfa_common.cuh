@@ -13,6 +13,7 @@
 namespace tfa {
 
 int set_error(int code, const std::string& msg);
+uint64_t next_mesh_uid();
 
 #define TFA_CUDA(expr)                                                                          \
   do {                                                                                          \
@@ -71,7 +72,7 @@ struct DevBuf {
 
 struct tfa_mesh {
   int64_t nn = 0, nc = 0, nf = 0, nnzb = 0, nst = 0;
-  uint64_t generation = 0;   // bumped by every (re)build; ctx workspaces key on it
+  uint64_t uid = 0;          // process-wide monotonic stamp, new at every (re)build; ctx workspaces key on it
   tfa::DevBuf<double> node_xy;     // [nn][2]
   tfa::DevBuf<int32_t> cell_nodes; // [nc][3]
   tfa::DevBuf<double> cell_xy;     // [nc][3][2]
@@ -91,9 +92,8 @@ struct tfa_mesh {
 struct tfa_ctx {
   tfa_physics ph;
   tfa_numerics nu;
-  // workspace, keyed on (mesh, generation, lsq_weight_power)
-  const tfa_mesh* ws_mesh = nullptr;
-  uint64_t ws_generation = 0;
+  // workspace, keyed on (mesh uid, lsq_weight_power).  A context serves one stream at a time and is not thread-safe.
+  uint64_t ws_uid = 0;
   double ws_power = -1.0;
   tfa::DevBuf<double> lsq_coef;   // [nst][2]
   tfa::DevBuf<double> fown;       // [nc][3][18] own-side face states P_i + phi grad P_i . (x_f - x_i)  (L232)
@@ -102,8 +102,8 @@ struct tfa_ctx {
   tfa::DevBuf<double> krylov, red;
   // matrix-free operator: perturbed state and its residual; the base residual
   tfa::DevBuf<double> jfnk, jfnk0;
-  // staging for tfa_assemble_host
-  tfa::DevBuf<double> h_state[3], h_rhs, h_vals;
+  // device staging buffers of tfa_assemble_host
+  tfa::DevBuf<double> stage_state[3], stage_rhs, stage_vals;
   int launches = 0;
   int asm_resident_ctas = 0;      // persistent grid of k_assemble on this context's device (0 = not queried yet)
   // optional per-kernel timing (tfa_timing_enable): a ring of event triples

@@ -9,6 +9,7 @@
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
 
+#include <atomic>
 #include <vector>
 
 #include "tfa_common.cuh"
@@ -19,6 +20,12 @@ thread_local std::string g_last_error;
 int set_error(int code, const std::string& msg) {
   g_last_error = msg;
   return code;
+}
+// Every (re)built mesh gets a stamp no other mesh of the process ever had: a context's per-mesh workspace keys
+// on it, so a new mesh allocated at the address of a destroyed one is never mistaken for it.
+uint64_t next_mesh_uid() {
+  static std::atomic<uint64_t> counter{0};
+  return ++counter;
 }
 
 namespace {
@@ -525,7 +532,7 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
     TFA_CUDA(m.face_nodes.alloc(0)); TFA_CUDA(m.face_cells.alloc(0)); TFA_CUDA(m.cell_faces.alloc(0));
     TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.nbrf.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
     TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0)); TFA_CUDA(m.blk4.alloc(0));
-    ++m.generation;
+    m.uid = next_mesh_uid();
     return 0;
   }
   k_cell_geom<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, nn, m.cell_nodes.p, m.cell_xy.p, m.cen.p, vol.p, olen.p, onrm.p,
@@ -616,7 +623,7 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
   k_nbr_face<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m.cell_nbr.p, m.cell_faces.p, m.nbrf.p);
   TFA_CUDA(cudaGetLastError());
   TFA_CUDA(cudaStreamSynchronize(st));
-  ++m.generation;
+  m.uid = next_mesh_uid();
   return 0;
 }
 

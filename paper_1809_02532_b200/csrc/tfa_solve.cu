@@ -8,6 +8,8 @@
 #include "tfa_common.cuh"
 
 namespace tfa {
+int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed);
 
 constexpr int SV_CELLS = 16;              // cells per CTA: thread = (cell, scalar row)
 constexpr int SV_T = SV_CELLS * NEQ;      // 288 threads
@@ -51,8 +53,7 @@ __global__ void __launch_bounds__(SV_T) k_bsr_spmv(int64_t nc, const int32_t* __
 // per element made it shared-memory-bandwidth bound, 9.8 ms at 1M cells.)
 // ------------------------------------------------------------------------------------------------
 constexpr int BJ_WARPS = 8;
-__global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ rowptr,
-                                                               const int32_t* __restrict__ col,
+__global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ blk4,
                                                                const double* __restrict__ vals,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
   __shared__ __align__(16) double rowbuf[BJ_WARPS][2][NEQ];
@@ -60,9 +61,7 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
   if (i >= nc) return;
-  int64_t bd = -1;
-  for (int32_t b = rowptr[i]; b < rowptr[i + 1]; ++b)
-    if (col[b] == (int32_t)i) bd = b;
+  const int64_t bd = blk4[4 * i];   // the diagonal block of row i (every row of the mesh's pattern has one)
   const bool has = lane < NEQ;
   double a[NEQ];
 #pragma unroll
@@ -259,7 +258,11 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
     TFA_TRY(G.dots(1, w, n, w));
     const double beta = std::sqrt(G.host[0]);
     rel = beta / bnorm;
-    if (rel <= rtol || iters >= max_iters || !std::isfinite(beta)) break;
+    info[0] = (double)iters;
+    info[1] = rel;
+    // a non-finite residual (NaN / Inf in the matrix, the preconditioner or b): x holds the last iterate
+    if (!std::isfinite(beta)) return set_error(TFA_ESINGULAR, "tfa_gmres: the residual norm is not finite");
+    if (rel <= rtol || iters >= max_iters) break;
     k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / beta, w, 0.0, nullptr, V);
     std::fill(g.begin(), g.end(), 0.0);
     g[0] = beta;
@@ -285,6 +288,7 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
         before = hk1;
       }
       h[k + 1] = hk1;
+      if (!std::isfinite(hk1)) return set_error(TFA_ESINGULAR, "tfa_gmres: a Krylov vector is not finite");
       if (hk1 > 0.0) k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / hk1, w, 0.0, nullptr, V + (int64_t)(k + 1) * n);
       // Givens rotations on column k of the Hessenberg matrix
       for (int j = 0; j < k; ++j) {
@@ -293,6 +297,9 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
         h[j] = t;
       }
       const double den = std::hypot(h[k], h[k + 1]);
+      // breakdown with a singular Hessenberg column (A M^-1 maps the Krylov space into itself without reaching
+      // b): the least-squares problem has no unique solution; x keeps the previous cycle's iterate
+      if (den == 0.0) return set_error(TFA_ESINGULAR, "tfa_gmres: breakdown on a singular operator");
       cs[k] = den > 0.0 ? h[k] / den : 1.0;
       sn[k] = den > 0.0 ? h[k + 1] / den : 0.0;
       h[k] = den;
@@ -349,7 +356,7 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, bsr_vals, dinv,
+  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->blk4.p, bsr_vals, dinv,
                                                                   ctx->flags.p);
   TFA_CUDA(cudaGetLastError());
   return 0;
@@ -390,7 +397,7 @@ static int jvp_core(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const 
     eps = 1e-7 * (1.0 + rms_state) / rv;
   }
   k_axpby<<<RED_B, RED_T, 0, st>>>(n, eps, v, 1.0, state, Pp);                                  // P + eps v
-  TFA_TRY(tfa_assemble(ctx, m, Pp, state_n, state_nm1, dt, rp, nullptr, stream));              // rhs = -R~
+  TFA_TRY(assemble_impl(ctx, m, Pp, state_n, state_nm1, dt, rp, nullptr, stream, false));   // rhs = -R~
   k_axpby<<<RED_B, RED_T, 0, st>>>(n, -1.0 / eps, rp, 1.0 / eps, rhs0, out);                    // (R~' - R~) / eps
   TFA_CUDA(cudaGetLastError());
   return 0;
@@ -403,7 +410,7 @@ int tfa_jvp(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* 
   if (!state || !state_n || !state_nm1 || !v || !out) return set_error(TFA_EINVAL, "null argument");
   const int64_t n = (int64_t)NEQ * m->nc;
   if (ctx->jfnk0.n < n) TFA_CUDA(ctx->jfnk0.alloc(n));
-  TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream));
+  TFA_TRY(assemble_impl(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream, false));
   return jvp_core(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, v, out, eps, -1.0, stream);
 }
 
@@ -421,7 +428,7 @@ int tfa_gmres_jfnk(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const d
   if (ctx->jfnk0.n < n) TFA_CUDA(ctx->jfnk0.alloc(n));
   if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
   // the base residual and the state's size, once per solve
-  TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream));
+  TFA_TRY(assemble_impl(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream, false));
   Gm G{m, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
   TFA_TRY(G.dots(1, state, n, state));
   const double rms_state = std::sqrt(G.host[0] / (double)n);

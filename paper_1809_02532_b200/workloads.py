@@ -26,28 +26,54 @@ IB, IE, IPSI, IPHI, IRHOI, IRHOE, IUI, IUE, ITI, ITE = 0, 3, 6, 7, 8, 9, 10, 13,
 
 @dataclasses.dataclass
 class MeshInput:
-    """What ``tfa_mesh_create`` consumes: nodes, CCW triangles, per-cell corner coordinates."""
+    """What ``tfa_mesh_create`` / ``tfa_mesh_create_poly`` consume: nodes, counter-clockwise cells, per-cell corner
+    coordinates.  Triangle meshes: ``cell_nodes [nc][3]``, ``cell_xy [nc][3][2]``, ``cell_ptr`` None.  Mixed
+    triangle / quadrilateral meshes: ``cell_ptr [nc+1]`` and flat ``cell_nodes [cell_ptr[nc]]``,
+    ``cell_xy [cell_ptr[nc]][2]``."""
 
     node_xy: np.ndarray      # [nn][2] f64 (periodic images identified: one entry per topological node)
-    cell_nodes: np.ndarray   # [nc][3] i32, counter-clockwise
-    cell_xy: np.ndarray      # [nc][3][2] f64, each cell's own (unwrapped) corner coordinates
+    cell_nodes: np.ndarray   # i32, counter-clockwise
+    cell_xy: np.ndarray      # f64, each cell's own (unwrapped) corner coordinates
     name: str = ""
+    cell_ptr: np.ndarray | None = None
 
     @property
     def n_cells(self) -> int:
-        return int(self.cell_nodes.shape[0])
+        return int(self.cell_nodes.shape[0]) if self.cell_ptr is None else int(self.cell_ptr.shape[0] - 1)
 
     @property
     def n_nodes(self) -> int:
         return int(self.node_xy.shape[0])
 
     def centroids(self) -> np.ndarray:
-        return self.cell_xy.mean(axis=1)
+        """Where the initial states are sampled (S23): the area centroid of each cell (for a triangle, the mean
+        of its corners)."""
+        if self.cell_ptr is None:
+            return self.cell_xy.mean(axis=1)
+        cp = self.cell_ptr
+        out = np.empty((self.n_cells, 2))
+        for nv in np.unique(np.diff(cp)):
+            idx = np.nonzero(np.diff(cp) == nv)[0]
+            X = self.cell_xy[cp[idx][:, None] + np.arange(nv)[None, :]]      # [n][nv][2]
+            if nv == 3:
+                out[idx] = X.mean(axis=1)
+                continue
+            r = X - X[:, :1]
+            a, b = r[:, 1:-1], r[:, 2:]
+            cr = a[..., 0] * b[..., 1] - a[..., 1] * b[..., 0]               # twice the fan triangles' areas
+            out[idx] = X[:, 0] + (cr[..., None] * (a + b)).sum(axis=1) / (3.0 * cr.sum(axis=1)[:, None])
+        return out
 
     def permuted(self, perm_new_to_old: np.ndarray) -> "MeshInput":
         p = np.asarray(perm_new_to_old)
-        return MeshInput(self.node_xy, np.ascontiguousarray(self.cell_nodes[p]),
-                         np.ascontiguousarray(self.cell_xy[p]), self.name + "+perm")
+        if self.cell_ptr is None:
+            return MeshInput(self.node_xy, np.ascontiguousarray(self.cell_nodes[p]),
+                             np.ascontiguousarray(self.cell_xy[p]), self.name + "+perm")
+        cnt = np.diff(self.cell_ptr)[p]
+        cp = np.concatenate([[0], np.cumsum(cnt)]).astype(np.int32)
+        src = np.repeat(self.cell_ptr[:-1][p], cnt) + (np.arange(cp[-1]) - np.repeat(cp[:-1], cnt))
+        return MeshInput(self.node_xy, np.ascontiguousarray(self.cell_nodes[src]),
+                         np.ascontiguousarray(self.cell_xy[src]), self.name + "+perm", cp)
 
     def rotated(self, theta: float, origin=(0.0, 0.0)) -> "MeshInput":
         c, s = np.cos(theta), np.sin(theta)
@@ -55,7 +81,59 @@ class MeshInput:
         o = np.asarray(origin, dtype=np.float64)
         return MeshInput(np.ascontiguousarray((self.node_xy - o) @ R.T + o),
                          self.cell_nodes.copy(),
-                         np.ascontiguousarray((self.cell_xy - o) @ R.T + o), self.name + "+rot")
+                         np.ascontiguousarray((self.cell_xy - o) @ R.T + o), self.name + "+rot",
+                         None if self.cell_ptr is None else self.cell_ptr.copy())
+
+
+def quad_mesh(nx: int, ny: int, x0=0.0, x1=1.0, y0=0.0, y1=1.0, periodic_x=True, periodic_y=True,
+              jitter: float = 0.0, seed: int = 0, tri_every: int = 0) -> MeshInput:
+    """nx x ny quadrilaterals (the paper's Cartesian meshes, L433 "2N x N cells", L559 "512x512 elements").
+
+    ``jitter`` moves every topological node by ``jitter*h*U(-1,1)`` per axis (hull nodes of a non-periodic
+    direction stay on the hull), which makes the quadrilaterals general convex ones.  ``tri_every`` = k > 0 splits
+    every cell with (i + j) % k == 0 by its (i,j)->(i+1,j+1) diagonal into two triangles: a mixed mesh.  Periodic
+    directions identify nodes topologically; ``cell_xy`` keeps the unwrapped coordinates (S9).
+    """
+    nxn = nx if periodic_x else nx + 1
+    nyn = ny if periodic_y else ny + 1
+    hx, hy = (x1 - x0) / nx, (y1 - y0) / ny
+    jj, ii = np.meshgrid(np.arange(nyn), np.arange(nxn), indexing="ij")
+    shift = np.zeros((nyn, nxn, 2))
+    if jitter > 0:
+        rng = np.random.default_rng(seed)
+        shift = rng.uniform(-1.0, 1.0, size=(nyn, nxn, 2)) * np.array([hx, hy]) * jitter
+        if not periodic_x:
+            shift[:, 0, 0] = shift[:, -1, 0] = 0.0
+        if not periodic_y:
+            shift[0, :, 1] = shift[-1, :, 1] = 0.0
+    node_xy = (np.stack([x0 + ii * hx, y0 + jj * hy], axis=-1) + shift).reshape(-1, 2).astype(np.float64)
+    j, i = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    i, j = i.reshape(-1), j.reshape(-1)
+
+    def nid(a, b):
+        return (b % nyn) * nxn + (a % nxn)
+
+    def xy(a, b):    # unwrapped lattice position + the shift of the topological node
+        return np.stack([x0 + a * hx, y0 + b * hy], axis=-1) + shift[b % nyn, a % nxn]
+
+    corners = [(i, j), (i + 1, j), (i + 1, j + 1), (i, j + 1)]
+    qn = np.stack([nid(a, b) for a, b in corners], axis=-1).astype(np.int32)     # [n][4]
+    qx = np.stack([xy(a, b) for a, b in corners], axis=1)                         # [n][4][2]
+    if tri_every <= 0:
+        cp = (4 * np.arange(nx * ny + 1)).astype(np.int32)
+        return MeshInput(node_xy, np.ascontiguousarray(qn.reshape(-1)), np.ascontiguousarray(qx.reshape(-1, 2)),
+                         f"quad{nx}x{ny}", cp)
+    split = (i + j) % tri_every == 0
+    nodes, coords, counts = [], [], []
+    for c in range(nx * ny):
+        if split[c]:
+            for tri in ((0, 1, 2), (0, 2, 3)):
+                nodes.extend(qn[c, list(tri)]); coords.extend(qx[c, list(tri)]); counts.append(3)
+        else:
+            nodes.extend(qn[c]); coords.extend(qx[c]); counts.append(4)
+    cp = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    return MeshInput(node_xy, np.asarray(nodes, dtype=np.int32), np.asarray(coords, dtype=np.float64),
+                     f"mixed{nx}x{ny}", cp)
 
 
 def split_quad_mesh(nx: int, ny: int, x0=0.0, x1=1.0, y0=0.0, y1=1.0,
@@ -256,7 +334,9 @@ GEM_DOMAIN = (-12.8, 12.8, -6.4, 6.4)
 
 
 def make_workload(name: str, scale: float = 1.0) -> Workload:
-    """BASELINE.json configs by name: c1 c2 c3 c4a (random order) c4b (RCM) c5.
+    """BASELINE.json configs by name: c1 c2 c3 c4a (random order) c4b (RCM) c5; and the quadrilateral / mixed meshes
+    of SURVEY 8(f)1: q1 (512x512 periodic quads, double current sheet), q2 (256x128 periodic quads, wave), qm
+    (mixed triangles and jittered quadrilaterals, GEM).
 
     ``scale`` < 1 shrinks the lattice (linear factor) for tests that want the same recipe at a
     size the oracle finishes in seconds.
@@ -283,4 +363,16 @@ def make_workload(name: str, scale: float = 1.0) -> Workload:
         npx, npy = int(round(2000 * scale)) + 1, int(round(1000 * scale)) + 1
         m = delaunay_mesh(npx, npy, *GEM_DOMAIN, jitter=0.3, seed=3, shuffle_cells=False)
         return Workload(name, m, gem_state(m.centroids()), ph, 1e-3, 3, reorder="rcm", seed=3)
+    if name == "q1":   # the paper's second case on its own mesh (L559; Table 9): double current sheet, 512x512 quads
+        n = max(6, int(round(512 * scale)))
+        m = quad_mesh(n, n, -12.8, 12.8, -12.8, 12.8)
+        return Workload(name, m, gem_double_state(m.centroids()), ph, 1e-3, 10)
+    if name == "q2":   # the paper's first case on its own mesh (L433; Table 4): wave on 2N x N quads, N = 128
+        n = max(4, int(round(128 * scale)))
+        m = quad_mesh(2 * n, n, 0.0, 2.0, 0.0, 1.0)
+        return Workload(name, m, wave_state(m.centroids(), seed=5), ph, 1e-3, 10, seed=5)
+    if name == "qm":   # mixed mesh: jittered quads, every third one split into two triangles, boundaries in y
+        nx, ny = max(6, int(round(768 * scale))), max(6, int(round(384 * scale)))
+        m = quad_mesh(nx, ny, *GEM_DOMAIN, periodic_x=True, periodic_y=False, jitter=0.2, seed=6, tri_every=3)
+        return Workload(name, m, gem_state(m.centroids()), ph, 1e-3, 10, reorder="rcm", seed=6)
     raise ValueError(f"unknown workload {name!r}")

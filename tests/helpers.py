@@ -20,24 +20,31 @@ def read_golden_sections(name):
     return out
 
 
-def brute_connectivity(cell_nodes):
+def cells_as_lists(cell_nodes, cell_ptr=None):
+    """Corner lists of every cell: [nc][3] array, or flat array + CSR pointer for mixed meshes."""
+    if cell_ptr is None:
+        return [[int(x) for x in row] for row in cell_nodes]
+    return [[int(x) for x in cell_nodes[cell_ptr[c]:cell_ptr[c + 1]]] for c in range(len(cell_ptr) - 1)]
+
+
+def brute_connectivity(cell_nodes, cell_ptr=None):
     """O(n^2)-style set arithmetic, independent of the sort-based builders.
 
     Returns faces (sorted (lo,hi) -> [cells]), face-neighbour sets, vertex-neighbour sets.
     """
-    nc = len(cell_nodes)
+    cells = cells_as_lists(cell_nodes, cell_ptr)
+    nc = len(cells)
     edge_cells = {}
-    for c in range(nc):
-        a = [int(x) for x in cell_nodes[c]]
-        for k in range(3):
-            key = (min(a[k], a[(k + 1) % 3]), max(a[k], a[(k + 1) % 3]))
+    for c, a in enumerate(cells):
+        for k in range(len(a)):
+            key = (min(a[k], a[(k + 1) % len(a)]), max(a[k], a[(k + 1) % len(a)]))
             edge_cells.setdefault(key, []).append(c)
     faces = sorted(edge_cells.items())
     node_cells = {}
-    for c in range(nc):
-        for v in cell_nodes[c]:
-            node_cells.setdefault(int(v), set()).add(c)
-    vert_nb = [sorted(set().union(*[node_cells[int(v)] for v in cell_nodes[c]]) - {c}) for c in range(nc)]
+    for c, a in enumerate(cells):
+        for v in a:
+            node_cells.setdefault(v, set()).add(c)
+    vert_nb = [sorted(set().union(*[node_cells[v] for v in cells[c]]) - {c}) for c in range(nc)]
     face_nb = [set() for _ in range(nc)]
     for _, cs in faces:
         if len(cs) == 2:
@@ -46,21 +53,23 @@ def brute_connectivity(cell_nodes):
     return faces, face_nb, vert_nb
 
 
-def check_connectivity_against_brute(mesh_get, sizes, cell_nodes):
+def check_connectivity_against_brute(mesh_get, sizes, cell_nodes, cell_ptr=None):
     """mesh_get(name)->array, sizes=(nc,nf,nnzb,nst).  Bit-exact comparison with brute force."""
     nc, nf, nnzb, nst = sizes
-    faces, face_nb, vert_nb = brute_connectivity(cell_nodes)
+    cells = cells_as_lists(cell_nodes, cell_ptr)
+    faces, face_nb, vert_nb = brute_connectivity(cell_nodes, cell_ptr)
     assert nf == len(faces)
     fc = mesh_get("face_cells")
     exp_fc = np.array([[min(cs), max(cs) if len(cs) == 2 else -1] for _, cs in faces], dtype=np.int32)
     np.testing.assert_array_equal(fc, exp_fc)
     cf = mesh_get("cell_faces")
+    assert cf.shape == (nc, max(len(a) for a in cells))
     key_to_face = {k: i for i, (k, _) in enumerate(faces)}
-    for c in range(nc):
-        a = [int(x) for x in cell_nodes[c]]
-        for k in range(3):
-            key = (min(a[k], a[(k + 1) % 3]), max(a[k], a[(k + 1) % 3]))
+    for c, a in enumerate(cells):
+        for k in range(len(a)):
+            key = (min(a[k], a[(k + 1) % len(a)]), max(a[k], a[(k + 1) % len(a)]))
             assert cf[c, k] == key_to_face[key]
+        assert (cf[c, len(a):] == -1).all()
     sp, si = mesh_get("stencil_ptr"), mesh_get("stencil_idx")
     assert sp[0] == 0 and sp[-1] == nst == sum(len(v) for v in vert_nb)
     for c in range(nc):
@@ -118,11 +127,36 @@ def jacobian_error_rows(vals_rows, ref_rows):
     return float((diff / rowmax).max())
 
 
-def bsr_to_rows(vals, rowptr, rows=None):
-    """[nnzb][18][18] -> zero-padded [n_rows][4][18][18] (blocks in BSR order)."""
+def jacobian_error_blocks(vals, ref, rowptr):
+    """vals, ref: [nnzb][18][18] in the same BSR pattern.  Same measure as jacobian_error_rows (error relative to
+    the scalar row's largest |entry| over all blocks of the BSR row), vectorised for large meshes."""
+    n = len(rowptr) - 1
+    rows = np.repeat(np.arange(n), np.diff(rowptr))
+    diff = np.zeros((n, 18))
+    rowmax = np.zeros((n, 18))
+    np.maximum.at(diff, rows, np.abs(vals - ref).max(axis=2))
+    np.maximum.at(rowmax, rows, np.abs(ref).max(axis=2))
+    return float((diff / np.where(rowmax > 0, rowmax, 1.0)).max())
+
+
+def jacobian_error_padded(vals, ref_rows, rowptr):
+    """vals: [nblk][18][18], the blocks of consecutive BSR rows (rowptr relative to the first of them);
+    ref_rows: the oracle's zero-padded [n_rows][B][18][18] for the same rows."""
+    n = len(rowptr) - 1
+    cnt = np.diff(rowptr)
+    rows = np.repeat(np.arange(n), cnt)
+    slot = np.arange(len(rows)) - np.repeat(rowptr[:-1], cnt)
+    ref = ref_rows[rows, slot]
+    assert not ref_rows[np.arange(ref_rows.shape[1])[None, :] >= cnt[:, None]].any(), "padding blocks must be zero"
+    return jacobian_error_blocks(vals, ref, rowptr)
+
+
+def bsr_to_rows(vals, rowptr, rows=None, width=None):
+    """[nnzb][18][18] -> zero-padded [n_rows][width][18][18] (blocks in BSR order; width = the longest row)."""
     n = len(rowptr) - 1
     rows = np.arange(n) if rows is None else np.asarray(rows)
-    out = np.zeros((len(rows), 4, 18, 18))
+    width = max(4, int(np.diff(rowptr).max())) if width is None else width
+    out = np.zeros((len(rows), width, 18, 18))
     for q, i in enumerate(rows):
         b, e = rowptr[i], rowptr[i + 1]
         out[q, :e - b] = vals[b:e]

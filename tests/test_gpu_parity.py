@@ -7,8 +7,8 @@ import numpy as np
 import pytest
 
 from conftest import random_state, rot18
-from helpers import (RES_TOL, JAC_TOL, residual_error, jacobian_error_rows, bsr_to_rows,
-                     check_connectivity_against_brute)
+from helpers import (RES_TOL, JAC_TOL, residual_error, jacobian_error_rows, jacobian_error_blocks,
+                     jacobian_error_padded, bsr_to_rows, check_connectivity_against_brute)
 
 pytestmark = pytest.mark.gpu
 
@@ -304,6 +304,29 @@ def test_run_to_run_determinism_and_no_memset_needed(api, orc, W):
     assert ctx.launches_per_assemble == 2
 
 
+def test_context_workspace_follows_the_mesh_not_its_address(api, orc, W):
+    """One context used on mesh A, A destroyed, then on a larger mesh B (which the allocator may well place at A's
+    address): the per-mesh workspace (least-squares coefficients, face-state buffer) must be rebuilt for B."""
+    ctx = api.Context()
+    for trial in range(4):                           # several rounds make an address reuse near certain
+        a = W.split_quad_mesh(4 + trial, 4)
+        ga = api.Mesh.from_input(a)
+        ctx.assemble(ga, dev(W.wave_state(a.centroids(), seed=1)))
+        ctx.check()
+        ga.close()
+        del ga
+        b = W.delaunay_mesh(23, 17, *W.GEM_DOMAIN, jitter=0.3, seed=4 + trial, shuffle_cells=True)
+        gb, ob = api.Mesh.from_input(b), orc.OracleMesh.from_input(b)
+        P = W.gem_state(b.centroids()) + np.random.default_rng(trial).uniform(-1e-3, 1e-3, (b.n_cells, 18))
+        rhs, vals = ctx.assemble(gb, dev(P))
+        ctx.check()
+        ph_o = orc.physics_c()
+        rhs_o, sc_o, vals_o = orc.assemble(ob, ph_o, orc.default_numerics(ph_o), P)
+        assert residual_error(rhs.cpu().numpy(), rhs_o, sc_o) < RES_TOL
+        assert jacobian_error_blocks(vals.cpu().numpy(), vals_o, gb.get("bsr_rowptr")) < JAC_TOL
+        gb.close()
+
+
 def test_host_entry_point_matches_device_entry_point(api, W):
     import torch
     mi = small_meshes(W)["channel"]
@@ -333,9 +356,10 @@ def test_nonphysical_state_is_reported(api, W):
 
 
 def test_config2_first_and_last_of_ten_calls(api, orc, W):
-    """BASELINE config 2 at a size the oracle finishes in seconds (64x64 quads = 8192 cells):
-    10 consecutive assemblies with the state perturbed by 1e-6 between calls; parity on 1st and 10th."""
-    w = W.make_workload("c2", scale=0.25)
+    """BASELINE config 2 at its full size (256x256 quads split = 131 072 cells): 10 consecutive assemblies with
+    the state perturbed by 1e-6 between calls; every row of the 1st and of the 10th call against the oracle."""
+    w = W.make_workload("c2")
+    assert w.mesh.n_cells == 131072
     g, o = api.Mesh.from_input(w.mesh), orc.OracleMesh.from_input(w.mesh)
     ctx = api.Context(w.physics)
     ph_o = orc.physics_c(w.physics)
@@ -347,18 +371,26 @@ def test_config2_first_and_last_of_ten_calls(api, orc, W):
         if call in (0, 9):
             rhs_o, sc_o, vals_o = orc.assemble(o, ph_o, nu_o, P, P_prev, P_prev2, w.dt)
             er = residual_error(rhs.cpu().numpy(), rhs_o, sc_o)
-            ej = jacobian_error_rows(bsr_to_rows(vals.cpu().numpy(), rp), bsr_to_rows(vals_o, rp))
+            ej = jacobian_error_blocks(vals.cpu().numpy(), vals_o, rp)
             assert er < RES_TOL and ej < JAC_TOL, (call, er, ej)
         P_prev2, P_prev, P = P_prev, P, W.perturb(P, 100 + call, 1e-6)
     ctx.check()
 
 
+SWEEP_CHUNK = 100_000
+RES_TOL_CANCELLING = 1e-10   # mass / energy rows against the flux + source scale (derivation in the test)
+
+
 @pytest.mark.parametrize("name", ["c2", "c3", "c4a", "c4b", "c5"])
-def test_full_size_sampled_rows(api, orc, W, name):
-    """BASELINE configs 2-5 at their full sizes, in the launch configuration bench.py times (device
-    buffers, RCM where the config says so): rhs and whole BSR rows of a seeded row sample (plus the first
-    and the last tile of the mesh) against the oracle's row-subset mode; pattern compared bit-exactly on
-    the sample; every entry of the value array written (NaN canary)."""
+def test_full_size_every_row(api, orc, W, name):
+    """BASELINE configs 2-5 at their full sizes, in the launch configuration bench.py times (device buffers,
+    RCM where the config says so): EVERY row of rhs and of the BSR Jacobian against the oracle, swept in chunks
+    of 100 000 consecutive rows (oracle row-subset mode; the GPU's value array is sliced per chunk), so that
+    every persistent CTA, both stages of the input pipeline and the tail tile are covered.  The pattern is
+    compared bit-exactly over the whole mesh; every entry of the value array must have been written (NaN canary).
+    The residual is held to 1e-12 of the full sum-of-|terms| scale (S18), and -- with the BDF2 term masked out of
+    both sides, term_mask = 3 -- to the flux + source scale alone, which in these configurations
+    (P^n = P^{n-1} = P) is up to 1e3 times smaller for the density and energy rows (bars at the end)."""
     import torch
     w = W.make_workload(name)
     g, o = api.Mesh.from_input(w.mesh), orc.OracleMesh.from_input(w.mesh)
@@ -369,32 +401,48 @@ def test_full_size_sampled_rows(api, orc, W, name):
     assert np.array_equal(perm, o.get("perm"))
     P = np.ascontiguousarray(w.state[perm])
     nc = g.n_cells
-    rng = np.random.default_rng(77)
-    rows = np.unique(np.concatenate([rng.choice(nc, size=3000, replace=False), np.arange(25), np.arange(nc - 25, nc)]))
-    rows = rows.astype(np.int32)
+    rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
+    assert np.array_equal(rp, o.get("bsr_rowptr")) and np.array_equal(col, o.get("bsr_col"))
     ctx = api.Context(w.physics)
-    rhs = torch.empty((nc, 18), dtype=torch.float64, device="cuda")
+    Pd = dev(P)
+    rhs = torch.full((nc, 18), float("nan"), dtype=torch.float64, device="cuda")
     vals = torch.full((g.nnzb, 18, 18), float("nan"), dtype=torch.float64, device="cuda")
-    ctx.assemble(g, dev(P), dt=w.dt, rhs=rhs, vals=vals)
+    ctx.assemble(g, Pd, dt=w.dt, rhs=rhs, vals=vals)
     ctx.check()
     assert not bool(torch.isnan(vals).any()), "an entry of the BSR value array was not written"
-    rp, rp_o = g.get("bsr_rowptr"), o.get("bsr_rowptr")
-    col, col_o = g.get("bsr_col"), o.get("bsr_col")
-    assert np.array_equal(rp, rp_o)
-    blk = np.concatenate([np.arange(rp[i], rp[i + 1]) for i in rows])
-    assert np.array_equal(col[blk], col_o[blk])
-    vals_s = vals[torch.from_numpy(blk).cuda()].cpu().numpy()
-    got = np.zeros((len(rows), 4, 18, 18))
-    q = 0
-    for r, i in enumerate(rows):
-        n = rp[i + 1] - rp[i]
-        got[r, :n] = vals_s[q:q + n]
-        q += n
+    assert not bool(torch.isnan(rhs).any())
+    # flux + source only (residual-only kernel and Jacobian kernel), for the second residual bar
+    nu3 = api.default_numerics(ctx.physics, term_mask=3)
+    ctx3 = api.Context(w.physics, nu3)
+    rhs3, _ = ctx3.assemble(g, Pd, dt=w.dt, jacobian=False)
+    ctx3.check()
+    rhs_h, rhs3_h = rhs.cpu().numpy(), rhs3.cpu().numpy()
     ph_o = orc.physics_c(w.physics)
-    rhs_o, sc_o, vals_o = orc.assemble(o, ph_o, orc.default_numerics(ph_o), P, dt=w.dt, rows=rows)
-    er = residual_error(rhs[torch.from_numpy(rows.astype(np.int64)).cuda()].cpu().numpy(), rhs_o, sc_o)
-    ej = jacobian_error_rows(got, vals_o)
+    nu_o, nu3_o = orc.default_numerics(ph_o), orc.default_numerics(ph_o, term_mask=3)
+    num = np.zeros(18); den = np.zeros(18); num3 = np.zeros(18); den3 = np.zeros(18)
+    ej = 0.0
+    for r0 in range(0, nc, SWEEP_CHUNK):
+        r1 = min(nc, r0 + SWEEP_CHUNK)
+        rows = np.arange(r0, r1, dtype=np.int32)
+        rhs_o, sc_o, vals_o = orc.assemble(o, ph_o, nu_o, P, dt=w.dt, rows=rows)
+        got = vals[int(rp[r0]):int(rp[r1])].cpu().numpy()
+        ej = max(ej, jacobian_error_padded(got, vals_o, rp[r0:r1 + 1] - rp[r0]))
+        num = np.maximum(num, np.abs(rhs_h[r0:r1] - rhs_o).max(axis=0))
+        den = np.maximum(den, sc_o.max(axis=0))
+        rhs3_o, sc3_o, _ = orc.assemble(o, ph_o, nu3_o, P, dt=w.dt, rows=rows, jacobian=False)
+        num3 = np.maximum(num3, np.abs(rhs3_h[r0:r1] - rhs3_o).max(axis=0))
+        den3 = np.maximum(den3, sc3_o.max(axis=0))
+    er = float((num / np.where(den > 0, den, 1.0)).max())
+    e3 = num3 / np.where(den3 > 0, den3, 1.0)
     assert er < RES_TOL and ej < JAC_TOL, (name, er, ej)
+    # Flux + source scale: the field and momentum rows meet 1e-12 of it.  The mass and energy rows (8, 9, 16, 17)
+    # carry mdot (1, H); in the GEM configurations u_s.n = 0 on every face, so mdot is the pressure-diffusion
+    # term alone, proportional to p_R - p_L: a difference of two nearly equal face pressures, whose rounding
+    # (2^-53 p from the reconstruction) is amplified by p / |p_R - p_L| ~ 1e4..1e5 on these meshes.  That is the
+    # conditioning of the term itself (both sides compute it in the same order), so those rows are held to 1e-10.
+    cancelling = np.zeros(18, dtype=bool)
+    cancelling[[8, 9, 16, 17]] = True
+    assert e3[~cancelling].max() < RES_TOL and e3[cancelling].max() < RES_TOL_CANCELLING, (name, e3)
 
 
 def test_flux_sqrt_and_reciprocal_error_bound(api):

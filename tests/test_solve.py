@@ -201,11 +201,43 @@ def test_gmres_edge_cases(system):
     xs, it1, rel1 = ctx.gmres(g, vals, b, dinv=ctx.block_jacobi(g, vals), rtol=1e-9)
     x2, it2, rel2 = ctx.gmres(g, vals, b, x=xs.clone(), dinv=ctx.block_jacobi(g, vals), rtol=1e-9)
     assert it2 == 0 and rel2 == pytest.approx(rel1)
+    # singular operator (A = 0): the Hessenberg column vanishes -> TFA_ESINGULAR, x left at the initial guess
+    x0 = torch.full((n,), 0.5, dtype=torch.float64, device="cuda")
+    with pytest.raises(api.TfaError) as e:
+        ctx.gmres(g, torch.zeros_like(vals), b, x=x0)
+    assert e.value.code == -6 and float((x0 - 0.5).abs().max()) == 0.0
+    # NaN in the matrix: reported, not returned as success
+    bad = vals.clone()
+    bad[0, 0, 0] = float("nan")
+    with pytest.raises(api.TfaError) as e:
+        ctx.gmres(g, bad, b)
+    assert e.value.code == -6
 
 
 # ---------------------------------------------------------------------------------------------------
 # matrix-free operator
 # ---------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+def test_jfnk_solve_with_kernel_timing_enabled(W):
+    """A matrix-free solve applies the operator more often than the timing ring of tfa_assemble has slots (64);
+    the operator's evaluations are untimed, so the solve must not fail on it."""
+    import torch
+    from paper_1809_02532_b200 import api
+    m = W.split_quad_mesh(12, 8)
+    P = torch.from_numpy(W.wave_state(m.centroids(), seed=7)).cuda()
+    g = api.Mesh.from_input(m)
+    ctx = api.Context()
+    rhs, vals = ctx.assemble(g, P, dt=0.05)
+    dinv = ctx.block_jacobi(g, vals)
+    ctx.timing_enable(True)
+    x, it, rel = ctx.gmres_jfnk(g, P, rhs.reshape(-1).contiguous(), dt=0.05, restart=20, max_iters=90, rtol=1e-30)
+    assert it == 90                                   # 90 operator applications > 64 ring slots
+    ctx.assemble(g, P, dt=0.05)
+    assert ctx.timing_read()[2] == 1                  # only the explicit assembly was timed
+    ctx.timing_enable(False)
+    ctx.check()
+
+
 def _wave_case(W, orc):
     m = W.split_quad_mesh(12, 8)
     P = W.wave_state(m.centroids(), seed=7)
