@@ -2,7 +2,8 @@
  *
  * What it computes: one Newton-step assembly of the implicit ideal two-fluid (ion + electron +
  * full Maxwell with hyperbolic divergence cleaning) finite-volume method of arXiv 1809.02532 on
- * an unstructured 2-D triangle mesh with 18 FP64 unknowns per cell: the pseudo-steady residual
+ * an unstructured 2-D mesh of triangles and convex quadrilaterals (mixed freely; the paper's own meshes are
+ * Cartesian quadrilaterals, L433, L559) with 18 FP64 unknowns per cell: the pseudo-steady residual
  * R~ (Eq. 13) and its block Jacobian dR~/dP (Eq. 14; computed numerically,
  * L130, by the perturbation loop of Algorithm 1) in 18x18 BSR form, ready for an
  * external Krylov solver.  "L<n>" cites a line of the paper text; "S<n>" a reading in DESIGN.md.
@@ -69,7 +70,8 @@ typedef struct tfa_ctx tfa_ctx;
 /* items for tfa_mesh_get / tfa_mesh_device_ptr */
 enum {
   TFA_FACE_CELLS = 0,      /* int32 [n_faces][2]: (L, R) with L < R, R = -1 on the boundary (S10) */
-  TFA_CELL_FACES = 1,      /* int32 [n_cells][3]: face of local edge k = (node k -> node k+1) */
+  TFA_CELL_FACES = 1,      /* int32 [n_cells][F]: face of local edge k = (node k -> node k+1); F = max_faces of
+                              tfa_mesh_info (3 or 4); -1 in the fourth slot of a triangle of a mixed mesh */
   TFA_STENCIL_PTR = 2,     /* int32 [n_cells+1]: CSR of the face-vertex neighbour stencil (L74) */
   TFA_STENCIL_IDX = 3,     /* int32 [n_stencil]: ascending, unique, without the cell itself */
   TFA_BSR_ROWPTR = 4,      /* int32 [n_cells+1] */
@@ -79,7 +81,22 @@ enum {
   TFA_FACE_NORMAL_LEN = 8, /* f64 [n_faces][3]: unit normal (L -> R) and length Sigma_f */
   TFA_CENTROID = 9,        /* f64 [n_cells][2] (in the cell's own, unwrapped frame) */
   TFA_FACE_NODES = 10,     /* int32 [n_faces][2]: (lo, hi) node ids; faces are sorted by this key */
-  TFA_CELL_NBR = 11        /* int32 [n_cells][3]: neighbour across local edge k, -1 on the boundary */
+  TFA_CELL_NBR = 11,       /* int32 [n_cells][F]: neighbour across local edge k, -1 on the boundary / no such edge */
+  TFA_BFACES = 12,         /* int32 [n_bfaces]: the boundary faces (R = -1) in ascending face id; faces are numbered by
+                              their node pair, so this list and the tags attached to it survive tfa_mesh_reorder */
+  TFA_BC_TAGS = 13         /* int32 [n_bfaces]: TFA_BC_* of each boundary face */
+};
+
+/* Rule for the far side P_R of a boundary face (the paper's separate boundary loop, L260; readings S9, S24).
+ * Periodic boundaries are not a tag: periodic images are identified topologically in cell_nodes (S9). */
+enum {
+  TFA_BC_TRANSMISSIVE = 0, /* P_R := P_L; the perturbations of the Jacobian move both arguments (default) */
+  TFA_BC_GHOST = 1,        /* P_R := the caller's ghost state of that face (tfa_set_ghost_states), held fixed while
+                              P_L is perturbed: Dirichlet / far-field data, or whatever a host loop over the boundary
+                              faces (L260) wrote there before the call */
+  TFA_BC_WALL = 2          /* P_R := mirror image of P_L: perfectly conducting slip wall, B.n = 0, E_t = 0, u_s.n = 0
+                              at the face (B and u_s flip their normal component, E its tangential ones, Phi flips,
+                              Psi, rho_s, T_s are kept; S24); moves with P_L */
 };
 
 /* ---- step a1: connectivity, geometry, stencil, BSR pattern (L74, L230, L276-319 Listing 1) ----
@@ -91,6 +108,17 @@ enum {
  * itself or reaches one neighbour through two faces (periodic direction narrower than 3 cells). */
 int tfa_mesh_create(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
                     const int32_t* cell_nodes, const double* cell_xy, void* stream);
+/* Mixed mesh of triangles and convex quadrilaterals: the corners of cell i are
+ * cell_nodes[cell_ptr[i] .. cell_ptr[i+1]) (3 or 4 of them, counter-clockwise), cell_xy [cell_ptr[n_cells]][2] in the
+ * same layout (or NULL).  HOST pointers, copied.  A quadrilateral has 5 BSR blocks in its row.  TFA_EMESH also for a
+ * non-convex quadrilateral; TFA_EINVAL for a cell with another number of corners.
+ * Limit of both builders: the cells around the corners of one cell (with repetitions) may not exceed 192. */
+int tfa_mesh_create_poly(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
+                         const int32_t* cell_ptr, const int32_t* cell_nodes, const double* cell_xy, void* stream);
+/* max_faces: 3 for a pure triangle mesh, else 4; n_bfaces: number of boundary faces. */
+int tfa_mesh_info(const tfa_mesh* m, int32_t* max_faces, int64_t* n_bfaces);
+/* Boundary rule of every boundary face: tags [n_bfaces] (HOST pointer, copied) in the order of TFA_BFACES. */
+int tfa_mesh_set_bc(tfa_mesh* m, const int32_t* tags, void* stream);
 /* Renumber the cells for locality and rebuild every derived array under the same rules.
  * kind 0: none; 1: reverse Cuthill-McKee on the face-neighbour graph, computed on the device
  * (S11: start = unvisited cell of minimum (degree, id); neighbours appended by (degree, id));
@@ -98,7 +126,8 @@ int tfa_mesh_create(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int6
 int tfa_mesh_reorder(tfa_mesh* m, int kind, const int32_t* user_perm, void* stream);
 int tfa_mesh_sizes(const tfa_mesh* m, int64_t* n_cells, int64_t* n_faces, int64_t* nnzb,
                    int64_t* n_stencil);
-/* Copy one item to host memory; `bytes` must equal the item's size. */
+/* Copy one item to host memory; `bytes` must equal the item's size.  Blocking: it synchronises the device (the
+ * two derived items TFA_VOLUME and TFA_FACE_NORMAL_LEN run a small kernel on the default stream first). */
 int tfa_mesh_get(const tfa_mesh* m, int which, void* host_dst, int64_t bytes);
 /* Device pointer of an int32 pattern item (TFA_BSR_ROWPTR, TFA_BSR_COL, TFA_PERM, ...) for the
  * solver hand-over (zero copy, as Listing 3); valid until destroy/reorder. */
@@ -111,6 +140,12 @@ void tfa_default_numerics(tfa_numerics* n, const tfa_physics* p);
 int  tfa_ctx_create(tfa_ctx** out);
 int  tfa_set_physics(tfa_ctx* ctx, const tfa_physics* p);
 int  tfa_set_numerics(tfa_ctx* ctx, const tfa_numerics* n);
+/* Ghost states of the TFA_BC_GHOST faces: ghost [n_bfaces][18] FP64, DEVICE pointer in the order of TFA_BFACES,
+ * owned by the caller and read (not copied) by every later assembly of this context until replaced; rows of
+ * faces with another tag are ignored.  NULL forgets it.  An assembly on a mesh with TFA_BC_GHOST faces and no
+ * (or a wrongly sized) ghost array returns TFA_EINVAL. */
+int  tfa_set_ghost_states(tfa_ctx* ctx, const double* ghost, int64_t n_bfaces);
+/* A context holds the workspace of one assembly at a time: use it from one thread and one stream at a time. */
 void tfa_ctx_destroy(tfa_ctx* ctx);
 
 /* ---- step a2 (test hook): least-squares gradient (L74) and Venkatakrishnan limiter (L208) ----
@@ -160,13 +195,17 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
  * with Givens rotations (each iteration synchronises the stream).  Stops when the true residual norm
  * ||b - A x|| <= rtol * ||b|| (checked at every restart; the recurrence's estimate ends a cycle) or after
  * max_iters iterations.  info[0] = iterations done, info[1] = ||b - A x|| / ||b|| on return.
- * The Krylov basis ((restart + 2) vectors) lives in the context's workspace. */
+ * The Krylov basis ((restart + 2) vectors) lives in the context's workspace.
+ * TFA_ESINGULAR: a residual norm or Krylov vector is not finite, or the Hessenberg column vanished (singular
+ * operator); x then holds the last completed cycle's iterate. */
 int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
               double* x, int restart, int max_iters, double rtol, double* info, void* stream);
 
 /* ---- matrix-free operator (the paper's future work, L130): out = (dR~/dP) v by a forward
  * difference of the residual-only assembly, (R~(P + eps v) - R~(P)) / eps — the full dependence, gradient and
- * limiter included (the assembled Jacobian freezes them, S8).  eps <= 0: eps = 1e-7 (1 + rms(P)) / rms(v).
+ * limiter included (the assembled Jacobian freezes them, S8): NOT the same linearisation as bsr_vals; where the
+ * limiter is active its min/max make the residual non-smooth and the difference quotient noisy.
+ * eps <= 0: eps = 1e-7 (1 + rms(P)) / rms(v).
  * DEVICE pointers; synchronises the stream when eps is chosen automatically. */
 int tfa_jvp(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n, const double* state_nm1,
             double dt, const double* v, double* out, double eps, void* stream);
@@ -181,7 +220,8 @@ int tfa_gmres_jfnk(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const d
  * its two kernels and accumulates their durations at the next tfa_timing_read, which
  * synchronises on the last event, writes the accumulated milliseconds since the previous read
  * to ms[0] (gradient + limiter kernel) and ms[1] (assembly kernel), the number of assemblies
- * to *n_calls, and resets the accumulators.  At most 64 assemblies may be outstanding. */
+ * to *n_calls, and resets the accumulators.  At most 64 assemblies may be outstanding (the residual evaluations
+ * inside tfa_jvp / tfa_gmres_jfnk are not timed and do not count). */
 int tfa_timing_enable(tfa_ctx* ctx, int on);
 int tfa_timing_read(tfa_ctx* ctx, double* ms /*[2]*/, int* n_calls);
 

@@ -34,6 +34,9 @@ class Numerics(C.Structure):
 _vp, _i64, _dbl, _int = C.c_void_p, C.c_int64, C.c_double, C.c_int
 SYMBOLS = {
     "tfa_mesh_create": (_int, [C.POINTER(_vp), _i64, _vp, _i64, _vp, _vp, _vp]),
+    "tfa_mesh_create_poly": (_int, [C.POINTER(_vp), _i64, _vp, _i64, _vp, _vp, _vp, _vp]),
+    "tfa_mesh_info": (_int, [_vp, C.POINTER(C.c_int32), C.POINTER(_i64)]),
+    "tfa_mesh_set_bc": (_int, [_vp, _vp, _vp]),
     "tfa_mesh_reorder": (_int, [_vp, _int, _vp, _vp]),
     "tfa_mesh_sizes": (_int, [_vp] + [C.POINTER(_i64)] * 4),
     "tfa_mesh_get": (_int, [_vp, _int, _vp, _i64]),
@@ -44,6 +47,7 @@ SYMBOLS = {
     "tfa_ctx_create": (_int, [C.POINTER(_vp)]),
     "tfa_set_physics": (_int, [_vp, C.POINTER(Physics)]),
     "tfa_set_numerics": (_int, [_vp, C.POINTER(Numerics)]),
+    "tfa_set_ghost_states": (_int, [_vp, _vp, _i64]),
     "tfa_ctx_destroy": (None, [_vp]),
     "tfa_gradients": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "tfa_assemble": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),

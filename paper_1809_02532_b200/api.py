@@ -17,8 +17,10 @@ from ._lib import NEQ, BLOCK, Physics, Numerics, TfaError  # noqa: F401
 MESH_ITEMS = dict(face_cells=(0, np.int32), cell_faces=(1, np.int32), stencil_ptr=(2, np.int32),
                   stencil_idx=(3, np.int32), bsr_rowptr=(4, np.int32), bsr_col=(5, np.int32),
                   perm=(6, np.int32), volume=(7, np.float64), face_normal_len=(8, np.float64),
-                  centroid=(9, np.float64), face_nodes=(10, np.int32), cell_nbr=(11, np.int32))
+                  centroid=(9, np.float64), face_nodes=(10, np.int32), cell_nbr=(11, np.int32),
+                  bfaces=(12, np.int32), bc_tags=(13, np.int32))
 _REORDER = {"none": 0, "rcm": 1, "user": 2}
+BC_TRANSMISSIVE, BC_GHOST, BC_WALL = 0, 1, 2
 
 
 def _stream() -> int:
@@ -63,24 +65,41 @@ def default_numerics(ph: Physics | None = None, **over) -> Numerics:
 class Mesh:
     """Owner of a ``tfa_mesh*`` (tfa_mesh_create / tfa_mesh_destroy)."""
 
-    def __init__(self, node_xy, cell_nodes, cell_xy=None):
+    def __init__(self, node_xy, cell_nodes, cell_xy=None, cell_ptr=None):
+        """Triangles: cell_nodes [nc][3] (tfa_mesh_create).  Mixed triangles / quadrilaterals: cell_ptr [nc+1] and
+        flat cell_nodes, cell_xy [cell_ptr[nc]][2] (tfa_mesh_create_poly)."""
         lib = _lib.load()
         self._h = C.c_void_p()
         node_xy = np.ascontiguousarray(node_xy, dtype=np.float64)
         cell_nodes = np.ascontiguousarray(cell_nodes, dtype=np.int32)
         cxy = None if cell_xy is None else np.ascontiguousarray(cell_xy, dtype=np.float64)
-        _lib.check(lib.tfa_mesh_create(C.byref(self._h), node_xy.shape[0], _hp(node_xy), cell_nodes.shape[0],
-                                       _hp(cell_nodes), _hp(cxy), _stream()))
+        if cell_ptr is None:
+            _lib.check(lib.tfa_mesh_create(C.byref(self._h), node_xy.shape[0], _hp(node_xy), cell_nodes.shape[0],
+                                           _hp(cell_nodes), _hp(cxy), _stream()))
+        else:
+            cp = np.ascontiguousarray(cell_ptr, dtype=np.int32)
+            _lib.check(lib.tfa_mesh_create_poly(C.byref(self._h), node_xy.shape[0], _hp(node_xy), cp.shape[0] - 1,
+                                                _hp(cp), _hp(cell_nodes), _hp(cxy), _stream()))
         self._sizes()
 
     @classmethod
     def from_input(cls, mi) -> "Mesh":
-        return cls(mi.node_xy, mi.cell_nodes, mi.cell_xy)
+        return cls(mi.node_xy, mi.cell_nodes, mi.cell_xy, getattr(mi, "cell_ptr", None))
 
     def _sizes(self):
         v = [C.c_int64() for _ in range(4)]
         _lib.check(_lib.load().tfa_mesh_sizes(self._h, *[C.byref(x) for x in v]))
         self.n_cells, self.n_faces, self.nnzb, self.n_stencil = [int(x.value) for x in v]
+        mf, nb = C.c_int32(), C.c_int64()
+        _lib.check(_lib.load().tfa_mesh_info(self._h, C.byref(mf), C.byref(nb)))
+        self.max_faces, self.n_bfaces = int(mf.value), int(nb.value)
+
+    def set_bc(self, tags):
+        """tfa_mesh_set_bc: tags [n_bfaces] (BC_*) in the order of get("bfaces")."""
+        tags = np.ascontiguousarray(tags, dtype=np.int32)
+        if tags.shape != (self.n_bfaces,):
+            raise ValueError("one tag per boundary face")
+        _lib.check(_lib.load().tfa_mesh_set_bc(self._h, _hp(tags), _stream()))
 
     def reorder(self, kind: str = "rcm", perm=None):
         pp = None if perm is None else np.ascontiguousarray(perm, dtype=np.int32)
@@ -89,13 +108,15 @@ class Mesh:
 
     def get(self, name: str) -> np.ndarray:
         which, dt = MESH_ITEMS[name]
-        n = dict(face_cells=2 * self.n_faces, face_nodes=2 * self.n_faces, cell_faces=3 * self.n_cells,
-                 cell_nbr=3 * self.n_cells, stencil_ptr=self.n_cells + 1, stencil_idx=self.n_stencil,
+        F = self.max_faces
+        n = dict(face_cells=2 * self.n_faces, face_nodes=2 * self.n_faces, cell_faces=F * self.n_cells,
+                 cell_nbr=F * self.n_cells, stencil_ptr=self.n_cells + 1, stencil_idx=self.n_stencil,
                  bsr_rowptr=self.n_cells + 1, bsr_col=self.nnzb, perm=self.n_cells, volume=self.n_cells,
-                 face_normal_len=3 * self.n_faces, centroid=2 * self.n_cells)[name]
+                 face_normal_len=3 * self.n_faces, centroid=2 * self.n_cells, bfaces=self.n_bfaces,
+                 bc_tags=self.n_bfaces)[name]
         out = np.empty(n, dtype=dt)
         _lib.check(_lib.load().tfa_mesh_get(self._h, which, _hp(out), out.nbytes))
-        shape = dict(face_cells=(-1, 2), face_nodes=(-1, 2), cell_faces=(-1, 3), cell_nbr=(-1, 3),
+        shape = dict(face_cells=(-1, 2), face_nodes=(-1, 2), cell_faces=(-1, F), cell_nbr=(-1, F),
                      face_normal_len=(-1, 3), centroid=(-1, 2)).get(name)
         return out.reshape(shape) if shape else out
 
@@ -131,6 +152,13 @@ class Context:
     def set_numerics(self, n: Numerics):
         _lib.check(_lib.load().tfa_set_numerics(self._h, C.byref(n)))
         self.numerics = n
+
+    def set_ghost_states(self, ghost: torch.Tensor | None):
+        """tfa_set_ghost_states: ghost [n_bfaces][18] device tensor, read (not copied) by later assemblies; the
+        binding keeps a reference so that it stays alive."""
+        self._ghost = ghost
+        n = 0 if ghost is None else ghost.shape[0]
+        _lib.check(_lib.load().tfa_set_ghost_states(self._h, _dp(ghost), n))
 
     def gradients(self, mesh: Mesh, state: torch.Tensor):
         grad = torch.empty((mesh.n_cells, NEQ, 2), dtype=torch.float64, device=state.device)
@@ -262,6 +290,18 @@ def bsr_spmv(mesh: Mesh, vals: torch.Tensor, x: torch.Tensor, y: torch.Tensor | 
 # C-style aliases, same names as the ABI
 def mesh_create(node_xy, cell_nodes, cell_xy=None) -> Mesh:
     return Mesh(node_xy, cell_nodes, cell_xy)
+
+
+def mesh_create_poly(node_xy, cell_ptr, cell_nodes, cell_xy=None) -> Mesh:
+    return Mesh(node_xy, cell_nodes, cell_xy, cell_ptr)
+
+
+def mesh_set_bc(mesh: Mesh, tags):
+    mesh.set_bc(tags)
+
+
+def set_ghost_states(ctx: Context, ghost):
+    ctx.set_ghost_states(ghost)
 
 
 def mesh_reorder(mesh: Mesh, kind="rcm", perm=None):

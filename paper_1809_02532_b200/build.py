@@ -2,8 +2,10 @@
 
     python -m paper_1809_02532_b200.build [--force] [--verbose]
 
-nvcc cross-compiles without a GPU.  No fast-math: FP64 parity with the oracle relies on IEEE
-division and square root; FMA contraction is left on.
+nvcc cross-compiles without a GPU.  No --use_fast_math; FMA contraction is left on.
+The one deliberate departure from IEEE sequences is local: the AUSM flux takes its square roots and reciprocals
+from a single-precision seed refined by Newton steps in FP64 (TFA_FAST_MATH64 = 1 in csrc/tfa_physics.cuh, error
+below 1 ulp for arguments in the normal single-precision range; tests bound it through tfa_probe_math).
 """
 from __future__ import annotations
 

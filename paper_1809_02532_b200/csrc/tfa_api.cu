@@ -9,8 +9,8 @@ int launch_lsq_coef(const tfa_mesh& m, double power, double* coef, cudaStream_t 
 int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* fown,
                     double* grad, double* phi, cudaStream_t st);
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-                    const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
-                    int32_t* flags, int* resident_ctas, cudaStream_t st);
+                    const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs,
+                    double* vals, int32_t* flags, int* resident_ctas, cudaStream_t st);
 int launch_probe_dfma(int grid, int iters, double* sink, cudaStream_t st);
 int launch_probe_copy(const double* src, double* dst, int64_t n, cudaStream_t st);
 int launch_probe_math(const double* x, double* s, double* r, int64_t n, cudaStream_t st);
@@ -24,11 +24,11 @@ int prepare(tfa_ctx* ctx, const tfa_mesh* m, cudaStream_t st) {
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
   if (ctx->ws_uid == m->uid && ctx->ws_power == ctx->nu.lsq_weight_power && ctx->lsq_coef.n >= 2 * m->nst &&
-      ctx->fown.n >= 3 * NEQ * m->nc)
+      ctx->fown.n >= (int64_t)m->F * NEQ * m->nc)
     return 0;
   ctx->ws_uid = 0;
   TFA_CUDA(ctx->lsq_coef.alloc(2 * m->nst));
-  TFA_CUDA(ctx->fown.alloc(3 * NEQ * m->nc));
+  TFA_CUDA(ctx->fown.alloc((int64_t)m->F * NEQ * m->nc));
   TFA_TRY(launch_lsq_coef(*m, ctx->nu.lsq_weight_power, ctx->lsq_coef.p, st));
   ctx->ws_uid = m->uid;
   ctx->ws_power = ctx->nu.lsq_weight_power;
@@ -97,6 +97,14 @@ int tfa_set_numerics(tfa_ctx* ctx, const tfa_numerics* n) {
   return 0;
 }
 
+int tfa_set_ghost_states(tfa_ctx* ctx, const double* ghost, int64_t n_bfaces) {
+  if (!ctx || n_bfaces < 0) return set_error(TFA_EINVAL, "bad argument");
+  if (ghost && ((uintptr_t)ghost & 15)) return set_error(TFA_EINVAL, "ghost states must be 16-byte aligned");
+  ctx->ghost = ghost;
+  ctx->ghost_n = ghost ? n_bfaces : 0;
+  return 0;
+}
+
 void tfa_ctx_destroy(tfa_ctx* ctx) { delete ctx; }
 
 int tfa_gradients(tfa_ctx* ctx, const tfa_mesh* m, const double* state, double* grad, double* phi, void* stream) {
@@ -119,6 +127,9 @@ int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const do
   if (m->nc == 0) { ctx->launches = 0; return 0; }   // empty mesh: nothing to write
   if (!state || !state_n || !state_nm1 || !rhs) return set_error(TFA_EINVAL, "null argument");
   if (!(dt > 0.0)) return set_error(TFA_EINVAL, "dt must be positive");
+  if (m->has_ghost && (!ctx->ghost || ctx->ghost_n != m->nb))
+    return set_error(TFA_EINVAL, "the mesh has TFA_BC_GHOST faces: tfa_set_ghost_states needs an array of " +
+                                     std::to_string(m->nb) + " x 18 ghost states");
   cudaStream_t st = (cudaStream_t)stream;
   TFA_TRY(prepare(ctx, m, st));
   const Consts K = make_consts(ctx->ph, ctx->nu);
@@ -132,8 +143,8 @@ int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const do
   }
   TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
-  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, rhs, bsr_vals, ctx->flags.p,
-                          &ctx->asm_resident_ctas, st));
+  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, ctx->flags.p,
+                          ctx->asm_resident_ctas, st));
   if (ev) {
     TFA_CUDA(cudaEventRecord(ev[2], st));
     ++ctx->timed;

@@ -98,19 +98,21 @@ struct AsmCfg {
 
 // Inputs of one tile, fetched by TMA one tile ahead (read latency under the Jacobian's write stream is
 // long): own-side and other-side face states of every (cell, face), geometry records, cell-centre states.
-template <int T>
+// NF = face slots per cell: 3 (triangle meshes) or 4 (meshes with quadrilaterals).
+template <int T, int NF>
 struct __align__(16) AsmIn {
-  double fx[T][3][NEQ];   // other side of face k of cell c (the cell's own row again on a boundary face)
-  double fo[T][3][NEQ];   // own side
-  double cg[T][CGEO];
+  double fx[T][NF][NEQ];  // other side of face k of cell c: the neighbour's face state; on a boundary face the
+                          // cell's own row again, or the caller's ghost state (TFA_BC_GHOST)
+  double fo[T][NF][NEQ];  // own side
+  double cg[T][8 * NF];
   double st[T][NEQ];
-  int32_t nf[T][3];       // 4 * neighbour + its local face, -1 on the boundary
-  int32_t pad_[2];
+  int32_t nf[T][NF];      // packed neighbour (tfa_common.cuh): 4 * neighbour + its local face, or < 0 on the boundary
+  int32_t pad_[4 - (T * NF) % 4];   // keeps the struct a multiple of 16 bytes
 };
 
-template <int T, int NM>
+template <int T, int NM, int NF>
 struct __align__(128) AsmSmem {
-  AsmIn<T> in[2];
+  AsmIn<T, NF> in[2];
   uint64_t full[2];        // mbarriers: stage s has landed
   // staged blocks: a stride of BLKP doubles (16-byte multiple, odd number of 16-byte units) spreads the
   // column stores of different cells over the banks
@@ -209,38 +211,48 @@ __device__ __forceinline__ void cell_group_rest(const int grp, const Consts& K, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// One warp fetches the inputs of the tile starting at cell cellN (nN cells) into a stage: lane l < 3 nN
-// holds nfN = the packed neighbour of (cell, face) = l and copies that face's other-side row.
+// One warp fetches the inputs of the tile starting at cell cellN (nN cells) into a stage: lane l handles the
+// (cell, face) pairs l and l + 32 (nfN[0], nfN[1] = their packed neighbours) and copies each pair's other-side row.
 // ------------------------------------------------------------------------------------------------
-template <int T>
-__device__ __forceinline__ void stage_inputs(AsmIn<T>& in, uint64_t* bar, int lane, int32_t nfN, int64_t cellN,
-                                             int nN, const double* __restrict__ state,
-                                             const double* __restrict__ fown, const double* __restrict__ cgeo) {
-  static_assert(3 * T <= 30, "one lane per (cell, face) plus two for the contiguous arrays");
-  if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)nN * (3 * NEQ * 8 + 3 * NEQ * 8 + CGEO * 8 + NEQ * 8));
-  if (lane < 3 * nN) {
-    // boundary face: the other side is the cell itself (P_R := P_L, S9)
-    const int64_t row = nfN < 0 ? 3 * cellN + lane : 3 * (int64_t)(nfN >> 2) + (nfN & 3);
-    bulk_load(&in.fx[0][0][0] + lane * NEQ, fown + row * NEQ, NEQ * 8, bar);
-    (&in.nf[0][0])[lane] = nfN;
+template <int T, int NF>
+__device__ __forceinline__ void stage_inputs(AsmIn<T, NF>& in, uint64_t* bar, int lane, const int32_t (&nfN)[2],
+                                             int64_t cellN, int nN, const double* __restrict__ state,
+                                             const double* __restrict__ fown, const double* __restrict__ cgeo,
+                                             const double* __restrict__ ghost) {
+  static_assert(NF * T <= 64, "two (cell, face) pairs per lane");
+  if (lane == 0)
+    mbar_arrive_expect_tx(bar, (uint32_t)nN * (NF * NEQ * 8 + NF * NEQ * 8 + 8 * NF * 8 + NEQ * 8));
+#pragma unroll
+  for (int h = 0; h < (NF * T > 32 ? 2 : 1); ++h) {
+    const int l = lane + 32 * h;
+    if (l < NF * nN) {
+      const int32_t nf = nfN[h];
+      const double* src;
+      if (nf >= 0) src = fown + (NF * (int64_t)(nf >> 2) + (nf & 3)) * NEQ;          // the neighbour's face state
+      else if (bc_tag_of(nf) == TFA_BC_GHOST) src = ghost + bc_face_of(nf) * NEQ;     // the caller's ghost state
+      else src = fown + (NF * cellN + l) * NEQ;                                       // the cell's own row (S9, S24)
+      bulk_load(&in.fx[0][0][0] + l * NEQ, src, NEQ * 8, bar);
+      (&in.nf[0][0])[l] = nf;
+    }
   }
-  if (lane == 30) bulk_load(&in.fo[0][0][0], fown + 3 * NEQ * cellN, (uint32_t)nN * 3 * NEQ * 8, bar);
-  if (lane == 31) bulk_load(&in.cg[0][0], cgeo + CGEO * cellN, (uint32_t)nN * CGEO * 8, bar);
-  if (lane == 0) bulk_load(&in.st[0][0], state + NEQ * cellN, (uint32_t)nN * NEQ * 8, bar);
+  if (lane == 31) bulk_load(&in.fo[0][0][0], fown + NF * NEQ * cellN, (uint32_t)nN * NF * NEQ * 8, bar);
+  if (lane == 30) bulk_load(&in.cg[0][0], cgeo + 8 * NF * cellN, (uint32_t)nN * 8 * NF * 8, bar);
+  if (lane == 29) bulk_load(&in.st[0][0], state + NEQ * cellN, (uint32_t)nN * NEQ * 8, bar);
 }
 
 // ------------------------------------------------------------------------------------------------
 // The tile loop of one warp role.  All roles execute the same sequence of CTA barriers.
 // ------------------------------------------------------------------------------------------------
-template <int T, int NM, int ROLE>
-__device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, const int64_t nc, const Consts& K,
+template <int T, int NM, int NF, int ROLE>
+__device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC, const int64_t nc, const Consts& K,
                                           const double* __restrict__ state, const double* __restrict__ state_n,
                                           const double* __restrict__ state_nm1, const double inv2dt,
                                           const double* __restrict__ fown, const double* __restrict__ cgeo,
-                                          const int32_t* __restrict__ nbrf, const int32_t* __restrict__ blk4,
-                                          double* __restrict__ rhs, double* __restrict__ vals,
-                                          int32_t* __restrict__ flags) {
+                                          const int32_t* __restrict__ nbrf, const int32_t* __restrict__ blkmap,
+                                          const double* __restrict__ ghost, double* __restrict__ rhs,
+                                          double* __restrict__ vals, int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
+  constexpr int BS = blk_stride(NF);
   constexpr int NV = ROLE == 2 ? 8 : 5;   // variables (= rows) of the role's group
   constexpr int GL = NV + 1;              // lanes per group: base + NV perturbed
   constexpr int NG = ROLE == 2 ? 3 : 5;   // groups per warp
@@ -277,7 +289,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     const int ca = act ? cl : 0;
     const int64_t i = cell0 + ca;
     // this tile's inputs were requested one tile ago (kernel prologue for the first one)
-    const AsmIn<T>& in = S.in[it & 1];
+    const AsmIn<T, NF>& in = S.in[it & 1];
     mbar_wait(&S.full[it & 1], (it >> 1) & 1);
     const double* __restrict__ cg = in.cg[ca];
     const double* __restrict__ sO = in.st[ca];
@@ -297,8 +309,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     // the lines its non-TMA reads touch, towards L2
     const int64_t cellN = cell0 + (int64_t)gridDim.x * T;
     const int nN = cellN < nc ? (int)min((int64_t)T, nc - cellN) : 0;
-    int32_t nfN = -1;
-    if (loader && lane < 3 * nN) nfN = nbrf[3 * cellN + lane];
+    int32_t nfN[2] = {-1, -1};
+    if (loader) {
+      if (lane < NF * nN) nfN[0] = nbrf[NF * cellN + lane];
+      if (NF * T > 32 && lane + 32 < NF * nN) nfN[1] = nbrf[NF * cellN + lane + 32];
+    }
     if (warp == 0 && nN > 0) {
       const char* base;
       int l, bytes;
@@ -308,23 +323,29 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
         bytes = nN * NEQ * 8;
       } else if (lane < 29) {
         l = lane - 26;
-        base = reinterpret_cast<const char*>(blk4 + 4 * cellN);
-        bytes = nN * 16;
+        base = reinterpret_cast<const char*>(blkmap + BS * cellN);
+        bytes = nN * BS * 4;
       } else {
         l = lane - 29;   // the tile after the next one
-        base = reinterpret_cast<const char*>(nbrf + 3 * (cellN + (int64_t)gridDim.x * T));
-        bytes = cellN + (int64_t)gridDim.x * T + T <= nc ? T * 12 : 0;
+        base = reinterpret_cast<const char*>(nbrf + NF * (cellN + (int64_t)gridDim.x * T));
+        bytes = cellN + (int64_t)gridDim.x * T + T <= nc ? T * NF * 4 : 0;
       }
       if (l * 128 < bytes + 127 && bytes > 0) prefetch_l2(base + min(l * 128, bytes - 1));
     }
-    const int32_t nb0 = in.nf[ca][0], nb1 = in.nf[ca][1], nb2 = in.nf[ca][2];
+    int32_t nbk[NF];
+#pragma unroll
+    for (int k = 0; k < NF; ++k) nbk[k] = in.nf[ca][k];
 
     // where this tile's blocks go: thread t < ncell issues the bulk stores of cell t
     int4 b4 = make_int4(-1, -1, -1, -1);
+    int32_t b5 = -1;   // block of the fourth face (quadrilaterals)
     // bulk stores are issued by lane c (cell c) of warp 0 for the faces 0, 1 and of warp 1 for the diagonal block
     // and face 2, so that neither warp carries all 4 T requests of a tile (about 70 cycles each)
     const bool issuer = JAC && (warp == 0 || warp == WB) && lane < ncell;
-    if (issuer) b4 = *reinterpret_cast<const int4*>(blk4 + 4 * (cell0 + lane));
+    if (issuer) {
+      b4 = *reinterpret_cast<const int4*>(blkmap + BS * (cell0 + lane));
+      if (NF == 4) b5 = blkmap[BS * (cell0 + lane) + 4];
+    }
 
     // eps_k = delta * max(|P_cell,k|, ref_k), made representable (S7)
     const double Pcv = sO[v];
@@ -341,7 +362,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
 
     // ---- one face (Alg. 1): d = this lane's scaled flux (base lane) or flux-Jacobian column ----
     auto face = [&](const int k, double* __restrict__ d) -> bool {
-      const int32_t nf = k == 0 ? nb0 : (k == 1 ? nb1 : nb2);   // 4 * neighbour + its local face, or -1
+      const int32_t nf = nbk[k];   // packed neighbour: 4 * neighbour + its local face, or < 0 on the boundary
       const double2 g01 = *reinterpret_cast<const double2*>(cg + 8 * k);   // outward unit normal
       const double len = cg[8 * k + 2];                                    // Sigma_f
       const bool bnd = nf < 0;
@@ -374,10 +395,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
           }
         }
         if (any_bnd) {
-          // boundary face: P_R := P_L, so the perturbation moves both arguments (S9)
+          // boundary face (L260): the far side follows the face's rule; under the transmissive and the wall rule
+          // it is a function of the own side, so the perturbation moves both arguments (S9, S24)
           if (bnd) {
-#pragma unroll
-            for (int q = 0; q < NV; ++q) oth[q] = own[q];
+            if (ROLE == 2) bc_fields(bc_tag_of(nf), own, nx, ny, oth);
+            else bc_species(bc_tag_of(nf), own, nx, ny, oth);
           }
         }
         if (ROLE == 2) {
@@ -409,15 +431,19 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
     static_assert(NM == 2, "the barrier sequence below is written for two mirror buffers");
     constexpr bool EARLY2 = TFA_ASM_EARLY2 & (ROLE == 2 ? 2 : 1);   // evaluate face 2 together with faces 0, 1
 
-    double d0[NV], d1[NV], d2[NV];
+    // faces 0, 1 go out first (mirror buffers 0, 1), then face 2 -- and face 3 of a quadrilateral -- reuse them
+    double d0[NV], d1[NV], d2[NV], d3[NF == 4 ? NV : 1];
     const bool bnd0 = face(0, d0);
     const bool bnd1 = face(1, d1);
-    bool bnd2 = false;
-    if (EARLY2) bnd2 = face(2, d2);
+    bool bnd2 = false, bnd3 = false;
+    if (EARLY2) {
+      bnd2 = face(2, d2);
+      if constexpr (NF == 4) bnd3 = face(3, d3);
+    }
     if (loader && nN > 0) {
       // request the next tile's inputs into the other stage (every read of that stage ended before the
       // previous tile's closing barrier) — here, while this Maxwell warp would wait for the AUSM warps
-      stage_inputs<T>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo);
+      stage_inputs<T, NF>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo, ghost);
     }
     // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
     // them.  This barrier also publishes S.rs / S.s0 of the tile.
@@ -433,9 +459,15 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
       if (b4.z >= 0) bulk_store(vals + (int64_t)b4.z * BLK, &S.mir[1][lane][0], BLK * 8);
       bulk_commit();
     }
-    if (!EARLY2) bnd2 = face(2, d2);   // (the Maxwell lanes: while the bulk stores read the buffers)
+    if (!EARLY2) {   // (the Maxwell lanes: while the bulk stores read the buffers)
+      bnd2 = face(2, d2);
+      if constexpr (NF == 4) bnd3 = face(3, d3);
+    }
 #pragma unroll
-    for (int q = 0; q < NV; ++q) acc[q] = __dadd_rn(__dadd_rn(d0[q], d1[q]), d2[q]);
+    for (int q = 0; q < NV; ++q) {
+      acc[q] = __dadd_rn(__dadd_rn(d0[q], d1[q]), d2[q]);
+      if constexpr (NF == 4) acc[q] = __dadd_rn(acc[q], d3[q]);
+    }
 
     // ---- residual, source Jacobian (L245-253), BDF2 diagonal (Eq. 13), diagonal block ----
     if (act && !pert) {
@@ -520,15 +552,17 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
         }
       }
     }
-    // mirror buffer 0 has been read by face 0's bulk store: face 2 takes it
+    // the mirror buffers have been read by the bulk stores of faces 0, 1: faces 2 (and 3) take them
     if (warp == 0 && lane < T) bulk_wait_read();
     cta_sync();   // 2
     stage_mirror(0, d2, bnd2);
+    if constexpr (NF == 4) stage_mirror(1, d3, bnd3);
     fence_async_smem();
     cta_sync();   // B: every block of the tile is staged
     if (issuer && warp == WB) {
       bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[lane][0], BLK * 8);
       if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[0][lane][0], BLK * 8);
+      if (NF == 4 && b5 >= 0) bulk_store(vals + (int64_t)b5 * BLK, &S.mir[1][lane][0], BLK * 8);
       bulk_commit();
     }
   }
@@ -536,16 +570,16 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM>& S, const bool JAC, con
   if (nonphys) atomicAdd(flags, 1);
 }
 
-template <int T, int NM>
+template <int T, int NM, int NF>
 __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
-    const int32_t* __restrict__ blk4, double* __restrict__ rhs, double* __restrict__ vals,
-    int32_t* __restrict__ flags) {
+    const int32_t* __restrict__ blkmap, const double* __restrict__ ghost, double* __restrict__ rhs,
+    double* __restrict__ vals, int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  AsmSmem<T, NM>& S = *reinterpret_cast<AsmSmem<T, NM>*>(smem_raw);
+  AsmSmem<T, NM, NF>& S = *reinterpret_cast<AsmSmem<T, NM, NF>*>(smem_raw);
   // (residual-only calls go to k_residual; the JAC = false path here is kept for completeness)
   const bool JAC = vals != nullptr;
   const int warp = threadIdx.x >> 5;
@@ -563,15 +597,19 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     const int64_t cellF = (int64_t)blockIdx.x * T;
     const int nF = cellF < nc ? (int)min((int64_t)T, nc - cellF) : 0;
     if (nF > 0) {
-      const int32_t nfF = lane < 3 * nF ? nbrf[3 * cellF + lane] : -1;
-      stage_inputs<T>(S.in[0], &S.full[0], lane, nfF, cellF, nF, state, fown, cgeo);
+      int32_t nfF[2] = {-1, -1};
+      if (lane < NF * nF) nfF[0] = nbrf[NF * cellF + lane];
+      if (NF * T > 32 && lane + 32 < NF * nF) nfF[1] = nbrf[NF * cellF + lane + 32];
+      stage_inputs<T, NF>(S.in[0], &S.full[0], lane, nfF, cellF, nF, state, fown, cgeo, ghost);
     }
   }
   __syncthreads();   // the prologue's neighbour table (plain stores) is visible
   if (warp >= C::AW)
-    role_loop<T, NM, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
+    role_loop<T, NM, NF, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs, vals,
+                            flags);
   else
-    role_loop<T, NM, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blk4, rhs, vals, flags);
+    role_loop<T, NM, NF, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs, vals,
+                            flags);
 }
 
 // ================================================================================================
@@ -580,30 +618,37 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
 // fields), the three faces in sequence, face states straight from the gradient kernel's array.
 // ================================================================================================
 constexpr int RES_CELLS = 32;
-template <int ROLE>
+template <int ROLE, int NF>
 __device__ __forceinline__ void residual_rows(const int64_t i, const Consts& K, const double* __restrict__ state,
                                               const double* __restrict__ state_n, const double* __restrict__ state_nm1,
                                               const double inv2dt, const double* __restrict__ fown,
                                               const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
-                                              double* __restrict__ rhs, bool& nonphys) {
+                                              const double* __restrict__ ghost, double* __restrict__ rhs,
+                                              bool& nonphys) {
   constexpr int NV = ROLE == 2 ? 8 : 5;
   constexpr int SPC = ROLE == 2 ? 0 : ROLE;
-  const double* __restrict__ cg = cgeo + CGEO * i;
+  const double* __restrict__ cg = cgeo + 8 * NF * i;
   double acc[NV];
 #pragma unroll
   for (int q = 0; q < NV; ++q) acc[q] = 0.0;
   if (K.mask & 1) {
 #pragma unroll 1
-    for (int k = 0; k < 3; ++k) {
-      const int32_t nf = nbrf[3 * i + k];
+    for (int k = 0; k < NF; ++k) {
+      const int32_t nf = nbrf[NF * i + k];
       const double nx = cg[8 * k], ny = cg[8 * k + 1], len = cg[8 * k + 2];
-      const double* __restrict__ fo = fown + (3 * i + k) * NEQ;
-      const double* __restrict__ fx = nf < 0 ? fo : fown + (3 * (int64_t)(nf >> 2) + (nf & 3)) * NEQ;
+      const double* __restrict__ fo = fown + (NF * i + k) * NEQ;
+      const int tag = nf < 0 ? bc_tag_of(nf) : 0;
+      const double* __restrict__ fx = nf >= 0 ? fown + (NF * (int64_t)(nf >> 2) + (nf & 3)) * NEQ
+                                              : (tag == TFA_BC_GHOST ? ghost + bc_face_of(nf) * NEQ : fo);
       double own[NV], oth[NV], H[NV];
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         own[q] = fo[vidx<ROLE>(q)];
         oth[q] = fx[vidx<ROLE>(q)];
+      }
+      if (nf < 0) {   // boundary face (L260): the far side follows the face's rule
+        if (ROLE == 2) bc_fields(tag, own, nx, ny, oth);
+        else bc_species(tag, own, nx, ny, oth);
       }
       if (ROLE == 2) maxwell_flux(K, own, oth, nx, ny, H);
       else nonphys |= !ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nx, ny, H);
@@ -618,59 +663,69 @@ __device__ __forceinline__ void residual_rows(const int64_t i, const Consts& K, 
   for (int q = 0; q < NV; ++q) rhs[NEQ * i + vidx<ROLE>(q)] = -(acc[q] + rs[vidx<ROLE>(q)]);
 }
 
+template <int NF>
 __global__ void __launch_bounds__(3 * RES_CELLS) k_residual(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
-    double* __restrict__ rhs, int32_t* __restrict__ flags) {
+    const double* __restrict__ ghost, double* __restrict__ rhs, int32_t* __restrict__ flags) {
   const int role = threadIdx.x >> 5;   // warp 0 ions, 1 electrons, 2 fields
   const int64_t i = blockIdx.x * (int64_t)RES_CELLS + (threadIdx.x & 31);
   if (i >= nc) return;
   bool nonphys = false;
-  if (role == 0) residual_rows<0>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, rhs, nonphys);
-  else if (role == 1) residual_rows<1>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, rhs, nonphys);
-  else residual_rows<2>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, rhs, nonphys);
+  if (role == 0) residual_rows<0, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys);
+  else if (role == 1) residual_rows<1, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys);
+  else residual_rows<2, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys);
   if (nonphys) atomicAdd(flags, 1);
 }
 
 // ================================================================================================
 namespace {
-template <int T, int NM>
+template <int T, int NM, int NF>
 int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-              const double* state_nm1, double dt, const double* fown, double* rhs, double* vals, int32_t* flags,
-              int* resident_ctas, cudaStream_t st) {
+              const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs, double* vals,
+              int32_t* flags, int* resident_ctas, cudaStream_t st) {
   using C = AsmCfg<T>;
-  const int smem = (int)sizeof(AsmSmem<T, NM>);
+  const int smem = (int)sizeof(AsmSmem<T, NM, NF>);
   if (*resident_ctas <= 0) {   // once per context (= per device): CTAs that fit the GPU at once
-    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, NM, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int dev = 0, occ = 0, n_sm = 0;
     TFA_CUDA(cudaGetDevice(&dev));
     TFA_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, NM>, C::NT, smem));
+    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, NM, NF>, C::NT, smem));
     if (occ < 1) return set_error(TFA_ECUDA, "k_assemble does not fit on an SM");
     *resident_ctas = n_sm * occ;
   }
   const int64_t ntiles = (m.nc + T - 1) / T;
   const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)*resident_ctas);
   const double inv2dt = 1.0 / (2.0 * dt);
-  k_assemble<T, NM><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
-                                               m.nbrf.p, m.blk4.p, rhs, vals, flags);
+  k_assemble<T, NM, NF><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
+                                                   m.nbrf.p, m.blkmap.p, ghost, rhs, vals, flags);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
 }  // namespace
 
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
-                    const double* state_nm1, double dt, const double* fown, double* rhs, double* vals,
-                    int32_t* flags, int* resident_ctas, cudaStream_t st) {
+                    const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs,
+                    double* vals, int32_t* flags, int* resident_ctas /*[2]: F = 3, 4*/, cudaStream_t st) {
   if (m.nc == 0) return 0;
   if (!vals) {
-    k_residual<<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, 1.0 / (2.0 * dt), fown,
-                                                             m.cgeo.p, m.nbrf.p, rhs, flags);
+    const double inv2dt = 1.0 / (2.0 * dt);
+    if (m.F == 3)
+      k_residual<3><<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown,
+                                                                   m.cgeo.p, m.nbrf.p, ghost, rhs, flags);
+    else
+      k_residual<4><<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown,
+                                                                   m.cgeo.p, m.nbrf.p, ghost, rhs, flags);
     TFA_CUDA(cudaGetLastError());
     return 0;
   }
-  return launch_nm<TFA_ASM_T, 2>(m, K, state, state_n, state_nm1, dt, fown, rhs, vals, flags, resident_ctas, st);
+  if (m.F == 3)
+    return launch_nm<TFA_ASM_T, 2, 3>(m, K, state, state_n, state_nm1, dt, fown, ghost, rhs, vals, flags,
+                                      resident_ctas, st);
+  return launch_nm<TFA_ASM_T, 2, 4>(m, K, state, state_n, state_nm1, dt, fown, ghost, rhs, vals, flags,
+                                    resident_ctas + 1, st);
 }
 
 }  // namespace tfa

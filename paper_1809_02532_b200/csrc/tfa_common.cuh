@@ -31,16 +31,24 @@ uint64_t next_mesh_uid();
 
 inline unsigned cdiv(int64_t a, int64_t b) { return (unsigned)((a + b - 1) / b); }
 
-// Per-cell geometry record, 24 doubles = 192 B:
-//   for local face k = 0..2 at [8k .. 8k+7]:
+// Per-cell geometry record, 8 F doubles (F = faces per cell slot of the mesh: 3 -> 192 B, 4 -> 256 B; DESIGN.md
+// "Data layout"):
+//   for local face k = 0..F-1 at [8k .. 8k+7]:
 //     0 nx, 1 ny   unit normal pointing OUT of this cell: the face's normal, computed from its L
 //                  cell's corners (S10), with the sign flipped when this cell is the face's R cell
 //     2 len        face length Sigma_f
 //     3 dxo, 4 dyo face midpoint minus OWN centroid (own corner coordinates)
 //     5 dxn, 6 dyn face midpoint minus NEIGHBOUR centroid (neighbour's corner coordinates);
-//                  on a boundary face the own-side values again (P_R := P_L, S9)
-//     7 extra      k=0: volume Omega_i;  k=1: sqrt(Omega_i);  k=2: unused (0)
-constexpr int CGEO = 24;
+//                  on a boundary face the own-side values again
+//     7 extra      k=0: volume Omega_i;  k=1: sqrt(Omega_i);  else unused (0)
+//   The fourth slot of a triangle in a mixed mesh is a face of zero length (normal (1,0), zero offsets): it runs
+//   through the same code as a transmissive boundary face and contributes exactly nothing.
+constexpr int cgeo_stride(int F) { return 8 * F; }
+// block map of cell i: [0] = BSR block index of (i,i), [1+k] = of (nbr_k, i), the block cell i writes INTO ITS
+// NEIGHBOUR'S ROW; -1 if none.  Stride 4 ints for F = 3, 8 ints for F = 4 (16-byte aligned rows).
+constexpr int blk_stride(int F) { return F == 3 ? 4 : 8; }
+// Packed neighbour of local face k (nbrf): interior 4 * neighbour + (the face's local index in the neighbour);
+// boundary -1 - (4 * boundary-face index + TFA_BC_* tag); a triangle's fourth slot -1 (= transmissive, zero length).
 
 template <class T>
 struct DevBuf {
@@ -71,22 +79,25 @@ struct DevBuf {
 }  // namespace tfa
 
 struct tfa_mesh {
-  int64_t nn = 0, nc = 0, nf = 0, nnzb = 0, nst = 0;
+  int64_t nn = 0, nc = 0, nf = 0, nnzb = 0, nst = 0, nb = 0;
+  int F = 3;                 // face slots per cell: 3 (triangles only) or 4 (some quadrilaterals)
+  bool has_ghost = false;    // some boundary face carries TFA_BC_GHOST
   uint64_t uid = 0;          // process-wide monotonic stamp, new at every (re)build; ctx workspaces key on it
   tfa::DevBuf<double> node_xy;     // [nn][2]
-  tfa::DevBuf<int32_t> cell_nodes; // [nc][3]
-  tfa::DevBuf<double> cell_xy;     // [nc][3][2]
+  tfa::DevBuf<int32_t> cell_nodes; // [nc][F], -1 in the fourth slot of a triangle
+  tfa::DevBuf<double> cell_xy;     // [nc][F][2]
   tfa::DevBuf<int32_t> perm;       // [nc] new -> original
   // derived
   tfa::DevBuf<int32_t> face_nodes, face_cells;  // [nf][2]
-  tfa::DevBuf<int32_t> cell_faces, cell_nbr;    // [nc][3]
-  tfa::DevBuf<int32_t> nbrf;                    // [nc][3] 4 * neighbour + its local face index, -1 on the boundary
+  tfa::DevBuf<int32_t> cell_faces, cell_nbr;    // [nc][F]
+  tfa::DevBuf<int32_t> nbrf;                    // [nc][F] packed neighbour (see above)
   tfa::DevBuf<int32_t> st_ptr, st_idx;          // CSR stencil
   tfa::DevBuf<double> st_d;                     // [nst][2] centroid displacement (S9)
   tfa::DevBuf<int32_t> bsr_rowptr, bsr_col;
-  tfa::DevBuf<int32_t> blk4;                    // [nc][4] BSR block index of (i,i) and of (nbr_k, i); -1 if none
+  tfa::DevBuf<int32_t> blkmap;                  // [nc][blk_stride(F)]
   tfa::DevBuf<double> cen;                      // [nc][2]
-  tfa::DevBuf<double> cgeo;                     // [nc][24]
+  tfa::DevBuf<double> cgeo;                     // [nc][8 F]
+  tfa::DevBuf<int32_t> bfaces, bface_of, bc_tag;  // [nb], [nf], [nb]
 };
 
 struct tfa_ctx {
@@ -96,7 +107,9 @@ struct tfa_ctx {
   uint64_t ws_uid = 0;
   double ws_power = -1.0;
   tfa::DevBuf<double> lsq_coef;   // [nst][2]
-  tfa::DevBuf<double> fown;       // [nc][3][18] own-side face states P_i + phi grad P_i . (x_f - x_i)  (L232)
+  tfa::DevBuf<double> fown;       // [nc][F][18] own-side face states P_i + phi grad P_i . (x_f - x_i)  (L232)
+  const double* ghost = nullptr;  // caller-owned device array [ghost_n][18] (tfa_set_ghost_states)
+  int64_t ghost_n = 0;
   tfa::DevBuf<int32_t> flags;     // [4] device counters: 0 = non-physical states
   // Krylov workspace of tfa_gmres: (restart + 2) vectors of 18 nc doubles, and reduction scratch
   tfa::DevBuf<double> krylov, red;
@@ -105,7 +118,7 @@ struct tfa_ctx {
   // device staging buffers of tfa_assemble_host
   tfa::DevBuf<double> stage_state[3], stage_rhs, stage_vals;
   int launches = 0;
-  int asm_resident_ctas = 0;      // persistent grid of k_assemble on this context's device (0 = not queried yet)
+  int asm_resident_ctas[2] = {0, 0};   // persistent grid of k_assemble<F = 3, 4> on this context's device (0 = not queried yet)
   // optional per-kernel timing (tfa_timing_enable): a ring of event triples
   static constexpr int kMaxTimed = 64;
   bool timing = false;

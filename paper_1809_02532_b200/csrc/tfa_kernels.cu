@@ -47,9 +47,12 @@ __global__ void k_lsq_coef(int64_t nc, const int32_t* __restrict__ st_ptr, const
 // 32 cells per CTA; 9 consecutive lanes read one neighbour state (144 contiguous bytes).  Four CTAs per SM
 // (56 registers: 32-bit stencil indices, the cell's geometry read after the stencil walk): 0.364 against 0.384 ms
 // with three CTAs at 72 registers; five CTAs spill into the walk (0.57-0.60 ms).
+// NF = face slots per cell (3: triangle meshes, 4: meshes with quadrilaterals; the empty fourth slot of a triangle
+// has a zero offset, hence Delta_2 = 0, and drops out of the limiter).
 constexpr int GP_CELLS = 32;
 constexpr int GP_T = GP_CELLS * (NEQ / 2);   // 288 threads
-__global__ void __launch_bounds__(GP_T, 4) k_gradient_limiter(
+template <int NF>
+__global__ void __launch_bounds__(GP_T, NF == 3 ? 4 : 3) k_gradient_limiter(
     int64_t nc, const double* __restrict__ state, const int32_t* __restrict__ st_ptr,
     const int32_t* __restrict__ st_idx, const double* __restrict__ coef, const double* __restrict__ cgeo,
     double venkK, double* __restrict__ fown, double* __restrict__ grad_out, double* __restrict__ phi_out) {
@@ -91,22 +94,22 @@ __global__ void __launch_bounds__(GP_T, 4) k_gradient_limiter(
   for (; q < e; ++q) add(coef2[q], *reinterpret_cast<const double2*>(state + NEQ * (int64_t)st_idx[q] + v));
   // the cell's own geometry is read here, not before the walk (volatile keeps the compiler from hoisting the loads
   // and holding 14 more registers across it)
-  const volatile double* g = cgeo + CGEO * i;
-  double ox[3], oy[3];
+  const volatile double* g = cgeo + 8 * NF * i;
+  double ox[NF], oy[NF];
 #pragma unroll
-  for (int k = 0; k < 3; ++k) {
+  for (int k = 0; k < NF; ++k) {
     ox[k] = g[8 * k + 3];
     oy[k] = g[8 * k + 4];
   }
   const double sqrt_vol = g[15];
   const double Kh = venkK * sqrt_vol;
   const double eps2 = Kh * Kh * Kh;
-  double phi[2], f[3][2];
+  double phi[2], f[NF][2];
 #pragma unroll
   for (int t = 0; t < 2; ++t) {
     double nb = 1.0, db = 1.0;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
+    for (int k = 0; k < NF; ++k) {
       const double d2 = gx[t] * ox[k] + gy[t] * oy[k];
       const double d1 = d2 > 0.0 ? dmax[t] : dmin[t];
       const double num = d1 * d1 + eps2 + 2.0 * d1 * d2;
@@ -119,12 +122,12 @@ __global__ void __launch_bounds__(GP_T, 4) k_gradient_limiter(
     const double lx = phi[t] * gx[t], ly = phi[t] * gy[t];
     const double P0 = t == 0 ? Pi.x : Pi.y;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) f[k][t] = P0 + (lx * ox[k] + ly * oy[k]);
+    for (int k = 0; k < NF; ++k) f[k][t] = P0 + (lx * ox[k] + ly * oy[k]);
   }
   if (fown) {
 #pragma unroll
-    for (int k = 0; k < 3; ++k)
-      *reinterpret_cast<double2*>(fown + (3 * i + k) * NEQ + v) = make_double2(f[k][0], f[k][1]);
+    for (int k = 0; k < NF; ++k)
+      *reinterpret_cast<double2*>(fown + (NF * i + k) * NEQ + v) = make_double2(f[k][0], f[k][1]);
   }
   if (grad_out) {
     *reinterpret_cast<double2*>(grad_out + 2 * (NEQ * i + v)) = make_double2(gx[0], gy[0]);
@@ -175,8 +178,12 @@ int launch_lsq_coef(const tfa_mesh& m, double power, double* coef, cudaStream_t 
 int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* fown,
                     double* grad, double* phi, cudaStream_t st) {
   if (m.nc == 0) return 0;
-  k_gradient_limiter<<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p, venkK,
-                                                           fown, grad, phi);
+  if (m.F == 3)
+    k_gradient_limiter<3><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
+                                                                venkK, fown, grad, phi);
+  else
+    k_gradient_limiter<4><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
+                                                                venkK, fown, grad, phi);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }

@@ -66,11 +66,6 @@ __host__ inline Consts make_consts(const tfa_physics& ph, const tfa_numerics& nu
   return K;
 }
 
-// index of the j-th variable (rho, u, v, w, T) of species s in the 18-vector
-__device__ __forceinline__ int sp_idx(int s, int j) {
-  return j == 0 ? 8 + s : (j == 4 ? 16 + s : 9 + 3 * s + j);
-}
-
 // Modified Rusanov flux of the Maxwell + cleaning rows (Eq. 9; F.n of Eq. 2).
 // |A_n|dU = c dU_t + (cleaning speed) dU_n for B and E, (cleaning speed) dPsi/dPhi (S3).
 __device__ __forceinline__ void maxwell_flux(const Consts& K, const double* L, const double* R, double nx,
@@ -99,9 +94,12 @@ __device__ __forceinline__ void maxwell_flux(const Consts& K, const double* L, c
 
 // Square root and reciprocal for the flux: a single-precision hardware seed (MUFU.RSQ / MUFU.RCP, 23
 // bits) refined by two Newton steps in FP64 (fused multiply-adds only) -- about half the instructions
-// and latency of the correctly rounded library sequences, error below 1 ulp.  Arguments are the
-// positive, O(1)-scaled quantities of a physical state (a non-physical one is reported by the
-// rho, T > 0 test, whatever these return).
+// and latency of the correctly rounded library sequences, error below 1 ulp (tests: tfa_probe_math).
+// Precondition: the argument lies in the normal single-precision range (about 1e-38 .. 3e38) and is positive:
+// zero, negative, subnormal-in-float or huge arguments give NaN / Inf, not the IEEE result.  The callers pass
+// gamma R T, a_1/2, f_a rho of a physical state, O(1e-3 .. 1e3) in the normalised units; a non-physical state
+// (rho <= 0 or T <= 0) is reported by the separate test, whatever these return.  TFA_FAST_MATH64 = 0 compiles
+// the IEEE sequences instead.
 __device__ __forceinline__ double nsqrt(double x) {
   const double y = (double)rsqrtf((float)x);
   double g = x * y, h = 0.5 * y;
@@ -171,76 +169,36 @@ __device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, doubl
   return ok;
 }
 
-// Two-fluid source (Eq. 4, Eq. 6; charge density rho_s q_s/m_s, S5; eps0 = 1/c^2)
-__device__ __forceinline__ void source_terms(const Consts& K, const double* P, double* S) {
-  const double qi = K.qm[0] * P[8], qe = K.qm[1] * P[9];   // q_s n_s
-  const double Bx = P[0], By = P[1], Bz = P[2], Ex = P[3], Ey = P[4], Ez = P[5];
-  const double ux = P[10], uy = P[11], uz = P[12], vx = P[13], vy = P[14], vz = P[15];
-  S[0] = S[1] = S[2] = 0.0;
-  S[3] = -K.c2 * (qi * ux + qe * vx);
-  S[4] = -K.c2 * (qi * uy + qe * vy);
-  S[5] = -K.c2 * (qi * uz + qe * vz);
-  S[6] = 0.0;
-  S[7] = K.c2 * (qi + qe);
-  S[8] = S[9] = 0.0;
-  S[10] = qi * (Ex + (uy * Bz - uz * By));
-  S[11] = qi * (Ey + (uz * Bx - ux * Bz));
-  S[12] = qi * (Ez + (ux * By - uy * Bx));
-  S[13] = qe * (Ex + (vy * Bz - vz * By));
-  S[14] = qe * (Ey + (vz * Bx - vx * Bz));
-  S[15] = qe * (Ez + (vx * By - vy * Bx));
-  S[16] = qi * (ux * Ex + uy * Ey + uz * Ez);
-  S[17] = qe * (vx * Ex + vy * Ey + vz * Ez);
-}
-
-// conservative variables of one species, U = (rho, rho u, rho (c_v T + u^2/2))  (Eq. 5)
-__device__ __forceinline__ void cons_species(const Consts& K, int s, const double* Q, double* U) {
-  const double rho = Q[0];
-  U[0] = rho;
-  U[1] = rho * Q[1];
-  U[2] = rho * Q[2];
-  U[3] = rho * Q[3];
-  U[4] = rho * (K.cv[s] * Q[4] + 0.5 * (Q[1] * Q[1] + Q[2] * Q[2] + Q[3] * Q[3]));
-}
-
-// static-index access to the five rows/variables of species SP inside an 18-vector held in registers
-template <int SP>
-__device__ __forceinline__ void sp_get(const double* v18, double* v5) {
-  v5[0] = v18[8 + SP];
-  v5[1] = v18[10 + 3 * SP];
-  v5[2] = v18[11 + 3 * SP];
-  v5[3] = v18[12 + 3 * SP];
-  v5[4] = v18[16 + SP];
-}
-template <int SP>
-__device__ __forceinline__ void sp_put(double* v18, const double* v5) {
-  v18[8 + SP] = v5[0];
-  v18[10 + 3 * SP] = v5[1];
-  v18[11 + 3 * SP] = v5[2];
-  v18[12 + 3 * SP] = v5[3];
-  v18[16 + SP] = v5[4];
-}
-// column v of (3 Omega / 2 dt) dU/dP for a species variable v (analytic, S15)
-template <int SP>
-__device__ __forceinline__ void time_column(const Consts& K, double* col, int v, const double* P, double ft) {
-  constexpr int ir = 8 + SP, iu = 10 + 3 * SP, iT = 16 + SP;
-  const double rho = P[ir], ux = P[iu], uy = P[iu + 1], uz = P[iu + 2], T = P[iT];
-  if (v == ir) {
-    col[ir] += ft;
-    col[iu] += ft * ux;
-    col[iu + 1] += ft * uy;
-    col[iu + 2] += ft * uz;
-    col[iT] += ft * (K.cv[SP] * T + 0.5 * (ux * ux + uy * uy + uz * uz));
-  } else if (v == iT) {
-    col[iT] += ft * rho * K.cv[SP];
-  } else {
+// Far side of a boundary face, per group of variables (the boundary loop of L260 folded into the face lanes;
+// include/tfa.h TFA_BC_*).  TRANSMISSIVE: the own side again (S9).  WALL: its mirror image (S24): B and u_s flip
+// their normal component, E its tangential ones (z included), Phi flips; Psi, rho_s, T_s are kept.  GHOST: `oth`
+// already holds the caller's ghost state (fetched in place of a neighbour's face state) and is left alone.
+__device__ __forceinline__ void bc_fields(int tag, const double* own, double nx, double ny, double* oth) {
+  if (tag == TFA_BC_GHOST) return;
 #pragma unroll
-    for (int d = 0; d < 3; ++d)
-      if (v == iu + d) {
-        col[iu + d] += ft * rho;
-        col[iT] += ft * rho * P[iu + d];
-      }
+  for (int q = 0; q < 8; ++q) oth[q] = own[q];
+  if (tag == TFA_BC_WALL) {
+    const double Bn = own[0] * nx + own[1] * ny, En = own[3] * nx + own[4] * ny;
+    oth[0] = own[0] - 2.0 * Bn * nx;
+    oth[1] = own[1] - 2.0 * Bn * ny;
+    oth[3] = 2.0 * En * nx - own[3];
+    oth[4] = 2.0 * En * ny - own[4];
+    oth[5] = -own[5];
+    oth[7] = -own[7];
   }
 }
+__device__ __forceinline__ void bc_species(int tag, const double* own, double nx, double ny, double* oth) {
+  if (tag == TFA_BC_GHOST) return;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) oth[q] = own[q];
+  if (tag == TFA_BC_WALL) {
+    const double un = own[1] * nx + own[2] * ny;
+    oth[1] = own[1] - 2.0 * un * nx;
+    oth[2] = own[2] - 2.0 * un * ny;
+  }
+}
+// tag of a boundary face from its packed neighbour entry (tfa_common.cuh): -1 - (4 b + tag)
+__device__ __forceinline__ int bc_tag_of(int32_t packed) { return (-1 - packed) & 3; }
+__device__ __forceinline__ int64_t bc_face_of(int32_t packed) { return (int64_t)((-1 - packed) >> 2); }
 
 }  // namespace tfa

@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(SV_T) k_bsr_spmv(int64_t nc, const int32_t* __
 // per element made it shared-memory-bandwidth bound, 9.8 ms at 1M cells.)
 // ------------------------------------------------------------------------------------------------
 constexpr int BJ_WARPS = 8;
-__global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ blk4,
+__global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ blkmap, int BS,
                                                                const double* __restrict__ vals,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
   __shared__ __align__(16) double rowbuf[BJ_WARPS][2][NEQ];
@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
   if (i >= nc) return;
-  const int64_t bd = blk4[4 * i];   // the diagonal block of row i (every row of the mesh's pattern has one)
+  const int64_t bd = blkmap[(int64_t)BS * i];   // the diagonal block of row i (every row of the mesh's pattern has one)
   const bool has = lane < NEQ;
   double a[NEQ];
 #pragma unroll
@@ -356,7 +356,7 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->blk4.p, bsr_vals, dinv,
+  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->blkmap.p, blk_stride(m->F), bsr_vals, dinv,
                                                                   ctx->flags.p);
   TFA_CUDA(cudaGetLastError());
   return 0;

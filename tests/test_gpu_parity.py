@@ -378,21 +378,18 @@ def test_config2_first_and_last_of_ten_calls(api, orc, W):
 
 
 SWEEP_CHUNK = 100_000
-RES_TOL_CANCELLING = 1e-10   # mass / energy rows against the flux + source scale (derivation in the test)
 
 
-@pytest.mark.parametrize("name", ["c2", "c3", "c4a", "c4b", "c5"])
-def test_full_size_every_row(api, orc, W, name):
-    """BASELINE configs 2-5 at their full sizes, in the launch configuration bench.py times (device buffers,
-    RCM where the config says so): EVERY row of rhs and of the BSR Jacobian against the oracle, swept in chunks
-    of 100 000 consecutive rows (oracle row-subset mode; the GPU's value array is sliced per chunk), so that
-    every persistent CTA, both stages of the input pipeline and the tail tile are covered.  The pattern is
-    compared bit-exactly over the whole mesh; every entry of the value array must have been written (NaN canary).
-    The residual is held to 1e-12 of the full sum-of-|terms| scale (S18), and -- with the BDF2 term masked out of
-    both sides, term_mask = 3 -- to the flux + source scale alone, which in these configurations
-    (P^n = P^{n-1} = P) is up to 1e3 times smaller for the density and energy rows (bars at the end)."""
+def sweep_every_row(api, orc, W, w, bc=None, flux_noise=0.0):
+    """Assemble workload `w` on the GPU in the launch configuration bench.py times (device buffers, RCM where the
+    workload says so) and compare EVERY row of rhs and of the BSR Jacobian with the oracle, swept in chunks of
+    100 000 consecutive rows (oracle row-subset mode; the GPU's value array is sliced per chunk), so that every
+    persistent CTA, both stages of the input pipeline and the tail tile are covered.  The pattern is compared
+    bit-exactly over the whole mesh; every entry of the value array must have been written (NaN canary).
+    bc(g, o) -> (tags, ghost) sets boundary rules on both sides.  A second, residual-only pass compares flux +
+    source alone (term_mask = 3 on both sides) against their own scale, on the state plus U(-flux_noise,
+    flux_noise).  Returns (er, er_flux_source_per_variable, ej)."""
     import torch
-    w = W.make_workload(name)
     g, o = api.Mesh.from_input(w.mesh), orc.OracleMesh.from_input(w.mesh)
     if w.reorder == "rcm":
         g.reorder("rcm")
@@ -404,6 +401,14 @@ def test_full_size_every_row(api, orc, W, name):
     rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
     assert np.array_equal(rp, o.get("bsr_rowptr")) and np.array_equal(col, o.get("bsr_col"))
     ctx = api.Context(w.physics)
+    ctx3 = api.Context(w.physics, api.default_numerics(ctx.physics, term_mask=3))
+    if bc is not None:
+        tags, ghost = bc(g, o)
+        g.set_bc(tags)
+        o.set_bc(tags, ghost)
+        gd = None if ghost is None else dev(ghost)
+        ctx.set_ghost_states(gd)
+        ctx3.set_ghost_states(gd)
     Pd = dev(P)
     rhs = torch.full((nc, 18), float("nan"), dtype=torch.float64, device="cuda")
     vals = torch.full((g.nnzb, 18, 18), float("nan"), dtype=torch.float64, device="cuda")
@@ -411,10 +416,9 @@ def test_full_size_every_row(api, orc, W, name):
     ctx.check()
     assert not bool(torch.isnan(vals).any()), "an entry of the BSR value array was not written"
     assert not bool(torch.isnan(rhs).any())
-    # flux + source only (residual-only kernel and Jacobian kernel), for the second residual bar
-    nu3 = api.default_numerics(ctx.physics, term_mask=3)
-    ctx3 = api.Context(w.physics, nu3)
-    rhs3, _ = ctx3.assemble(g, Pd, dt=w.dt, jacobian=False)
+    # flux + source only, through the residual-only kernel, for the second residual bar
+    P3 = P + np.random.default_rng(31).uniform(-flux_noise, flux_noise, P.shape) if flux_noise > 0 else P
+    rhs3, _ = ctx3.assemble(g, dev(P3), dt=w.dt, jacobian=False)
     ctx3.check()
     rhs_h, rhs3_h = rhs.cpu().numpy(), rhs3.cpu().numpy()
     ph_o = orc.physics_c(w.physics)
@@ -429,20 +433,32 @@ def test_full_size_every_row(api, orc, W, name):
         ej = max(ej, jacobian_error_padded(got, vals_o, rp[r0:r1 + 1] - rp[r0]))
         num = np.maximum(num, np.abs(rhs_h[r0:r1] - rhs_o).max(axis=0))
         den = np.maximum(den, sc_o.max(axis=0))
-        rhs3_o, sc3_o, _ = orc.assemble(o, ph_o, nu3_o, P, dt=w.dt, rows=rows, jacobian=False)
+        rhs3_o, sc3_o, _ = orc.assemble(o, ph_o, nu3_o, P3, dt=w.dt, rows=rows, jacobian=False)
         num3 = np.maximum(num3, np.abs(rhs3_h[r0:r1] - rhs3_o).max(axis=0))
         den3 = np.maximum(den3, sc3_o.max(axis=0))
     er = float((num / np.where(den > 0, den, 1.0)).max())
     e3 = num3 / np.where(den3 > 0, den3, 1.0)
+    return er, e3, ej
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4a", "c4b", "c5"])
+def test_full_size_every_row(api, orc, W, name):
+    """BASELINE configs 2-5 at their full sizes: every row against the oracle (sweep_every_row).  The residual is
+    held to 1e-12 of the full sum-of-|terms| scale (S18), and -- with the BDF2 term masked out of both sides,
+    term_mask = 3 -- to 1e-12 of the flux + source scale alone, which in these configurations (P^n = P^{n-1} = P)
+    is up to 1e3 times smaller for the density and energy rows.
+
+    The second bar is taken on the state plus U(-1e-3, 1e-3) (the noise config 2 carries anyway).  On the exactly
+    smooth GEM state whole rows of the flux are differences of two nearly equal reconstructed face states and
+    nothing else: the B_x, B_y rows (E_z = Psi = 0 leaves only the Rusanov dissipation c (B_R - B_L)) and the mass /
+    energy rows (u_s.n = 0 leaves only the pressure-diffusion term ~ p_R - p_L).  The jump is O(h^2) of the state,
+    so the rounding of the reconstruction (2^-53 |P|, different on the two sides: own-frame lanes against the
+    oracle's L/R frame) is amplified by |P| / |P_R - P_L| = 1e4..1e7 relative to such a row's own scale (measured
+    6e-12 on c3, 4e-11 on c5, 1e-9 on the Cartesian q1): the conditioning of those rows, not an error of either
+    side, and already bounded by the first bar, which is 1e-11 of the un-cancelled flux magnitude c |P| Sigma."""
+    er, e3, ej = sweep_every_row(api, orc, W, W.make_workload(name), flux_noise=0.0 if name == "c2" else 1e-3)
     assert er < RES_TOL and ej < JAC_TOL, (name, er, ej)
-    # Flux + source scale: the field and momentum rows meet 1e-12 of it.  The mass and energy rows (8, 9, 16, 17)
-    # carry mdot (1, H); in the GEM configurations u_s.n = 0 on every face, so mdot is the pressure-diffusion
-    # term alone, proportional to p_R - p_L: a difference of two nearly equal face pressures, whose rounding
-    # (2^-53 p from the reconstruction) is amplified by p / |p_R - p_L| ~ 1e4..1e5 on these meshes.  That is the
-    # conditioning of the term itself (both sides compute it in the same order), so those rows are held to 1e-10.
-    cancelling = np.zeros(18, dtype=bool)
-    cancelling[[8, 9, 16, 17]] = True
-    assert e3[~cancelling].max() < RES_TOL and e3[cancelling].max() < RES_TOL_CANCELLING, (name, e3)
+    assert e3.max() < RES_TOL, (name, e3)
 
 
 def test_flux_sqrt_and_reciprocal_error_bound(api):
