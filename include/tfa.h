@@ -165,6 +165,14 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
  * synchronises.  Pinned host memory makes the copies asynchronous DMA; pageable memory works. */
 int tfa_assemble_host(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                       const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream);
+/* The two kernels of tfa_assemble as separate calls, for callers that put something between them (the face-state
+ * halo exchange of a sharded assembly, below): tfa_assemble_gradient runs step a2 and leaves the reconstructed
+ * face states in the context; tfa_face_states returns that buffer ([n_cells][F][18] FP64, DEVICE pointer owned by
+ * the context, valid until the context meets another mesh); tfa_assemble_faces runs steps a3..a7 on it. */
+int tfa_assemble_gradient(tfa_ctx* ctx, const tfa_mesh* m, const double* state, void* stream);
+int tfa_assemble_faces(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                       const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream);
+double* tfa_face_states(tfa_ctx* ctx);
 /* Synchronise and report: 0, or TFA_ENONPHYS if any assembly since the last check met a face
  * state with rho <= 0 or T <= 0 (S16), or TFA_ECUDA for a sticky CUDA error. */
 int tfa_check(tfa_ctx* ctx, void* stream);
@@ -214,6 +222,53 @@ int tfa_jvp(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* 
 int tfa_gmres_jfnk(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                    const double* state_nm1, double dt, const double* dinv, const double* b, double* x, int restart,
                    int max_iters, double rtol, double* info, void* stream);
+
+/* ---- sharding over several GPUs (device memory is the limit the paper names, L26) ----
+ * Rank r of n owns the cells [r nc / n, (r+1) nc / n) of the global mesh's current order (reorder it first), their
+ * rows of rhs and of the BSR matrix, and keeps ghost copies of the cells its reconstruction stencils reach.  Local
+ * cell ids are ascending in global id: ghosts below the owned range, the owned range [first_owned_local,
+ * first_owned_local + n_owned), ghosts above; an owned row comes out bit-identical to the single-GPU assembly.
+ * One assembly = two neighbour-only exchanges, no reduction (the caller moves the packed buffers, e.g. with NCCL
+ * send/recv; api.py does):
+ *     exchange TFA_HALO_STATE on the state arrays          (18 doubles per ghost cell)
+ *     tfa_assemble_gradient(ctx, tfa_shard_mesh(s), state)
+ *     exchange TFA_HALO_FACE on tfa_face_states(ctx)       (F x 18 doubles per ghost cell next to an owned cell)
+ *     tfa_assemble_faces(ctx, tfa_shard_mesh(s), ..., rhs, vals)
+ * rhs has n_local rows (ghost rows are scratch); vals has nnzb_owned blocks: the owned rows of the local mesh's
+ * pattern, i.e. blocks [block_offset, block_offset + nnzb_owned) of it (rowptr / col: the local mesh's
+ * TFA_BSR_ROWPTR entries first_owned_local .. minus block_offset, TFA_BSR_COL from block_offset on; columns are
+ * LOCAL cell ids).  Boundary rules are taken over from the global mesh at creation; do not call tfa_mesh_set_bc
+ * on the shard's mesh.  Ghost states: row b of the context's array belongs to the LOCAL boundary face b, whose
+ * global boundary-face index (or -1 for a cut face) tfa_shard_bface_global gives.
+ *
+ * tfa_partition_* is the host-only half (no CUDA call): the same lists from HOST copies of the global mesh's
+ * TFA_CELL_NBR, TFA_STENCIL_PTR, TFA_STENCIL_IDX.  Lists hold LOCAL cell ids in ascending global id, so that the
+ * sender's TFA_PART_SEND_* list for a peer and that peer's TFA_PART_RECV_* list for the sender name the same
+ * cells in the same order. */
+typedef struct tfa_partition tfa_partition;
+typedef struct tfa_shard tfa_shard;
+enum { TFA_PART_LOCAL_TO_GLOBAL = 0, TFA_PART_SEND_STATE = 1, TFA_PART_RECV_STATE = 2, TFA_PART_SEND_FACE = 3,
+       TFA_PART_RECV_FACE = 4 };
+enum { TFA_HALO_STATE = 0, TFA_HALO_FACE = 1 };
+int  tfa_partition_create(tfa_partition** out, int64_t n_cells, int max_faces, const int32_t* cell_nbr,
+                          const int32_t* stencil_ptr, const int32_t* stencil_idx, int n_ranks, int rank);
+void tfa_partition_destroy(tfa_partition* p);
+int  tfa_partition_sizes(const tfa_partition* p, int64_t* n_local, int64_t* n_owned, int64_t* first_owned_local,
+                         int64_t* first_owned_global);
+/* number of entries of a list (peer ignored for TFA_PART_LOCAL_TO_GLOBAL), -1 on a bad argument */
+int64_t tfa_partition_count(const tfa_partition* p, int which, int peer);
+int  tfa_partition_get(const tfa_partition* p, int which, int peer, int32_t* host_dst, int64_t count);
+/* Build rank `rank`'s shard from the global mesh (which every rank builds for itself and may destroy afterwards). */
+int  tfa_shard_create(tfa_shard** out, const tfa_mesh* global_mesh, int n_ranks, int rank, void* stream);
+void tfa_shard_destroy(tfa_shard* s);
+const tfa_mesh* tfa_shard_mesh(const tfa_shard* s);             /* owned by the shard */
+const tfa_partition* tfa_shard_partition(const tfa_shard* s);   /* owned by the shard */
+int  tfa_shard_info(const tfa_shard* s, int64_t* nnzb_owned, int64_t* block_offset);
+int  tfa_shard_bface_global(const tfa_shard* s, int32_t* host_dst, int64_t count /* = local n_bfaces */);
+/* buf[r] = row (send list of `peer`)[r] of src;  row (recv list of `peer`)[r] of dst = buf[r].  Rows are 18 doubles
+ * (TFA_HALO_STATE) or F x 18 doubles (TFA_HALO_FACE).  DEVICE pointers, asynchronous on `stream`. */
+int  tfa_shard_pack(const tfa_shard* s, int kind, int peer, const double* src, double* buf, void* stream);
+int  tfa_shard_unpack(const tfa_shard* s, int kind, int peer, const double* buf, double* dst, void* stream);
 
 /* Per-kernel timing with CUDA events recorded on the launching stream (bench.py's roofline).
  * tfa_timing_enable(ctx, 1): every later tfa_assemble records events before, between and after

@@ -129,6 +129,10 @@ def num_threads() -> int:
     return int(lib().tfo_num_threads())
 
 
+def set_num_threads(n: int):
+    lib().tfo_set_num_threads(C.c_int(int(n)))
+
+
 class OracleMesh:
     def __init__(self, node_xy, cell_nodes, cell_xy=None, cell_ptr=None):
         """Triangles: cell_nodes [nc][3].  Mixed triangles / quadrilaterals: cell_ptr [nc+1] and flat cell_nodes,

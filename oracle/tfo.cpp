@@ -690,6 +690,14 @@ int tfo_num_threads(void) {
 #endif
 }
 
+void tfo_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
 void tfo_default_physics(tfo_physics* p) {
   p->gamma_gas = 5.0 / 3.0;
   p->mass_ratio = 25.0;

@@ -132,6 +132,7 @@ void tfo_dcons_dprim(const tfo_physics* ph, const double* P18, double* dUdP /*[1
 /* AUSM+-up split functions: out = {M4+(M), M4-(M), P5+(M), P5-(M)} */
 void tfo_ausm_split(double M, double alpha, double beta, double* out4);
 int  tfo_num_threads(void);
+void tfo_set_num_threads(int n);   /* size of the OpenMP team of later calls (bench.py's one-thread timing) */
 const char* tfo_last_error(void);
 
 #ifdef __cplusplus

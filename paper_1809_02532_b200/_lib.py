@@ -52,6 +52,22 @@ SYMBOLS = {
     "tfa_gradients": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "tfa_assemble": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "tfa_assemble_host": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
+    "tfa_assemble_gradient": (_int, [_vp, _vp, _vp, _vp]),
+    "tfa_assemble_faces": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
+    "tfa_face_states": (_vp, [_vp]),
+    "tfa_partition_create": (_int, [C.POINTER(_vp), _i64, _int, _vp, _vp, _vp, _int, _int]),
+    "tfa_partition_destroy": (None, [_vp]),
+    "tfa_partition_sizes": (_int, [_vp] + [C.POINTER(_i64)] * 4),
+    "tfa_partition_count": (_i64, [_vp, _int, _int]),
+    "tfa_partition_get": (_int, [_vp, _int, _int, _vp, _i64]),
+    "tfa_shard_create": (_int, [C.POINTER(_vp), _vp, _int, _int, _vp]),
+    "tfa_shard_destroy": (None, [_vp]),
+    "tfa_shard_mesh": (_vp, [_vp]),
+    "tfa_shard_partition": (_vp, [_vp]),
+    "tfa_shard_info": (_int, [_vp, C.POINTER(_i64), C.POINTER(_i64)]),
+    "tfa_shard_bface_global": (_int, [_vp, _vp, _i64]),
+    "tfa_shard_pack": (_int, [_vp, _int, _int, _vp, _vp, _vp]),
+    "tfa_shard_unpack": (_int, [_vp, _int, _int, _vp, _vp, _vp]),
     "tfa_check": (_int, [_vp, _vp]),
     "tfa_probe_dfma": (_int, [_int, _int, _vp, _vp]),
     "tfa_probe_copy": (_int, [_vp, _vp, _i64, _vp]),

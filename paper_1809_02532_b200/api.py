@@ -86,6 +86,15 @@ class Mesh:
     def from_input(cls, mi) -> "Mesh":
         return cls(mi.node_xy, mi.cell_nodes, mi.cell_xy, getattr(mi, "cell_ptr", None))
 
+    @classmethod
+    def _borrowed(cls, handle, keep_alive) -> "Mesh":
+        """View of a tfa_mesh* owned by another object (a Shard), which `keep_alive` keeps alive."""
+        m = cls.__new__(cls)
+        m._h = C.c_void_p(handle)
+        m._owner = keep_alive
+        m._sizes()
+        return m
+
     def _sizes(self):
         v = [C.c_int64() for _ in range(4)]
         _lib.check(_lib.load().tfa_mesh_sizes(self._h, *[C.byref(x) for x in v]))
@@ -125,7 +134,8 @@ class Mesh:
 
     def close(self):
         if getattr(self, "_h", None):
-            _lib.load().tfa_mesh_destroy(self._h)
+            if getattr(self, "_owner", None) is None:
+                _lib.load().tfa_mesh_destroy(self._h)
             self._h = C.c_void_p()
 
     def __del__(self):
@@ -177,6 +187,31 @@ class Context:
             vals = torch.empty((mesh.nnzb, NEQ, NEQ), dtype=torch.float64, device=state.device)
         _lib.check(_lib.load().tfa_assemble(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
                                             _dp(rhs), _dp(vals) if jacobian else None, _stream()))
+        return rhs, vals
+
+    def assemble_gradient(self, mesh: Mesh, state):
+        """tfa_assemble_gradient: step a2 only; the face states stay in the context (face_states)."""
+        _lib.check(_lib.load().tfa_assemble_gradient(self._h, mesh._h, _dp(state), _stream()))
+
+    def face_states(self, mesh: Mesh) -> torch.Tensor:
+        """tfa_face_states as a tensor view [n_cells][F][18] of the context's buffer (no copy)."""
+        ptr = _lib.load().tfa_face_states(self._h)
+        n = mesh.n_cells * mesh.max_faces * NEQ
+        if not ptr or n == 0:
+            return torch.empty((0, mesh.max_faces, NEQ), dtype=torch.float64, device="cuda")
+        iface = {"shape": (n,), "typestr": "<f8", "data": (int(ptr), False), "version": 3, "strides": None}
+        holder = type("_FaceStates", (), {"__cuda_array_interface__": iface})()
+        return torch.as_tensor(holder, device="cuda").view(mesh.n_cells, mesh.max_faces, NEQ)
+
+    def assemble_faces(self, mesh: Mesh, state, state_n=None, state_nm1=None, dt=1e-3, rhs=None, vals=None):
+        """tfa_assemble_faces: steps a3..a7 on the context's face states.  vals must be given (its size is the
+        caller's business: a shard's value array holds the owned rows only)."""
+        state_n = state if state_n is None else state_n
+        state_nm1 = state if state_nm1 is None else state_nm1
+        if rhs is None:
+            rhs = torch.empty((mesh.n_cells, NEQ), dtype=torch.float64, device=state.device)
+        _lib.check(_lib.load().tfa_assemble_faces(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
+                                                  _dp(rhs), _dp(vals), _stream()))
         return rhs, vals
 
     def assemble_host(self, mesh: Mesh, state, state_n, state_nm1, dt, rhs, vals):
@@ -259,6 +294,171 @@ class Context:
             self.close()
         except Exception:
             pass
+
+
+# ------------------------------------------------------------------------------------------------
+# sharding over several GPUs: one process per GPU, neighbour-only exchanges
+# ------------------------------------------------------------------------------------------------
+PART_LOCAL_TO_GLOBAL, PART_SEND_STATE, PART_RECV_STATE, PART_SEND_FACE, PART_RECV_FACE = range(5)
+HALO_STATE, HALO_FACE = 0, 1
+
+
+class Partition:
+    """tfa_partition_*: the host-only half of the sharding (no CUDA call): which cells a rank owns, which ghosts it
+    keeps, and the per-peer send / receive lists of the two halo exchanges."""
+
+    def __init__(self, cell_nbr=None, stencil_ptr=None, stencil_idx=None, n_ranks=1, rank=0, _handle=None, _owner=None):
+        lib = _lib.load()
+        self._owner = _owner
+        if _handle is not None:
+            self._h = C.c_void_p(_handle)
+        else:
+            nbr = np.ascontiguousarray(cell_nbr, dtype=np.int32)
+            sp = np.ascontiguousarray(stencil_ptr, dtype=np.int32)
+            si = np.ascontiguousarray(stencil_idx, dtype=np.int32)
+            self._h = C.c_void_p()
+            _lib.check(lib.tfa_partition_create(C.byref(self._h), nbr.shape[0], nbr.shape[1] if nbr.ndim == 2 else 3,
+                                                _hp(nbr), _hp(sp), _hp(si), int(n_ranks), int(rank)))
+        v = [C.c_int64() for _ in range(4)]
+        _lib.check(lib.tfa_partition_sizes(self._h, *[C.byref(x) for x in v]))
+        self.n_local, self.n_owned, self.first_owned_local, self.first_owned_global = [int(x.value) for x in v]
+        self.n_ranks, self.rank = int(n_ranks), int(rank)
+
+    def list(self, which: int, peer: int = 0) -> np.ndarray:
+        lib = _lib.load()
+        n = int(lib.tfa_partition_count(self._h, which, peer))
+        if n < 0:
+            raise ValueError("unknown list or peer")
+        out = np.empty(n, dtype=np.int32)
+        _lib.check(lib.tfa_partition_get(self._h, which, peer, _hp(out), n))
+        return out
+
+    @property
+    def local_to_global(self) -> np.ndarray:
+        return self.list(PART_LOCAL_TO_GLOBAL)
+
+    def count(self, which: int, peer: int) -> int:
+        return int(_lib.load().tfa_partition_count(self._h, which, peer))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            if self._owner is None:
+                _lib.load().tfa_partition_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def exchange_halo(part: Partition, kind: int, width: int, pack, unpack, new_buffer, group=None):
+    """One neighbour-only halo exchange over torch.distributed (NCCL send/recv on GPUs; any backend works).
+
+    pack(peer, buf) fills buf [count][width] with the rows `peer` needs; unpack(peer, buf) stores the rows received
+    from it; new_buffer(rows, width) allocates a buffer on the right device.  Only peers that share cells are
+    contacted; there is no reduction and no collective."""
+    import torch.distributed as dist
+    send_which = PART_SEND_STATE if kind == HALO_STATE else PART_SEND_FACE
+    recv_which = PART_RECV_STATE if kind == HALO_STATE else PART_RECV_FACE
+    ops, recvs = [], []
+    for peer in range(part.n_ranks):
+        if peer == part.rank:
+            continue
+        ns, nr = part.count(send_which, peer), part.count(recv_which, peer)
+        if nr:
+            rb = new_buffer(nr, width)
+            recvs.append((peer, rb))
+            ops.append(dist.P2POp(dist.irecv, rb, peer, group))
+        if ns:
+            sb = new_buffer(ns, width)
+            pack(peer, sb)
+            ops.append(dist.P2POp(dist.isend, sb, peer, group))
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+    for peer, rb in recvs:
+        unpack(peer, rb)
+
+
+class Shard:
+    """tfa_shard_*: rank `rank`'s part of a global mesh: the local mesh (owned + ghost cells), the block range of
+    the owned rows and the device-side pack / unpack of the halos."""
+
+    def __init__(self, global_mesh: Mesh, n_ranks: int, rank: int):
+        lib = _lib.load()
+        self._h = C.c_void_p()
+        _lib.check(lib.tfa_shard_create(C.byref(self._h), global_mesh._h, int(n_ranks), int(rank), _stream()))
+        self.mesh = Mesh._borrowed(lib.tfa_shard_mesh(self._h), self)
+        self.part = Partition(n_ranks=n_ranks, rank=rank, _handle=lib.tfa_shard_partition(self._h), _owner=self)
+        a, b = C.c_int64(), C.c_int64()
+        _lib.check(lib.tfa_shard_info(self._h, C.byref(a), C.byref(b)))
+        self.nnzb_owned, self.block_offset = int(a.value), int(b.value)
+        self.bface_global = np.empty(self.mesh.n_bfaces, dtype=np.int32)
+        _lib.check(lib.tfa_shard_bface_global(self._h, _hp(self.bface_global), self.mesh.n_bfaces))
+
+    def pack(self, kind: int, peer: int, src: torch.Tensor, buf: torch.Tensor):
+        _lib.check(_lib.load().tfa_shard_pack(self._h, kind, peer, _dp(src), _dp(buf), _stream()))
+
+    def unpack(self, kind: int, peer: int, buf: torch.Tensor, dst: torch.Tensor):
+        _lib.check(_lib.load().tfa_shard_unpack(self._h, kind, peer, _dp(buf), _dp(dst), _stream()))
+
+    def _width(self, kind: int) -> int:
+        return NEQ if kind == HALO_STATE else self.mesh.max_faces * NEQ
+
+    def exchange(self, kind: int, tensor: torch.Tensor, group=None):
+        """Halo exchange of `tensor` ([n_local][18] states or [n_local][F][18] face states) with the other ranks."""
+        exchange_halo(self.part, kind, self._width(kind),
+                      lambda peer, buf: self.pack(kind, peer, tensor, buf),
+                      lambda peer, buf: self.unpack(kind, peer, buf, tensor),
+                      lambda n, w: torch.empty((n, w), dtype=torch.float64, device=tensor.device), group)
+
+    def owned_bsr_pattern(self):
+        """(rowptr [n_owned + 1], col [nnzb_owned]) of the owned rows; columns are local cell ids."""
+        rp = self.mesh.get("bsr_rowptr")
+        o0 = self.part.first_owned_local
+        return (rp[o0:o0 + self.part.n_owned + 1] - self.block_offset,
+                self.mesh.get("bsr_col")[self.block_offset:self.block_offset + self.nnzb_owned])
+
+    def assemble(self, ctx: Context, state, state_n=None, state_nm1=None, dt=1e-3, rhs=None, vals=None, exchange=None):
+        """One sharded assembly (include/tfa.h): state halo, gradient kernel, face-state halo, flux / Jacobian
+        kernel.  `exchange(kind, tensor)` defaults to the torch.distributed exchange of this shard."""
+        exchange = exchange or self.exchange
+        if vals is None:
+            vals = torch.empty((self.nnzb_owned, NEQ, NEQ), dtype=torch.float64, device=state.device)
+        exchange(HALO_STATE, state)
+        ctx.assemble_gradient(self.mesh, state)
+        exchange(HALO_FACE, ctx.face_states(self.mesh))
+        return ctx.assemble_faces(self.mesh, state, state_n, state_nm1, dt, rhs, vals)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.mesh._h = C.c_void_p()
+            self.part._h = C.c_void_p()
+            _lib.load().tfa_shard_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def exchange_in_process(shards, kind: int, tensors):
+    """The halo exchange among shards that live in ONE process on one GPU (tests and debugging; the kernels of
+    the ranks do not wait on each other, so running them one after another is legitimate): the same pack and unpack
+    kernels, with a device buffer standing in for the wire."""
+    n = len(shards)
+    which = PART_SEND_STATE if kind == HALO_STATE else PART_SEND_FACE
+    for r in range(n):
+        for p in range(n):
+            cnt = shards[r].part.count(which, p) if p != r else 0
+            if cnt:
+                buf = torch.empty((cnt, shards[r]._width(kind)), dtype=torch.float64, device=tensors[r].device)
+                shards[r].pack(kind, p, tensors[r], buf)
+                shards[p].unpack(kind, r, buf, tensors[p])
 
 
 def probe_dfma(grid: int, iters: int, sink: torch.Tensor):

@@ -121,8 +121,11 @@ int tfa_gradients(tfa_ctx* ctx, const tfa_mesh* m, const double* state, double* 
 namespace tfa {
 // the two launches of one assembly, with optional per-kernel events (tfa_timing_enable); the matrix-free
 // operator's evaluations call it untimed, so that a long solve never exhausts the event ring
+// phases: 1 = gradient / limiter / face-state kernel only, 2 = flux / Jacobian kernel only (on the face states
+// the context holds), 3 = both
 int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
-                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed) {
+                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed,
+                  int phases = 3) {
   if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
   if (m->nc == 0) { ctx->launches = 0; return 0; }   // empty mesh: nothing to write
   if (!state || !state_n || !state_nm1 || !rhs) return set_error(TFA_EINVAL, "null argument");
@@ -141,15 +144,17 @@ int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const do
       if (!ev[q]) TFA_CUDA(cudaEventCreate(&ev[q]));
     TFA_CUDA(cudaEventRecord(ev[0], st));
   }
-  TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
+  if (phases & 1)
+    TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
+  if (phases & 2)
   TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, ctx->flags.p,
                           ctx->asm_resident_ctas, st));
   if (ev) {
     TFA_CUDA(cudaEventRecord(ev[2], st));
     ++ctx->timed;
   }
-  ctx->launches = 2;
+  ctx->launches = (phases & 1) + ((phases >> 1) & 1);
   return 0;
 }
 }  // namespace tfa
@@ -160,6 +165,25 @@ int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const dou
                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {
   return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream, true);
 }
+
+int tfa_assemble_gradient(tfa_ctx* ctx, const tfa_mesh* m, const double* state, void* stream) {
+  if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!state) return set_error(TFA_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  TFA_TRY(prepare(ctx, m, st));
+  ctx->launches = 1;
+  return launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st);
+}
+
+int tfa_assemble_faces(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                       const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {
+  if (ctx && m && ctx->ws_uid != m->uid)
+    return set_error(TFA_EINVAL, "tfa_assemble_faces: no face states of this mesh (call tfa_assemble_gradient first)");
+  return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream, false, 2);
+}
+
+double* tfa_face_states(tfa_ctx* ctx) { return ctx ? ctx->fown.p : nullptr; }
 
 int tfa_assemble_host(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                       const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {

@@ -560,7 +560,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC,
     fence_async_smem();
     cta_sync();   // B: every block of the tile is staged
     if (issuer && warp == WB) {
-      bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[lane][0], BLK * 8);
+      if (b4.x >= 0) bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[lane][0], BLK * 8);   // (-1: a shard's ghost cell)
       if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[0][lane][0], BLK * 8);
       if (NF == 4 && b5 >= 0) bulk_store(vals + (int64_t)b5 * BLK, &S.mir[1][lane][0], BLK * 8);
       bulk_commit();

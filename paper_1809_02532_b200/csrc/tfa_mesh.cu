@@ -753,9 +753,9 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
 
 using namespace tfa;
 
-namespace {
-// shared by the two builders: cells given as padded rows of F slots (host arrays)
-int create_from_padded(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells, int F,
+namespace tfa {
+// shared by the builders (and by tfa_shard_create): cells given as padded rows of F slots (host arrays)
+int create_mesh_from_padded(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells, int F,
                        const int32_t* cell_nodes, const double* cell_xy, cudaStream_t st) {
   tfa_mesh* m = new (std::nothrow) tfa_mesh;
   if (!m) return set_error(TFA_ENOMEM, "host allocation failed");
@@ -791,7 +791,7 @@ int create_from_padded(tfa_mesh** out, int64_t n_nodes, const double* node_xy, i
   *out = m;
   return 0;
 }
-}  // namespace
+}  // namespace tfa
 
 extern "C" {
 
@@ -802,7 +802,7 @@ int tfa_mesh_create(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int6
                     const int32_t* cell_nodes, const double* cell_xy, void* stream) {
   if (!out || n_nodes < 0 || n_cells < 0 || (n_cells > 0 && !cell_nodes) || (!node_xy && !cell_xy && n_cells > 0))
     return set_error(TFA_EINVAL, "tfa_mesh_create: bad argument");
-  return create_from_padded(out, n_nodes, node_xy, n_cells, 3, cell_nodes, cell_xy, (cudaStream_t)stream);
+  return create_mesh_from_padded(out, n_nodes, node_xy, n_cells, 3, cell_nodes, cell_xy, (cudaStream_t)stream);
 }
 
 int tfa_mesh_create_poly(tfa_mesh** out, int64_t n_nodes, const double* node_xy, int64_t n_cells,
@@ -828,7 +828,7 @@ int tfa_mesh_create_poly(tfa_mesh** out, int64_t n_nodes, const double* node_xy,
       cn[slot] = cell_nodes[q];
       if (cell_xy) { cx[2 * slot] = cell_xy[2 * (size_t)q]; cx[2 * slot + 1] = cell_xy[2 * (size_t)q + 1]; }
     }
-  return create_from_padded(out, n_nodes, node_xy, n_cells, F, cn.data(), cell_xy ? cx.data() : nullptr,
+  return create_mesh_from_padded(out, n_nodes, node_xy, n_cells, F, cn.data(), cell_xy ? cx.data() : nullptr,
                             (cudaStream_t)stream);
 }
 

@@ -9,7 +9,8 @@
 
 namespace tfa {
 int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
-                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed);
+                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed,
+                  int phases = 3);
 
 constexpr int SV_CELLS = 16;              // cells per CTA: thread = (cell, scalar row)
 constexpr int SV_T = SV_CELLS * NEQ;      // 288 threads
