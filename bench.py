@@ -31,11 +31,13 @@ UNIT = "Mcells/s"
 
 
 # --------------------------------------------------------------------------------------------
-def algorithmic_bytes(nc: int, nnzb: int, nst: int, F: int = 3):
+def algorithmic_bytes(nc: int, nnzb: int, nst: int, F: int = 3, packed: bool = False):
     """compulsory HBM bytes per launch of each kernel.  F = face slots per cell (3 on
-    triangle meshes, 4 on meshes with quadrilaterals)."""
+    triangle meshes, 4 on meshes with quadrilaterals).  packed: the Jacobian in the packed form of include/tfa.h
+    (full diagonal blocks, 114 entries per off-diagonal block)."""
     bs = 4 if F == 3 else 8
-    asm = (nnzb * 18 * 18 * 8      # BSR Jacobian blocks written once
+    jac = nc * 2592 + (nnzb - nc) * 912 if packed else nnzb * 18 * 18 * 8
+    asm = (jac                     # Jacobian blocks written once
            + nc * 144 * 3          # state, state_n, state_nm1 read
            + nc * 144              # rhs written
            + nc * F * 144          # own-side face states of the cell's faces (read once; both users hit L2)
@@ -220,6 +222,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--solve", action="store_true", help="also time the linear-solve step (SpMV, block-Jacobi, GMRES)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--packed", action="store_true",
+                    help="assemble the packed Jacobian (tfa_assemble_packed) instead of the BSR one")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
@@ -268,7 +272,18 @@ def main():
     P = torch.from_numpy(state_h).cuda()
     Pn, Pnm1 = P.clone(), P.clone()
     rhs = torch.empty((nc, 18), dtype=torch.float64, device="cuda")
-    vals = torch.empty((nnzb, 18, 18), dtype=torch.float64, device="cuda")
+    if args.packed:
+        pk_diag = torch.empty((nc, 18, 18), dtype=torch.float64, device="cuda")
+        pk_offd = torch.empty((nnzb - nc, 114), dtype=torch.float64, device="cuda")
+        vals = None
+    else:
+        vals = torch.empty((nnzb, 18, 18), dtype=torch.float64, device="cuda")
+
+    def assemble_step():
+        if args.packed:
+            ctx.assemble_packed(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, diag=pk_diag, offd=pk_offd)
+        else:
+            ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
     noise = torch.empty_like(P)
     gen = torch.Generator(device="cuda").manual_seed(1000 + rank)
 
@@ -306,7 +321,7 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None   # started early: nvidia-smi takes a while to come up
     for _ in range(max(args.warmup, 3)):
         perturb()
-        ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
+        assemble_step()
     ctx.check()
     # per-kernel events ride inside the timed region (the library keeps at most 64 assemblies of them)
     inline_events = args.steps <= 64
@@ -318,7 +333,7 @@ def main():
         for a, b in pairs:
             perturb()
             a.record()
-            ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
+            assemble_step()
             b.record()
         barrier()
         total_ms = sum(a.elapsed_time(b) for a, b in pairs)
@@ -326,7 +341,7 @@ def main():
         start, end = ev(), ev()
         start.record()
         for _ in range(args.steps):
-            ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
+            assemble_step()
         end.record()
         barrier()
         total_ms = start.elapsed_time(end)
@@ -335,7 +350,7 @@ def main():
     if not inline_events:   # long runs: the per-kernel split comes from 32 further steps right after
         ctx.timing_enable(True)
         for _ in range(32):
-            ctx.assemble(mesh, P, Pn, Pnm1, wl.dt, rhs=rhs, vals=vals)
+            assemble_step()
     ms_grad, ms_asm, ncalls = ctx.timing_read()
     ctx.timing_enable(False)
     ctx.check()
@@ -345,7 +360,7 @@ def main():
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region) ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.packed:
         k_e2e = max(1, min(args.steps, 3))
         sh = [torch.from_numpy(state_h).pin_memory() for _ in range(3)]
         rhs_h = torch.empty((nc, 18), dtype=torch.float64).pin_memory()
@@ -366,7 +381,7 @@ def main():
 
     # ---- optional: the next step of the method, the linear solve on the assembled system ----
     solve = None
-    if args.solve and rank == 0:
+    if args.solve and rank == 0 and not args.packed:
         n = 18 * nc
         xv = torch.randn(n, dtype=torch.float64, device="cuda")
         yv = torch.empty_like(xv)
@@ -414,7 +429,7 @@ def main():
         return
 
     # ---- roofline of the dominant kernel (k_assemble) ----
-    asm_bytes, grad_bytes = algorithmic_bytes(nc, nnzb, nst, F)
+    asm_bytes, grad_bytes = algorithmic_bytes(nc, nnzb, nst, F, args.packed)
     sv_fused, sv_stored = survey_bytes(nc, nnzb)
     step_gbs = lambda nbytes: nbytes / (ms_per_step * 1e-3) / 1e9
     peak, peak_src = measured_peaks()
@@ -449,7 +464,9 @@ def main():
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs+outputs per step (%.1f GB) exceed the 126 MB L2; no flush needed" %
                              ((asm_bytes + grad_bytes) / 1e9),
-                       "dt": wl.dt, "reorder": wl.reorder},
+                       "dt": wl.dt, "reorder": wl.reorder,
+                       "jacobian": "packed: full diagonal blocks + 114-entry off-diagonal blocks (tfa_assemble_packed)"
+                                   if args.packed else "18x18 BSR (cuSPARSE layout)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": ctx.launches_per_assemble * args.steps,
             "roofline": roofline, "cpu_baseline": cpu_baseline, "setup": setup_ms}
     if solve is not None:

@@ -39,6 +39,8 @@ extern "C" {
 
 #define TFA_NEQ 18
 #define TFA_BLOCK (TFA_NEQ * TFA_NEQ)
+/* entries of an off-diagonal block in the packed Jacobian: its structural non-zeros, 8x8 + 5x5 + 5x5 */
+#define TFA_PACKED_BLOCK 114
 
 enum { TFA_OK = 0, TFA_EINVAL = -1, TFA_EMESH = -2, TFA_ENOMEM = -3, TFA_ECUDA = -4, TFA_ENONPHYS = -5, TFA_ESINGULAR = -6 };
 
@@ -208,6 +210,32 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
  * operator); x then holds the last completed cycle's iterate. */
 int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
               double* x, int restart, int max_iters, double rtol, double* info, void* stream);
+
+/* ---- packed Jacobian (second option) ----
+ * The flux Jacobian of a face is block diagonal -- fields 8x8, ions 5x5, electrons 5x5 (only the source couples the
+ * groups, on the diagonal block) -- so 210 of the 324 entries of every off-diagonal BSR block are structural zeros:
+ * 5040 of the 10368 bytes per cell the BSR assembly writes.  The packed form stores the same matrix in two arrays:
+ *   diag_vals [n_cells][18][18]        the diagonal blocks, full, indexed by the cell;
+ *   offd_vals [nnzb - n_cells][114]    the off-diagonal blocks in BSR order with the diagonal ones taken out (row i:
+ *                                      slots BSR_ROWPTR[i] - i ..., columns = the row's BSR_COL entries other than
+ *                                      i); per block: the 8x8 field sub-block (rows / columns 0..7), then the ion
+ *                                      5x5 (rows / columns 8, 10, 11, 12, 16), then the electron 5x5 (9, 13, 14, 15,
+ *                                      17), each row-major.
+ * tfa_assemble_packed = tfa_assemble writing that form (same arithmetic, same rhs, bit-identical entries; 5328
+ * instead of 10368 bytes of Jacobian per triangle); tfa_packed_to_bsr expands it into the mesh's BSR value array;
+ * tfa_packed_spmv, tfa_block_jacobi_packed and tfa_gmres_packed are the linear-solve entry points on it.  Not
+ * available on a shard's mesh.  All pointers DEVICE pointers. */
+int tfa_assemble_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                        const double* state_nm1, double dt, double* rhs, double* diag_vals, double* offd_vals,
+                        void* stream);
+int tfa_packed_to_bsr(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, double* bsr_vals,
+                      void* stream);
+int tfa_packed_spmv(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, const double* x, double* y,
+                    void* stream);
+int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, double* dinv, void* stream);
+int tfa_gmres_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, const double* offd_vals,
+                     const double* dinv, const double* b, double* x, int restart, int max_iters, double rtol,
+                     double* info, void* stream);
 
 /* ---- matrix-free operator (the paper's future work, L130): out = (dR~/dP) v by a forward
  * difference of the residual-only assembly, (R~(P + eps v) - R~(P)) / eps — the full dependence, gradient and

@@ -7,7 +7,10 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "liboracle_tfo.so")
+# TFO_SANITIZE=1: an AddressSanitizer + UndefinedBehaviorSanitizer build of the oracle; run the
+# CPU tests with  LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 TFO_SANITIZE=1
+_SANITIZE = os.environ.get("TFO_SANITIZE", "0") == "1"
+_SO = os.path.join(_HERE, "liboracle_tfo_san.so" if _SANITIZE else "liboracle_tfo.so")
 NEQ = 18
 
 
@@ -40,6 +43,8 @@ def build(force: bool = False) -> str:
         return _SO
     cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-fPIC",
            "-shared", "-Wall", "-o", _SO, src]
+    if _SANITIZE:
+        cmd[3:3] = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
     subprocess.run(cmd, check=True, cwd=_HERE)
     return _SO
 

@@ -52,6 +52,11 @@ SYMBOLS = {
     "tfa_gradients": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "tfa_assemble": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "tfa_assemble_host": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
+    "tfa_assemble_packed": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp, _vp]),
+    "tfa_packed_to_bsr": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "tfa_packed_spmv": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "tfa_block_jacobi_packed": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "tfa_gmres_packed": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
     "tfa_assemble_gradient": (_int, [_vp, _vp, _vp, _vp]),
     "tfa_assemble_faces": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "tfa_face_states": (_vp, [_vp]),

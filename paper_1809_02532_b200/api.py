@@ -21,6 +21,7 @@ MESH_ITEMS = dict(face_cells=(0, np.int32), cell_faces=(1, np.int32), stencil_pt
                   bfaces=(12, np.int32), bc_tags=(13, np.int32))
 _REORDER = {"none": 0, "rcm": 1, "user": 2}
 BC_TRANSMISSIVE, BC_GHOST, BC_WALL = 0, 1, 2
+PACKED_BLOCK = 114
 
 
 def _stream() -> int:
@@ -188,6 +189,34 @@ class Context:
         _lib.check(_lib.load().tfa_assemble(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
                                             _dp(rhs), _dp(vals) if jacobian else None, _stream()))
         return rhs, vals
+
+    def assemble_packed(self, mesh: Mesh, state, state_n=None, state_nm1=None, dt=1e-3, rhs=None, diag=None, offd=None):
+        """tfa_assemble_packed: returns (rhs, diag [n_cells][18][18], offd [nnzb - n_cells][114])."""
+        state_n = state if state_n is None else state_n
+        state_nm1 = state if state_nm1 is None else state_nm1
+        if rhs is None:
+            rhs = torch.empty((mesh.n_cells, NEQ), dtype=torch.float64, device=state.device)
+        if diag is None:
+            diag = torch.empty((mesh.n_cells, NEQ, NEQ), dtype=torch.float64, device=state.device)
+        if offd is None:
+            offd = torch.empty((mesh.nnzb - mesh.n_cells, PACKED_BLOCK), dtype=torch.float64, device=state.device)
+        _lib.check(_lib.load().tfa_assemble_packed(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
+                                                   _dp(rhs), _dp(diag), _dp(offd), _stream()))
+        return rhs, diag, offd
+
+    def block_jacobi_packed(self, mesh: Mesh, diag, dinv=None):
+        if dinv is None:
+            dinv = torch.empty_like(diag)
+        _lib.check(_lib.load().tfa_block_jacobi_packed(self._h, mesh._h, _dp(diag), _dp(dinv), _stream()))
+        return dinv
+
+    def gmres_packed(self, mesh: Mesh, diag, offd, b, x=None, dinv=None, restart=30, max_iters=300, rtol=1e-8):
+        if x is None:
+            x = torch.zeros_like(b)
+        info = (C.c_double * 2)()
+        _lib.check(_lib.load().tfa_gmres_packed(self._h, mesh._h, _dp(diag), _dp(offd), _dp(dinv), _dp(b), _dp(x),
+                                                int(restart), int(max_iters), float(rtol), info, _stream()))
+        return x, int(info[0]), float(info[1])
 
     def assemble_gradient(self, mesh: Mesh, state):
         """tfa_assemble_gradient: step a2 only; the face states stay in the context (face_states)."""
@@ -477,6 +506,22 @@ def probe_math(x: torch.Tensor):
     s, r = torch.empty_like(x), torch.empty_like(x)
     _lib.check(_lib.load().tfa_probe_math(_dp(x), _dp(s), _dp(r), x.numel(), _stream()))
     return s, r
+
+
+def packed_spmv(mesh: Mesh, diag, offd, x, y=None):
+    """tfa_packed_spmv: y = A x on the packed Jacobian."""
+    if y is None:
+        y = torch.empty_like(x)
+    _lib.check(_lib.load().tfa_packed_spmv(mesh._h, _dp(diag), _dp(offd), _dp(x), _dp(y), _stream()))
+    return y
+
+
+def packed_to_bsr(mesh: Mesh, diag, offd, vals=None):
+    """tfa_packed_to_bsr: the packed Jacobian expanded into the mesh's BSR value array."""
+    if vals is None:
+        vals = torch.empty((mesh.nnzb, NEQ, NEQ), dtype=torch.float64, device=diag.device)
+    _lib.check(_lib.load().tfa_packed_to_bsr(mesh._h, _dp(diag), _dp(offd), _dp(vals), _stream()))
+    return vals
 
 
 def bsr_spmv(mesh: Mesh, vals: torch.Tensor, x: torch.Tensor, y: torch.Tensor | None = None):

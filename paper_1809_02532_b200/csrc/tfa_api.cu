@@ -10,7 +10,7 @@ int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, 
                     double* grad, double* phi, cudaStream_t st);
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
                     const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs,
-                    double* vals, int32_t* flags, int* resident_ctas, cudaStream_t st);
+                    double* vals, double* vals_o, int32_t* flags, int* resident_ctas, cudaStream_t st);
 int launch_probe_dfma(int grid, int iters, double* sink, cudaStream_t st);
 int launch_probe_copy(const double* src, double* dst, int64_t n, cudaStream_t st);
 int launch_probe_math(const double* x, double* s, double* r, int64_t n, cudaStream_t st);
@@ -125,7 +125,7 @@ namespace tfa {
 // the context holds), 3 = both
 int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                   const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed,
-                  int phases = 3) {
+                  int phases = 3, double* offd_vals = nullptr) {
   if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
   if (m->nc == 0) { ctx->launches = 0; return 0; }   // empty mesh: nothing to write
   if (!state || !state_n || !state_nm1 || !rhs) return set_error(TFA_EINVAL, "null argument");
@@ -148,8 +148,8 @@ int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const do
     TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
   if (phases & 2)
-  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, ctx->flags.p,
-                          ctx->asm_resident_ctas, st));
+  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, offd_vals,
+                          ctx->flags.p, ctx->asm_resident_ctas, st));
   if (ev) {
     TFA_CUDA(cudaEventRecord(ev[2], st));
     ++ctx->timed;
@@ -164,6 +164,16 @@ extern "C" {
 int tfa_assemble(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                  const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream) {
   return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream, true);
+}
+
+int tfa_assemble_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                        const double* state_nm1, double dt, double* rhs, double* diag_vals, double* offd_vals,
+                        void* stream) {
+  if (m && m->nc > 0 && (!diag_vals || (!offd_vals && m->nnzb > m->nc))) return set_error(TFA_EINVAL, "null argument");
+  if (m && m->shard_local) return set_error(TFA_EINVAL, "tfa_assemble_packed: not available on a shard's mesh");
+  // (a mesh without interior faces has no off-diagonal block: any non-null pointer selects the packed kernel)
+  return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, diag_vals, stream, true, 3,
+                       offd_vals ? offd_vals : diag_vals);
 }
 
 int tfa_assemble_gradient(tfa_ctx* ctx, const tfa_mesh* m, const double* state, void* stream) {

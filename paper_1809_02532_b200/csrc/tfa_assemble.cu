@@ -42,6 +42,11 @@
 namespace tfa {
 
 constexpr int BLKP = TFA_ASM_BLKP;
+// Packed Jacobian (second option; tfa_assemble_packed): an off-diagonal block holds only its 114
+// structural non-zeros -- fields 8x8, ions 5x5, electrons 5x5, each row-major, in that order -- and the diagonal
+// blocks sit in an array of their own.  Staged 118 doubles apart (odd number of 16-byte units, as BLKP).
+constexpr int PKB = TFA_PACKED_BLOCK;   // 114
+constexpr int PKP = 118;
 
 // ------------------------------------------------------------------------------------------------
 // TMA bulk-store helpers (PTX ISA: cp.async.bulk, bulk async-groups, async proxy fence)
@@ -110,13 +115,14 @@ struct __align__(16) AsmIn {
   int32_t pad_[4 - (T * NF) % 4];   // keeps the struct a multiple of 16 bytes
 };
 
-template <int T, int NM, int NF>
+template <int T, int NM, int NF, bool PK>
 struct __align__(128) AsmSmem {
+  static constexpr int MP = PK ? PKP : BLKP;
   AsmIn<T, NF> in[2];
   uint64_t full[2];        // mbarriers: stage s has landed
   // staged blocks: a stride of BLKP doubles (16-byte multiple, odd number of 16-byte units) spreads the
   // column stores of different cells over the banks
-  double mir[NM][T][BLKP];  // mirror blocks (j,i), face k in buffer k % NM; structural zeros persist
+  double mir[NM][T][MP];    // mirror blocks (j,i), face k in buffer k % NM; structural zeros persist
   double diag[T][BLKP];     // diagonal block (i,i); structural zeros persist
   double rs[T][NEQ];     // non-flux part of R~: Omega (BDF2 term) - Omega S
   double s0[T][8];       // Lorentz-force and Joule-heating rows of S(P_i): equations 10..17
@@ -243,16 +249,20 @@ __device__ __forceinline__ void stage_inputs(AsmIn<T, NF>& in, uint64_t* bar, in
 // ------------------------------------------------------------------------------------------------
 // The tile loop of one warp role.  All roles execute the same sequence of CTA barriers.
 // ------------------------------------------------------------------------------------------------
-template <int T, int NM, int NF, int ROLE>
-__device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC, const int64_t nc, const Consts& K,
+template <int T, int NM, int NF, bool PK, int ROLE>
+__device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF, PK>& S, const bool JAC, const int64_t nc, const Consts& K,
                                           const double* __restrict__ state, const double* __restrict__ state_n,
                                           const double* __restrict__ state_nm1, const double inv2dt,
                                           const double* __restrict__ fown, const double* __restrict__ cgeo,
                                           const int32_t* __restrict__ nbrf, const int32_t* __restrict__ blkmap,
                                           const double* __restrict__ ghost, double* __restrict__ rhs,
-                                          double* __restrict__ vals, int32_t* __restrict__ flags) {
+                                          double* __restrict__ vals, double* __restrict__ vals_o,
+                                          int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
   constexpr int BS = blk_stride(NF);
+  // where a mirror block goes: the BSR value array (324 doubles per block), or the packed off-diagonal array
+  constexpr int MBLK = PK ? PKB : BLK;
+  double* __restrict__ const mvals = PK ? vals_o : vals;
   constexpr int NV = ROLE == 2 ? 8 : 5;   // variables (= rows) of the role's group
   constexpr int GL = NV + 1;              // lanes per group: base + NV perturbed
   constexpr int NG = ROLE == 2 ? 3 : 5;   // groups per warp
@@ -425,7 +435,11 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC,
     auto stage_mirror = [&](const int buf, const double* __restrict__ d, const bool bnd) {
       if (JAC && pert && act && !bnd) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) S.mir[buf][cl][vx(q) * NEQ + v] = -d[q];
+        for (int q = 0; q < NV; ++q) {
+          // packed: entry (row q, column pj) of the group's dense sub-block; BSR: entry (vx(q), v) of the 18 x 18 block
+          const int e = PK ? (ROLE == 2 ? 8 * q + pj : 64 + 25 * SPC + 5 * q + pj) : vx(q) * NEQ + v;
+          S.mir[buf][cl][e] = -d[q];
+        }
       }
     };
     static_assert(NM == 2, "the barrier sequence below is written for two mirror buffers");
@@ -455,8 +469,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC,
     cta_sync();   // 1
     // a7: each block leaves the SM as one 2592-byte bulk store
     if (issuer && warp == 0) {
-      if (b4.y >= 0) bulk_store(vals + (int64_t)b4.y * BLK, &S.mir[0][lane][0], BLK * 8);
-      if (b4.z >= 0) bulk_store(vals + (int64_t)b4.z * BLK, &S.mir[1][lane][0], BLK * 8);
+      if (b4.y >= 0) bulk_store(mvals + (int64_t)b4.y * MBLK, &S.mir[0][lane][0], MBLK * 8);
+      if (b4.z >= 0) bulk_store(mvals + (int64_t)b4.z * MBLK, &S.mir[1][lane][0], MBLK * 8);
       bulk_commit();
     }
     if (!EARLY2) {   // (the Maxwell lanes: while the bulk stores read the buffers)
@@ -561,8 +575,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC,
     cta_sync();   // B: every block of the tile is staged
     if (issuer && warp == WB) {
       if (b4.x >= 0) bulk_store(vals + (int64_t)b4.x * BLK, &S.diag[lane][0], BLK * 8);   // (-1: a shard's ghost cell)
-      if (b4.w >= 0) bulk_store(vals + (int64_t)b4.w * BLK, &S.mir[0][lane][0], BLK * 8);
-      if (NF == 4 && b5 >= 0) bulk_store(vals + (int64_t)b5 * BLK, &S.mir[1][lane][0], BLK * 8);
+      if (b4.w >= 0) bulk_store(mvals + (int64_t)b4.w * MBLK, &S.mir[0][lane][0], MBLK * 8);
+      if (NF == 4 && b5 >= 0) bulk_store(mvals + (int64_t)b5 * MBLK, &S.mir[1][lane][0], MBLK * 8);
       bulk_commit();
     }
   }
@@ -570,16 +584,16 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF>& S, const bool JAC,
   if (nonphys) atomicAdd(flags, 1);
 }
 
-template <int T, int NM, int NF>
+template <int T, int NM, int NF, bool PK>
 __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
     const int32_t* __restrict__ blkmap, const double* __restrict__ ghost, double* __restrict__ rhs,
-    double* __restrict__ vals, int32_t* __restrict__ flags) {
+    double* __restrict__ vals, double* __restrict__ vals_o, int32_t* __restrict__ flags) {
   using C = AsmCfg<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  AsmSmem<T, NM, NF>& S = *reinterpret_cast<AsmSmem<T, NM, NF>*>(smem_raw);
+  AsmSmem<T, NM, NF, PK>& S = *reinterpret_cast<AsmSmem<T, NM, NF, PK>*>(smem_raw);
   // (residual-only calls go to k_residual; the JAC = false path here is kept for completeness)
   const bool JAC = vals != nullptr;
   const int warp = threadIdx.x >> 5;
@@ -588,8 +602,10 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     mbar_init(&S.full[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (JAC)
-    for (int q = threadIdx.x; q < (NM + 1) * T * BLKP; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;   // mir and diag
+  if (JAC) {   // structural zeros of the staged blocks, once per CTA
+    for (int q = threadIdx.x; q < NM * T * AsmSmem<T, NM, NF, PK>::MP; q += C::NT) (&S.mir[0][0][0])[q] = 0.0;
+    for (int q = threadIdx.x; q < T * BLKP; q += C::NT) (&S.diag[0][0])[q] = 0.0;
+  }
   __syncthreads();
   if (warp == C::AW + C::MW - 1) {
     // prologue: request the inputs of this CTA's first tile
@@ -605,11 +621,11 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
   }
   __syncthreads();   // the prologue's neighbour table (plain stores) is visible
   if (warp >= C::AW)
-    role_loop<T, NM, NF, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs, vals,
-                            flags);
+    role_loop<T, NM, NF, PK, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs,
+                                vals, vals_o, flags);
   else
-    role_loop<T, NM, NF, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs, vals,
-                            flags);
+    role_loop<T, NM, NF, PK, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs,
+                                vals, vals_o, flags);
 }
 
 // ================================================================================================
@@ -681,34 +697,38 @@ __global__ void __launch_bounds__(3 * RES_CELLS) k_residual(
 
 // ================================================================================================
 namespace {
-template <int T, int NM, int NF>
+template <int T, int NM, int NF, bool PK>
 int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
               const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs, double* vals,
-              int32_t* flags, int* resident_ctas, cudaStream_t st) {
+              double* vals_o, int32_t* flags, int* resident_ctas, cudaStream_t st) {
   using C = AsmCfg<T>;
-  const int smem = (int)sizeof(AsmSmem<T, NM, NF>);
+  const int smem = (int)sizeof(AsmSmem<T, NM, NF, PK>);
   if (*resident_ctas <= 0) {   // once per context (= per device): CTAs that fit the GPU at once
-    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, NM, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    TFA_CUDA(cudaFuncSetAttribute(k_assemble<T, NM, NF, PK>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int dev = 0, occ = 0, n_sm = 0;
     TFA_CUDA(cudaGetDevice(&dev));
     TFA_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, NM, NF>, C::NT, smem));
+    TFA_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_assemble<T, NM, NF, PK>, C::NT, smem));
     if (occ < 1) return set_error(TFA_ECUDA, "k_assemble does not fit on an SM");
     *resident_ctas = n_sm * occ;
   }
   const int64_t ntiles = (m.nc + T - 1) / T;
   const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)*resident_ctas);
   const double inv2dt = 1.0 / (2.0 * dt);
-  k_assemble<T, NM, NF><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
-                                                   m.nbrf.p, m.blkmap.p, ghost, rhs, vals, flags);
+  // packed: the block map is the packed one (diagonal slot = the cell, mirror slots index the off-diagonal array)
+  k_assemble<T, NM, NF, PK><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
+                                                       m.nbrf.p, PK ? m.pblkmap.p : m.blkmap.p, ghost, rhs, vals,
+                                                       vals_o, flags);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
 }  // namespace
 
+// vals_o == NULL: vals is the BSR value array.  Else packed output: vals = diagonal blocks [nc][324], vals_o =
+// off-diagonal blocks [nnzb - nc][114].  resident_ctas: 4 slots, (F - 3) + 2 * packed.
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
                     const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs,
-                    double* vals, int32_t* flags, int* resident_ctas /*[2]: F = 3, 4*/, cudaStream_t st) {
+                    double* vals, double* vals_o, int32_t* flags, int* resident_ctas, cudaStream_t st) {
   if (m.nc == 0) return 0;
   if (!vals) {
     const double inv2dt = 1.0 / (2.0 * dt);
@@ -721,11 +741,16 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
     TFA_CUDA(cudaGetLastError());
     return 0;
   }
-  if (m.F == 3)
-    return launch_nm<TFA_ASM_T, 2, 3>(m, K, state, state_n, state_nm1, dt, fown, ghost, rhs, vals, flags,
-                                      resident_ctas, st);
-  return launch_nm<TFA_ASM_T, 2, 4>(m, K, state, state_n, state_nm1, dt, fown, ghost, rhs, vals, flags,
-                                    resident_ctas + 1, st);
+#define TFA_LAUNCH(NF_, PK_, SLOT_)                                                                              \
+  return launch_nm<TFA_ASM_T, 2, NF_, PK_>(m, K, state, state_n, state_nm1, dt, fown, ghost, rhs, vals, vals_o, \
+                                           flags, resident_ctas + SLOT_, st)
+  if (!vals_o) {
+    if (m.F == 3) TFA_LAUNCH(3, false, 0);
+    TFA_LAUNCH(4, false, 1);
+  }
+  if (m.F == 3) TFA_LAUNCH(3, true, 2);
+  TFA_LAUNCH(4, true, 3);
+#undef TFA_LAUNCH
 }
 
 }  // namespace tfa

@@ -82,6 +82,7 @@ struct tfa_mesh {
   int64_t nn = 0, nc = 0, nf = 0, nnzb = 0, nst = 0, nb = 0;
   int F = 3;                 // face slots per cell: 3 (triangles only) or 4 (some quadrilaterals)
   bool has_ghost = false;    // some boundary face carries TFA_BC_GHOST
+  bool shard_local = false;  // the local mesh of a tfa_shard: its tables are the shard's (no set_bc, no packed output)
   uint64_t uid = 0;          // process-wide monotonic stamp, new at every (re)build; ctx workspaces key on it
   tfa::DevBuf<double> node_xy;     // [nn][2]
   tfa::DevBuf<int32_t> cell_nodes; // [nc][F], -1 in the fourth slot of a triangle
@@ -95,6 +96,8 @@ struct tfa_mesh {
   tfa::DevBuf<double> st_d;                     // [nst][2] centroid displacement (S9)
   tfa::DevBuf<int32_t> bsr_rowptr, bsr_col;
   tfa::DevBuf<int32_t> blkmap;                  // [nc][blk_stride(F)]
+  tfa::DevBuf<int32_t> pblkmap;                 // the same for the packed Jacobian: [0] = the cell, [1+k] = slot of (nbr_k, i)
+                                                // in the off-diagonal array (tfa.h TFA_PACKED_BLOCK)
   tfa::DevBuf<double> cen;                      // [nc][2]
   tfa::DevBuf<double> cgeo;                     // [nc][8 F]
   tfa::DevBuf<int32_t> bfaces, bface_of, bc_tag;  // [nb], [nf], [nb]
@@ -118,7 +121,7 @@ struct tfa_ctx {
   // device staging buffers of tfa_assemble_host
   tfa::DevBuf<double> stage_state[3], stage_rhs, stage_vals;
   int launches = 0;
-  int asm_resident_ctas[2] = {0, 0};   // persistent grid of k_assemble<F = 3, 4> on this context's device (0 = not queried yet)
+  int asm_resident_ctas[4] = {0, 0, 0, 0};   // persistent grid of k_assemble<F = 3, 4> x <BSR, packed> on this context's device
   // optional per-kernel timing (tfa_timing_enable): a ring of event triples
   static constexpr int kMaxTimed = 64;
   bool timing = false;

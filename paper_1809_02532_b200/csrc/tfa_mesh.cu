@@ -331,6 +331,23 @@ __global__ void k_blkmap(int64_t nc, int F, int BS, const int32_t* __restrict__ 
   }
 }
 
+// ---- the block map of the packed Jacobian (tfa.h TFA_PACKED_BLOCK): diagonal blocks are an array of their own
+// indexed by the cell; the off-diagonal blocks keep their BSR order with the diagonal ones taken out, so block b of
+// row j sits in slot b - j - (b lies after row j's diagonal block) ----
+__global__ void k_pblkmap(int64_t nc, int F, int BS, const int32_t* __restrict__ cell_nbr,
+                          const int32_t* __restrict__ blkmap, int32_t* __restrict__ pblkmap) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  for (int q = 0; q < BS; ++q) pblkmap[BS * i + q] = -1;
+  pblkmap[BS * i] = (int32_t)i;
+  for (int k = 0; k < F; ++k) {
+    const int32_t mb = blkmap[BS * i + 1 + k];
+    if (mb < 0) continue;
+    const int64_t j = cell_nbr[F * i + k];
+    pblkmap[BS * i + 1 + k] = mb - (int32_t)j - (mb > blkmap[BS * j] ? 1 : 0);
+  }
+}
+
 // ---- packed neighbour of each local face (tfa_common.cuh): interior 4 * neighbour + the face's local index there;
 // boundary -1 - (4 * boundary-face index + tag); a triangle's fourth slot -1 ----
 __global__ void k_nbr_face(int64_t nc, int F, const int32_t* __restrict__ cell_nbr,
@@ -632,7 +649,7 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
     TFA_CUDA(cudaMemsetAsync(m.bsr_rowptr.p, 0, 4, st));
     TFA_CUDA(m.face_nodes.alloc(0)); TFA_CUDA(m.face_cells.alloc(0)); TFA_CUDA(m.cell_faces.alloc(0));
     TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.nbrf.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
-    TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0)); TFA_CUDA(m.blkmap.alloc(0));
+    TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0)); TFA_CUDA(m.blkmap.alloc(0)); TFA_CUDA(m.pblkmap.alloc(0));
     TFA_CUDA(m.bfaces.alloc(0)); TFA_CUDA(m.bface_of.alloc(0)); TFA_CUDA(m.bc_tag.alloc(0));
     m.uid = next_mesh_uid();
     return 0;
@@ -690,6 +707,8 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
   k_bsr_cols<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, F, m.cell_nbr.p, m.bsr_rowptr.p, m.bsr_col.p);
   TFA_CUDA(m.blkmap.alloc(BS * nc));
   k_blkmap<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, F, BS, m.cell_nbr.p, m.bsr_rowptr.p, m.blkmap.p);
+  TFA_CUDA(m.pblkmap.alloc(BS * nc));
+  k_pblkmap<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, F, BS, m.cell_nbr.p, m.blkmap.p, m.pblkmap.p);
 
   // vertex-neighbour stencil
   {
@@ -841,6 +860,7 @@ int tfa_mesh_info(const tfa_mesh* m, int32_t* max_faces, int64_t* n_bfaces) {
 
 int tfa_mesh_set_bc(tfa_mesh* m, const int32_t* tags, void* stream) {
   if (!m || (m->nb > 0 && !tags)) return set_error(TFA_EINVAL, "null argument");
+  if (m->shard_local) return set_error(TFA_EINVAL, "tfa_mesh_set_bc: set the rules on the global mesh before sharding");
   bool ghost = false;
   for (int64_t b = 0; b < m->nb; ++b) {
     if (tags[b] < TFA_BC_TRANSMISSIVE || tags[b] > TFA_BC_WALL) return set_error(TFA_EINVAL, "unknown boundary tag");

@@ -294,6 +294,7 @@ int tfa_shard_create(tfa_shard** out, const tfa_mesh* g, int n_ranks, int rank, 
       if (gb >= 0) { s->bface_global[b] = gb; ltags[b] = tags[gb]; }
     }
     TFA_TRY(tfa_mesh_set_bc(&m, ltags.data(), stream));
+    m.shard_local = true;
     // block offset of the owned rows, then the shard's tables
     std::vector<int32_t> rp;
     TFA_TRY(download(m.bsr_rowptr, nl + 1, rp, st));

@@ -10,7 +10,7 @@
 namespace tfa {
 int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                   const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream, bool timed,
-                  int phases = 3);
+                  int phases = 3, double* offd_vals = nullptr);
 
 constexpr int SV_CELLS = 16;              // cells per CTA: thread = (cell, scalar row)
 constexpr int SV_T = SV_CELLS * NEQ;      // 288 threads
@@ -46,6 +46,89 @@ __global__ void __launch_bounds__(SV_T) k_bsr_spmv(int64_t nc, const int32_t* __
 }
 
 // ------------------------------------------------------------------------------------------------
+// The same product on the packed Jacobian (tfa.h TFA_PACKED_BLOCK): thread (i, r) reads row r of the diagonal block
+// and, of every off-diagonal block of the row, the 8 (field rows) or 5 (species rows) entries of its group's
+// sub-block; 5328 instead of 10368 matrix bytes per triangle.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void packed_row(int r, int& base, int& n, int& c0, int& cs, int& cT) {
+  // row r of the 18-vector -> start of its sub-block row inside a packed block, the number of columns n, and the
+  // columns: fields 0..7; species s: rho 8+s, u 10+3s .. 12+3s, T 16+s
+  if (r < 8) { base = 8 * r; n = 8; c0 = 0; cs = 0; cT = 0; return; }
+  const int s = r == 9 || (r >= 13 && r <= 15) || r == 17;
+  const int q = (r == 8 + s) ? 0 : (r == 16 + s ? 4 : r - (9 + 3 * s));
+  base = 64 + 25 * s + 5 * q;
+  n = 5;
+  c0 = 8 + s;
+  cs = 10 + 3 * s;
+  cT = 16 + s;
+}
+__global__ void __launch_bounds__(SV_T) k_packed_spmv(int64_t nc, int BS, const int32_t* __restrict__ rowptr,
+                                                     const int32_t* __restrict__ col, const int32_t* __restrict__ blkmap,
+                                                     const double* __restrict__ dvals, const double* __restrict__ ovals,
+                                                     const double* __restrict__ x, double* __restrict__ y) {
+  const int r = threadIdx.x % NEQ;
+  const int64_t i = blockIdx.x * (int64_t)SV_CELLS + threadIdx.x / NEQ;
+  if (i >= nc) return;
+  double acc = 0.0;
+  {
+    const double2* __restrict__ a = reinterpret_cast<const double2*>(dvals + i * BLK + r * NEQ);
+    const double2* __restrict__ xv = reinterpret_cast<const double2*>(x + NEQ * i);
+#pragma unroll
+    for (int c = 0; c < NEQ / 2; ++c) {
+      const double2 av = a[c], xx = xv[c];
+      acc = fma(av.x, xx.x, acc);
+      acc = fma(av.y, xx.y, acc);
+    }
+  }
+  int base, n, c0, cs, cT;
+  packed_row(r, base, n, c0, cs, cT);
+  const int64_t b0 = rowptr[i], b1 = rowptr[i + 1], bd = blkmap[(int64_t)BS * i];
+  int64_t slot = b0 - i;   // the row's first off-diagonal slot
+  for (int64_t b = b0; b < b1; ++b) {
+    if (b == bd) continue;
+    const double* __restrict__ a = ovals + slot * TFA_PACKED_BLOCK + base;
+    const double* __restrict__ xj = x + NEQ * (int64_t)col[b];
+    if (n == 8) {
+#pragma unroll
+      for (int c = 0; c < 8; ++c) acc = fma(a[c], xj[c], acc);
+    } else {
+      acc = fma(a[0], xj[c0], acc);
+      acc = fma(a[1], xj[cs], acc);
+      acc = fma(a[2], xj[cs + 1], acc);
+      acc = fma(a[3], xj[cs + 2], acc);
+      acc = fma(a[4], xj[cT], acc);
+    }
+    ++slot;
+  }
+  y[NEQ * i + r] = acc;
+}
+
+// packed -> BSR: thread (block b, entry e) of the mesh's pattern
+__global__ void k_packed_to_bsr(int64_t nc, int64_t nnzb, int BS, const int32_t* __restrict__ rowptr,
+                                const int32_t* __restrict__ blkmap, const int32_t* __restrict__ row_of_block,
+                                const double* __restrict__ dvals, const double* __restrict__ ovals,
+                                double* __restrict__ vals) {
+  const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (t >= nnzb * BLK) return;
+  const int64_t b = t / BLK;
+  const int e = (int)(t - b * BLK), r = e / NEQ, c = e - NEQ * r;
+  const int64_t i = row_of_block[b], bd = blkmap[(int64_t)BS * i];
+  if (b == bd) { vals[t] = dvals[i * BLK + e]; return; }
+  const int64_t slot = b - i - (b > bd ? 1 : 0);
+  int base, n, c0, cs, cT;
+  packed_row(r, base, n, c0, cs, cT);
+  int cc = -1;   // position of column c inside the row's group, -1 outside it
+  if (n == 8) cc = c < 8 ? c : -1;
+  else cc = c == c0 ? 0 : (c == cT ? 4 : (c >= cs && c < cs + 3 ? 1 + c - cs : -1));
+  vals[t] = cc >= 0 ? ovals[slot * TFA_PACKED_BLOCK + base + cc] : 0.0;
+}
+__global__ void k_row_of_block(int64_t nc, const int32_t* __restrict__ rowptr, int32_t* __restrict__ row_of_block) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  for (int32_t b = rowptr[i]; b < rowptr[i + 1]; ++b) row_of_block[b] = (int32_t)i;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Inverse of each diagonal block: one warp per cell, Gauss-Jordan with partial pivoting.  Lane r keeps row r in
 // registers; rows are never moved (the pivot of step k is the largest |a[r][k]| among the rows not yet used,
 // p_k); the pivot row goes through a double-buffered 18-double row of shared memory, one __syncwarp per step.  With P the permutation (PA)[k] = A[p_k], the in-place result S = (PA)^-1 sits as row k in lane p_k and
@@ -62,7 +145,9 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
   if (i >= nc) return;
-  const int64_t bd = blkmap[(int64_t)BS * i];   // the diagonal block of row i (every row of the mesh's pattern has one)
+  // the diagonal block of row i (every row of the mesh's pattern has one); blkmap == NULL: vals is the packed
+  // Jacobian's array of diagonal blocks
+  const int64_t bd = blkmap ? (int64_t)blkmap[(int64_t)BS * i] : i;
   const bool has = lane < NEQ;
   double a[NEQ];
 #pragma unroll
@@ -197,6 +282,7 @@ namespace {
 struct Gm {
   const tfa_mesh* m;
   const double *vals, *dinv;
+  const double* vals_o;   // non-null: (vals, vals_o) is the packed Jacobian
   int64_t n;
   cudaStream_t st;
   double *part, *out;   // reduction scratch (device)
@@ -205,7 +291,11 @@ struct Gm {
 
   int spmv(const double* x, double* y) const {
     if (op) return op(x, y);
-    k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, vals, x, y);
+    if (vals_o)
+      k_packed_spmv<<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, blk_stride(m->F), m->bsr_rowptr.p, m->bsr_col.p,
+                                                           m->blkmap.p, vals, vals_o, x, y);
+    else
+      k_bsr_spmv<false><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, m->bsr_rowptr.p, m->bsr_col.p, vals, x, y);
     return 0;
   }
   // z = M^-1 v (block-diagonal product), or a copy without preconditioner
@@ -230,7 +320,7 @@ using namespace tfa;
 
 static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv,
                       std::function<int(const double*, double*)> op, const double* b, double* x, int restart,
-                      int max_iters, double rtol, double* info, void* stream) {
+                      int max_iters, double rtol, double* info, void* stream, const double* offd_vals = nullptr) {
   if (restart < 1 || restart > MAXK - 2 || max_iters < 0 || !(rtol >= 0.0))
     return set_error(TFA_EINVAL, "tfa_gmres: restart must be in 1..62, max_iters >= 0, rtol >= 0");
   cudaStream_t st = (cudaStream_t)stream;
@@ -241,7 +331,7 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
   double* V = ctx->krylov.p;              // V_0 .. V_mk
   double* w = V + (int64_t)(mk + 1) * n;  // work vector
   double* z = w + n;                      // preconditioned vector
-  Gm G{m, bsr_vals, dinv, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, op};
+  Gm G{m, bsr_vals, dinv, offd_vals, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, op};
 
   TFA_TRY(G.dots(1, b, n, b));
   const double bnorm = std::sqrt(G.host[0]);
@@ -373,6 +463,61 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
   return gmres_core(ctx, m, bsr_vals, dinv, nullptr, b, x, restart, max_iters, rtol, info, stream);
 }
 
+// ---- packed Jacobian (second option; include/tfa.h) ----
+int tfa_packed_spmv(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, const double* x, double* y,
+                    void* stream) {
+  if (!m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!diag_vals || !x || !y || (!offd_vals && m->nnzb > m->nc)) return set_error(TFA_EINVAL, "null argument");
+  k_packed_spmv<<<cdiv(m->nc, SV_CELLS), SV_T, 0, (cudaStream_t)stream>>>(m->nc, blk_stride(m->F), m->bsr_rowptr.p,
+                                                                        m->bsr_col.p, m->blkmap.p, diag_vals,
+                                                                        offd_vals, x, y);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_packed_to_bsr(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, double* bsr_vals,
+                      void* stream) {
+  if (!m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!diag_vals || !bsr_vals || (!offd_vals && m->nnzb > m->nc)) return set_error(TFA_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  DevBuf<int32_t> rob;
+  TFA_CUDA(rob.alloc(m->nnzb));
+  k_row_of_block<<<cdiv(m->nc, 256), 256, 0, st>>>(m->nc, m->bsr_rowptr.p, rob.p);
+  k_packed_to_bsr<<<cdiv(m->nnzb * BLK, 256), 256, 0, st>>>(m->nc, m->nnzb, blk_stride(m->F), m->bsr_rowptr.p,
+                                                          m->blkmap.p, rob.p, diag_vals, offd_vals, bsr_vals);
+  TFA_CUDA(cudaGetLastError());
+  TFA_CUDA(cudaStreamSynchronize(st));   // the block-to-row table is a temporary
+  return 0;
+}
+
+int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, double* dinv, void* stream) {
+  if (!ctx || !m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  if (!diag_vals || !dinv) return set_error(TFA_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!ctx->flags.p) {
+    TFA_CUDA(ctx->flags.alloc(4));
+    TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
+  }
+  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, nullptr, 0, diag_vals, dinv, ctx->flags.p);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
+int tfa_gmres_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, const double* offd_vals,
+                     const double* dinv, const double* b, double* x, int restart, int max_iters, double rtol,
+                     double* info, void* stream) {
+  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
+  info[0] = 0.0;
+  info[1] = 0.0;
+  if (m->nc == 0) return 0;
+  if (!diag_vals || !b || !x || (!offd_vals && m->nnzb > m->nc)) return set_error(TFA_EINVAL, "null argument");
+  return gmres_core(ctx, m, diag_vals, dinv, nullptr, b, x, restart, max_iters, rtol, info, stream,
+                    offd_vals ? offd_vals : diag_vals);
+}
+
 // ---- matrix-free operator (the paper's future work, L130) ----
 static int jvp_core(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                     const double* state_nm1, double dt, const double* rhs0, const double* v, double* out, double eps,
@@ -384,7 +529,7 @@ static int jvp_core(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const 
   double *Pp = ctx->jfnk.p, *rp = Pp + n;
   if (!(eps > 0.0)) {
     // eps = 1e-7 (1 + rms(P)) / rms(v)
-    Gm G{m, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
+    Gm G{m, nullptr, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
     TFA_TRY(G.dots(1, v, n, v));
     const double rv = std::sqrt(G.host[0] / (double)n);
     if (rv == 0.0) {
@@ -430,7 +575,7 @@ int tfa_gmres_jfnk(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const d
   if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
   // the base residual and the state's size, once per solve
   TFA_TRY(assemble_impl(ctx, m, state, state_n, state_nm1, dt, ctx->jfnk0.p, nullptr, stream, false));
-  Gm G{m, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
+  Gm G{m, nullptr, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
   TFA_TRY(G.dots(1, state, n, state));
   const double rms_state = std::sqrt(G.host[0] / (double)n);
   auto op = [=](const double* xin, double* yout) -> int {
