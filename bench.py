@@ -437,7 +437,7 @@ def main():
     grad_ms = ms_grad / max(ncalls, 1)
     achieved = asm_bytes / (asm_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "k_assemble", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(args.workload),
+                "frac": achieved / peak, "traffic": ncu_traffic(args.workload + ("+packed" if args.packed else "")),
                 "algorithmic_bytes_per_launch": asm_bytes, "kernel_ms": asm_ms, "peak_source": peak_src,
                 "kernel_share_of_step": asm_ms / ms_per_step,
                 "copy_probe_gbs_this_run": copy_gbs, "fp64_probe_tflops_this_run": fp64_tflops,

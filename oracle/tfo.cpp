@@ -878,7 +878,7 @@ int tfo_mesh_get(const tfo_mesh* m, int which, void* dst, int64_t bytes) {
     default: return fail(-1, "tfo_mesh_get: unknown item");
   }
   if (bytes != n) return fail(-1, "tfo_mesh_get: size mismatch, need " + std::to_string(n));
-  std::memcpy(dst, src, n);
+  if (n > 0) std::memcpy(dst, src, n);   // (an empty item has no storage: memcpy must not see its null pointer)
   return 0;
 }
 
