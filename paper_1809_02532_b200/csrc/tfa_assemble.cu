@@ -415,7 +415,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF, PK>& S, const bool 
         if (ROLE == 2) {
           maxwell_flux(K, own, oth, nx, ny, H);
         } else {
-          const bool ok = ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nx, ny, H);
+          const bool ok = ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K.Minf[SPC], K, own, oth, nx, ny, H);
           if (!pert && act) nonphys |= !ok;
         }
       } else {
@@ -667,7 +667,7 @@ __device__ __forceinline__ void residual_rows(const int64_t i, const Consts& K, 
         else bc_species(tag, own, nx, ny, oth);
       }
       if (ROLE == 2) maxwell_flux(K, own, oth, nx, ny, H);
-      else nonphys |= !ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K, own, oth, nx, ny, H);
+      else nonphys |= !ausm_flux(K.Rs[SPC], K.gR[SPC], K.cp[SPC], K.Minf2[SPC], K.Minf[SPC], K, own, oth, nx, ny, H);
 #pragma unroll
       for (int q = 0; q < NV; ++q) acc[q] = __dadd_rn(acc[q], __dmul_rn(H[q], len));
     }

@@ -30,7 +30,7 @@ struct Consts {
   double qm[2];            // q_s/m_s
   double gR[2];            // gamma R_s  (a^2 = gamma R T)
   double cp[2], cv[2];
-  double Minf2[2];
+  double Minf2[2], Minf[2];
   double Kp, Ku, sigma, beta16;
   double delta;
   double ref[NEQ];
@@ -54,6 +54,7 @@ __host__ inline Consts make_consts(const tfa_physics& ph, const tfa_numerics& nu
     K.cv[s] = K.Rs[s] / (ph.gamma_gas - 1.0);
     K.cp[s] = ph.gamma_gas * K.Rs[s] / (ph.gamma_gas - 1.0);
     K.Minf2[s] = nu.ausm_Minf[s] * nu.ausm_Minf[s];
+    K.Minf[s] = nu.ausm_Minf[s];
   }
   K.Kp = nu.ausm_Kp;
   K.Ku = nu.ausm_Ku;
@@ -100,13 +101,13 @@ __device__ __forceinline__ void maxwell_flux(const Consts& K, const double* L, c
 // gamma R T, a_1/2, f_a rho of a physical state, O(1e-3 .. 1e3) in the normalised units; a non-physical state
 // (rho <= 0 or T <= 0) is reported by the separate test, whatever these return.  TFA_FAST_MATH64 = 0 compiles
 // the IEEE sequences instead.
+// Error budget: the seed is good to 2^-22; one coupled Newton step squares that (2^-44), and the closing
+// correction squares it again, below the last bit; a second full step before the correction (round 1 had one) only
+// cost three FMAs on the flux's critical path.  Likewise two steps suffice for the reciprocal (2^-23 -> 2^-46 -> 2^-92).
 __device__ __forceinline__ double nsqrt(double x) {
   const double y = (double)rsqrtf((float)x);
   double g = x * y, h = 0.5 * y;
-  double r = fma(-g, h, 0.5);
-  g = fma(g, r, g);
-  h = fma(h, r, h);
-  r = fma(-g, h, 0.5);
+  const double r = fma(-g, h, 0.5);
   g = fma(g, r, g);
   h = fma(h, r, h);
   return fma(fma(-g, g, x), h, g);   // last correction: g + (x - g^2) / (2 g)
@@ -114,8 +115,6 @@ __device__ __forceinline__ double nsqrt(double x) {
 __device__ __forceinline__ double nrcp(double d) {
   double y = (double)__frcp_rn((float)d);
   double e = fma(-d, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-d, y, 1.0);
   y = fma(y, e, y);
   e = fma(-d, y, 1.0);
   return fma(y, e, y);
@@ -129,20 +128,23 @@ __device__ __forceinline__ double sel_min(double a, double b) { return a < b ? a
 // Multi-fluid AUSM+-up for one species (Eq. 10; Liou's scheme = ref. [30]; S4).
 // L, R = (rho, u, v, w, T).  Returns true if the states are physical.
 // Rs, gR, cp, Minf2: the species' constants (K.Rs[s], ...), passed in registers (warp uniform).
-__device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, double Minf2, const Consts& K,
+__device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, double Minf2, double Minf, const Consts& K,
                                           const double* L, const double* R, double nx, double ny, double* H) {
   const double rL = L[0], rR = R[0], TL = L[4], TR = R[4];
   const bool ok = (rL > 0.0) & (rR > 0.0) & (TL > 0.0) & (TR > 0.0);
   const double aL = TFA_SQRT(gR * TL), aR = TFA_SQRT(gR * TR);
   const double pL = rL * Rs * TL, pR = rR * Rs * TR;
   const double unL = L[1] * nx + L[2] * ny, unR = R[1] * nx + R[2] * ny;
-  const double HtL = cp * TL + 0.5 * (L[1] * L[1] + L[2] * L[2] + L[3] * L[3]);
-  const double HtR = cp * TR + 0.5 * (R[1] * R[1] + R[2] * R[2] + R[3] * R[3]);
   const double a12 = 0.5 * (aL + aR);
   const double ia = TFA_RCP(a12);
   const double ML = unL * ia, MR = unR * ia;
   const double Mb2 = 0.5 * (unL * unL + unR * unR) * (ia * ia);
-  const double Mo = TFA_SQRT(sel_min(1.0, sel_max(Mb2, Minf2)));
+  // M_o = sqrt(min(1, max(Mbar^2, M_inf^2))): below the cut-off it is M_inf itself (per lane, so that a result never
+  // depends on which lanes share the warp); the square root is skipped when the whole warp is below it -- every face
+  // of the GEM configurations, whose in-plane velocities vanish
+  const bool low = Mb2 <= Minf2;
+  double Mo = Minf;
+  if (!__all_sync(__activemask(), low)) Mo = low ? Minf : TFA_SQRT(sel_min(1.0, Mb2));
   const double fa = Mo * (2.0 - Mo);
   const double al16 = 3.0 * (5.0 * fa * fa - 4.0);             // 16 alpha, alpha = 3/16 (-4 + 5 fa^2)
   // split Mach numbers and pressures; for |M| >= 1:  M4+ = max(M,0), P5+ = (M > 0), etc.
@@ -160,12 +162,14 @@ __device__ __forceinline__ bool ausm_flux(double Rs, double gR, double cp, doubl
   const double mdot = a12 * M12 * (up ? rL : rR);
   const double pu = -K.Ku * P5p * P5m * rsum * (fa * a12) * (unR - unL);
   const double p12 = P5p * pL + P5m * pR + pu;
+  // the upwind side's velocity and total enthalpy H = c_p T + u^2 / 2 (only that side's is needed)
   const bool upm = mdot > 0.0;
+  const double uu = upm ? L[1] : R[1], uv = upm ? L[2] : R[2], uw = upm ? L[3] : R[3], uT = upm ? TL : TR;
   H[0] = mdot;
-  H[1] = mdot * (upm ? L[1] : R[1]) + p12 * nx;
-  H[2] = mdot * (upm ? L[2] : R[2]) + p12 * ny;
-  H[3] = mdot * (upm ? L[3] : R[3]);
-  H[4] = mdot * (upm ? HtL : HtR);
+  H[1] = mdot * uu + p12 * nx;
+  H[2] = mdot * uv + p12 * ny;
+  H[3] = mdot * uw;
+  H[4] = mdot * (cp * uT + 0.5 * (uu * uu + uv * uv + uw * uw));
   return ok;
 }
 
