@@ -3,8 +3,6 @@
 // Step-by-step restatement of the assembly of arXiv 1809.02532 in the paper's order and
 // notation.  "L<n>" = line of /root/reference/PAPER.md; "S<n>" = reading listed in DESIGN.md.
 // Shares no code with paper_1809_02532_b200/csrc.
-#include "tfo.h"
-
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
@@ -15,6 +13,12 @@
 #ifdef _OPENMP
 #include <omp.h>
 #endif
+#ifdef TFO_COUNT_OPS
+// measurement build (oracle/count_ops.py): every `double` below is the op-counting scalar of opcount.h
+#include "opcount.h"
+#define double tfo_count::real
+#endif
+#include "tfo.h"
 
 namespace {
 
@@ -689,6 +693,15 @@ int tfo_num_threads(void) {
   return 1;
 #endif
 }
+
+#ifdef TFO_COUNT_OPS
+#undef double
+// out[0..6] = additions (incl. subtractions), multiplications, divisions, square roots, pow calls, comparisons,
+// sign operations (fabs, negation) of the calling thread since the last reset
+void tfo_opcount_get(int64_t* out) { for (int q = 0; q < tfo_count::N; ++q) out[q] = tfo_count::ops[q]; }
+void tfo_opcount_reset(void) { for (int q = 0; q < tfo_count::N; ++q) tfo_count::ops[q] = 0; }
+#define double tfo_count::real
+#endif
 
 void tfo_set_num_threads(int n) {
 #ifdef _OPENMP
