@@ -7,7 +7,7 @@
 namespace tfa {
 int launch_lsq_coef(const tfa_mesh& m, double power, double* coef, cudaStream_t st);
 int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* fown,
-                    double* grad, double* phi, cudaStream_t st);
+                    double* grad, double* phi, int32_t* flags, cudaStream_t st);
 int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, const double* state_n,
                     const double* state_nm1, double dt, const double* fown, const double* ghost, double* rhs,
                     double* vals, double* vals_o, int32_t* flags, int* resident_ctas, cudaStream_t st);
@@ -113,7 +113,7 @@ int tfa_gradients(tfa_ctx* ctx, const tfa_mesh* m, const double* state, double* 
   if (!state || !grad || !phi) return set_error(TFA_EINVAL, "null argument");
   cudaStream_t st = (cudaStream_t)stream;
   TFA_TRY(prepare(ctx, m, st));
-  return launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, nullptr, grad, phi, st);
+  return launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, nullptr, grad, phi, ctx->flags.p, st);
 }
 
 }  // extern "C"
@@ -145,7 +145,7 @@ int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const do
     TFA_CUDA(cudaEventRecord(ev[0], st));
   }
   if (phases & 1)
-    TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st));
+    TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, ctx->flags.p, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
   if (phases & 2)
   TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, offd_vals,
@@ -183,7 +183,7 @@ int tfa_assemble_gradient(tfa_ctx* ctx, const tfa_mesh* m, const double* state, 
   cudaStream_t st = (cudaStream_t)stream;
   TFA_TRY(prepare(ctx, m, st));
   ctx->launches = 1;
-  return launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, st);
+  return launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, ctx->flags.p, st);
 }
 
 int tfa_assemble_faces(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
@@ -232,6 +232,7 @@ int tfa_check(tfa_ctx* ctx, void* stream) {
   if (h[0]) return set_error(TFA_ENONPHYS, "non-physical face state (rho <= 0 or T <= 0) met in " +
                                                std::to_string(h[0]) + " tiles");
   if (h[1]) return set_error(TFA_ESINGULAR, "singular diagonal block in tfa_block_jacobi: " + std::to_string(h[1]));
+  if (h[2]) return set_error(TFA_ECUDA, "bounds-checking build: " + std::to_string(h[2]) + " index violations");
   return 0;
 }
 

@@ -224,7 +224,8 @@ template <int T, int NF>
 __device__ __forceinline__ void stage_inputs(AsmIn<T, NF>& in, uint64_t* bar, int lane, const int32_t (&nfN)[2],
                                              int64_t cellN, int nN, const double* __restrict__ state,
                                              const double* __restrict__ fown, const double* __restrict__ cgeo,
-                                             const double* __restrict__ ghost) {
+                                             const double* __restrict__ ghost, int32_t* __restrict__ flags,
+                                             const Limits& lim) {
   static_assert(NF * T <= 64, "two (cell, face) pairs per lane");
   if (lane == 0)
     mbar_arrive_expect_tx(bar, (uint32_t)nN * (NF * NEQ * 8 + NF * NEQ * 8 + 8 * NF * 8 + NEQ * 8));
@@ -234,6 +235,9 @@ __device__ __forceinline__ void stage_inputs(AsmIn<T, NF>& in, uint64_t* bar, in
     if (l < NF * nN) {
       const int32_t nf = nfN[h];
       const double* src;
+      TFA_BOUND(flags, nf >= 0 ? (nf >> 2) < lim.n_cells && (nf & 3) < NF
+                               : (bc_tag_of(nf) != TFA_BC_GHOST || (ghost != nullptr && bc_face_of(nf) < lim.n_ghost)));
+      TFA_BOUND(flags, cellN >= 0 && cellN + nN <= lim.n_cells && l < NF * T);
       if (nf >= 0) src = fown + (NF * (int64_t)(nf >> 2) + (nf & 3)) * NEQ;          // the neighbour's face state
       else if (bc_tag_of(nf) == TFA_BC_GHOST) src = ghost + bc_face_of(nf) * NEQ;     // the caller's ghost state
       else src = fown + (NF * cellN + l) * NEQ;                                       // the cell's own row (S9, S24)
@@ -257,7 +261,7 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF, PK>& S, const bool 
                                           const int32_t* __restrict__ nbrf, const int32_t* __restrict__ blkmap,
                                           const double* __restrict__ ghost, double* __restrict__ rhs,
                                           double* __restrict__ vals, double* __restrict__ vals_o,
-                                          int32_t* __restrict__ flags) {
+                                          int32_t* __restrict__ flags, const Limits& lim) {
   using C = AsmCfg<T>;
   constexpr int BS = blk_stride(NF);
   // where a mirror block goes: the BSR value array (324 doubles per block), or the packed off-diagonal array
@@ -457,7 +461,8 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF, PK>& S, const bool 
     if (loader && nN > 0) {
       // request the next tile's inputs into the other stage (every read of that stage ended before the
       // previous tile's closing barrier) — here, while this Maxwell warp would wait for the AUSM warps
-      stage_inputs<T, NF>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo, ghost);
+      stage_inputs<T, NF>(S.in[(it + 1) & 1], &S.full[(it + 1) & 1], lane, nfN, cellN, nN, state, fown, cgeo, ghost, flags,
+                          lim);
     }
     // both mirror buffers and the diagonal staging are free: the previous tile's bulk stores have read
     // them.  This barrier also publishes S.rs / S.s0 of the tile.
@@ -468,6 +473,10 @@ __device__ __forceinline__ void role_loop(AsmSmem<T, NM, NF, PK>& S, const bool 
     fence_async_smem();
     cta_sync();   // 1
     // a7: each block leaves the SM as one 2592-byte bulk store
+    if (issuer) {
+      TFA_BOUND(flags, b4.x < lim.n_blocks && b4.y < lim.n_mirror_blocks && b4.z < lim.n_mirror_blocks &&
+                           b4.w < lim.n_mirror_blocks && b5 < lim.n_mirror_blocks && cell0 + lane < lim.n_cells);
+    }
     if (issuer && warp == 0) {
       if (b4.y >= 0) bulk_store(mvals + (int64_t)b4.y * MBLK, &S.mir[0][lane][0], MBLK * 8);
       if (b4.z >= 0) bulk_store(mvals + (int64_t)b4.z * MBLK, &S.mir[1][lane][0], MBLK * 8);
@@ -590,7 +599,8 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
     const int32_t* __restrict__ blkmap, const double* __restrict__ ghost, double* __restrict__ rhs,
-    double* __restrict__ vals, double* __restrict__ vals_o, int32_t* __restrict__ flags) {
+    double* __restrict__ vals, double* __restrict__ vals_o, int32_t* __restrict__ flags,
+    const __grid_constant__ Limits lim) {
   using C = AsmCfg<T>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   AsmSmem<T, NM, NF, PK>& S = *reinterpret_cast<AsmSmem<T, NM, NF, PK>*>(smem_raw);
@@ -616,16 +626,16 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
       int32_t nfF[2] = {-1, -1};
       if (lane < NF * nF) nfF[0] = nbrf[NF * cellF + lane];
       if (NF * T > 32 && lane + 32 < NF * nF) nfF[1] = nbrf[NF * cellF + lane + 32];
-      stage_inputs<T, NF>(S.in[0], &S.full[0], lane, nfF, cellF, nF, state, fown, cgeo, ghost);
+      stage_inputs<T, NF>(S.in[0], &S.full[0], lane, nfF, cellF, nF, state, fown, cgeo, ghost, flags, lim);
     }
   }
   __syncthreads();   // the prologue's neighbour table (plain stores) is visible
   if (warp >= C::AW)
     role_loop<T, NM, NF, PK, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs,
-                                vals, vals_o, flags);
+                                vals, vals_o, flags, lim);
   else
     role_loop<T, NM, NF, PK, 0>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs,
-                                vals, vals_o, flags);
+                                vals, vals_o, flags, lim);
 }
 
 // ================================================================================================
@@ -640,7 +650,7 @@ __device__ __forceinline__ void residual_rows(const int64_t i, const Consts& K, 
                                               const double inv2dt, const double* __restrict__ fown,
                                               const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
                                               const double* __restrict__ ghost, double* __restrict__ rhs,
-                                              bool& nonphys) {
+                                              bool& nonphys, int32_t* __restrict__ flags, const Limits& lim) {
   constexpr int NV = ROLE == 2 ? 8 : 5;
   constexpr int SPC = ROLE == 2 ? 0 : ROLE;
   const double* __restrict__ cg = cgeo + 8 * NF * i;
@@ -654,6 +664,8 @@ __device__ __forceinline__ void residual_rows(const int64_t i, const Consts& K, 
       const double nx = cg[8 * k], ny = cg[8 * k + 1], len = cg[8 * k + 2];
       const double* __restrict__ fo = fown + (NF * i + k) * NEQ;
       const int tag = nf < 0 ? bc_tag_of(nf) : 0;
+      TFA_BOUND(flags, nf >= 0 ? (nf >> 2) < lim.n_cells && (nf & 3) < NF
+                               : (tag != TFA_BC_GHOST || (ghost != nullptr && bc_face_of(nf) < lim.n_ghost)));
       const double* __restrict__ fx = nf >= 0 ? fown + (NF * (int64_t)(nf >> 2) + (nf & 3)) * NEQ
                                               : (tag == TFA_BC_GHOST ? ghost + bc_face_of(nf) * NEQ : fo);
       double own[NV], oth[NV], H[NV];
@@ -684,14 +696,18 @@ __global__ void __launch_bounds__(3 * RES_CELLS) k_residual(
     const int64_t nc, const __grid_constant__ Consts K, const double* __restrict__ state,
     const double* __restrict__ state_n, const double* __restrict__ state_nm1, const double inv2dt,
     const double* __restrict__ fown, const double* __restrict__ cgeo, const int32_t* __restrict__ nbrf,
-    const double* __restrict__ ghost, double* __restrict__ rhs, int32_t* __restrict__ flags) {
+    const double* __restrict__ ghost, double* __restrict__ rhs, int32_t* __restrict__ flags,
+    const __grid_constant__ Limits lim) {
   const int role = threadIdx.x >> 5;   // warp 0 ions, 1 electrons, 2 fields
   const int64_t i = blockIdx.x * (int64_t)RES_CELLS + (threadIdx.x & 31);
   if (i >= nc) return;
   bool nonphys = false;
-  if (role == 0) residual_rows<0, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys);
-  else if (role == 1) residual_rows<1, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys);
-  else residual_rows<2, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys);
+  if (role == 0)
+    residual_rows<0, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys, flags, lim);
+  else if (role == 1)
+    residual_rows<1, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys, flags, lim);
+  else
+    residual_rows<2, NF>(i, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, ghost, rhs, nonphys, flags, lim);
   if (nonphys) atomicAdd(flags, 1);
 }
 
@@ -715,10 +731,11 @@ int launch_nm(const tfa_mesh& m, const Consts& K, const double* state, const dou
   const int64_t ntiles = (m.nc + T - 1) / T;
   const unsigned grid = (unsigned)std::min<int64_t>(ntiles, (int64_t)*resident_ctas);
   const double inv2dt = 1.0 / (2.0 * dt);
+  const Limits lim{m.nc, (int64_t)m.F * m.nc, PK ? m.nc : m.nnzb, PK ? m.nnzb - m.nc : m.nnzb, m.nb, m.nst};
   // packed: the block map is the packed one (diagonal slot = the cell, mirror slots index the off-diagonal array)
   k_assemble<T, NM, NF, PK><<<grid, C::NT, smem, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown, m.cgeo.p,
                                                        m.nbrf.p, PK ? m.pblkmap.p : m.blkmap.p, ghost, rhs, vals,
-                                                       vals_o, flags);
+                                                       vals_o, flags, lim);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
@@ -732,12 +749,13 @@ int launch_assemble(const tfa_mesh& m, const Consts& K, const double* state, con
   if (m.nc == 0) return 0;
   if (!vals) {
     const double inv2dt = 1.0 / (2.0 * dt);
+    const Limits lim{m.nc, (int64_t)m.F * m.nc, 0, 0, m.nb, m.nst};
     if (m.F == 3)
       k_residual<3><<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown,
-                                                                   m.cgeo.p, m.nbrf.p, ghost, rhs, flags);
+                                                                   m.cgeo.p, m.nbrf.p, ghost, rhs, flags, lim);
     else
       k_residual<4><<<cdiv(m.nc, RES_CELLS), 3 * RES_CELLS, 0, st>>>(m.nc, K, state, state_n, state_nm1, inv2dt, fown,
-                                                                   m.cgeo.p, m.nbrf.p, ghost, rhs, flags);
+                                                                   m.cgeo.p, m.nbrf.p, ghost, rhs, flags, lim);
     TFA_CUDA(cudaGetLastError());
     return 0;
   }

@@ -31,6 +31,24 @@ uint64_t next_mesh_uid();
 
 inline unsigned cdiv(int64_t a, int64_t b) { return (unsigned)((a + b - 1) / b); }
 
+// Index limits of one assembly, for the bounds-checking build (-DTFA_DEBUG_BOUNDS: `TFA_NVCC_EXTRA=-DTFA_DEBUG_BOUNDS
+// python -m paper_1809_02532_b200.build --force`).  compute-sanitizer is closed on the GPU pool this was developed on
+// (profiles/r2_sanitizers.md); this build checks every gathered row index and every block index the per-step kernels
+// form against the sizes of the arrays they address and counts violations in flags[2], which tfa_check reports.
+struct Limits {
+  int64_t n_cells, n_face_rows, n_blocks, n_mirror_blocks, n_ghost, n_stencil;
+};
+#ifdef TFA_DEBUG_BOUNDS
+#define TFA_BOUND(flags, cond)                 \
+  do {                                         \
+    if (!(cond)) atomicAdd((flags) + 2, 1);    \
+  } while (0)
+#else
+#define TFA_BOUND(flags, cond) \
+  do {                         \
+  } while (0)
+#endif
+
 // Per-cell geometry record, 8 F doubles (F = faces per cell slot of the mesh: 3 -> 192 B, 4 -> 256 B; DESIGN.md
 // "Data layout"):
 //   for local face k = 0..F-1 at [8k .. 8k+7]:

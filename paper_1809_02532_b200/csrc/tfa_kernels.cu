@@ -55,13 +55,18 @@ template <int NF>
 __global__ void __launch_bounds__(GP_T, NF == 3 ? 4 : 3) k_gradient_limiter(
     int64_t nc, const double* __restrict__ state, const int32_t* __restrict__ st_ptr,
     const int32_t* __restrict__ st_idx, const double* __restrict__ coef, const double* __restrict__ cgeo,
-    double venkK, double* __restrict__ fown, double* __restrict__ grad_out, double* __restrict__ phi_out) {
+    double venkK, double* __restrict__ fown, double* __restrict__ grad_out, double* __restrict__ phi_out,
+    int32_t* __restrict__ flags, const __grid_constant__ Limits lim) {
   const int v = 2 * (threadIdx.x % (NEQ / 2));
   const int64_t i = blockIdx.x * (int64_t)GP_CELLS + threadIdx.x / (NEQ / 2);
   if (i >= nc) return;
   const double2 Pi = *reinterpret_cast<const double2*>(state + NEQ * i + v);
   double gx[2] = {0.0, 0.0}, gy[2] = {0.0, 0.0}, dmax[2] = {0.0, 0.0}, dmin[2] = {0.0, 0.0};
   const int32_t b = st_ptr[i], e = st_ptr[i + 1];
+  TFA_BOUND(flags, b >= 0 && b <= e && e <= lim.n_stencil);
+#ifdef TFA_DEBUG_BOUNDS
+  for (int32_t qq = b; qq < e; ++qq) TFA_BOUND(flags, st_idx[qq] >= 0 && st_idx[qq] < lim.n_cells);
+#endif
   const double2* __restrict__ coef2 = reinterpret_cast<const double2*>(coef);
   int32_t q = b;
   auto add = [&](double2 c, double2 Pj) {
@@ -176,14 +181,15 @@ int launch_lsq_coef(const tfa_mesh& m, double power, double* coef, cudaStream_t 
 }
 
 int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, double venkK, double* fown,
-                    double* grad, double* phi, cudaStream_t st) {
+                    double* grad, double* phi, int32_t* flags, cudaStream_t st) {
   if (m.nc == 0) return 0;
+  const Limits lim{m.nc, (int64_t)m.F * m.nc, m.nnzb, 0, m.nb, m.nst};
   if (m.F == 3)
     k_gradient_limiter<3><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
-                                                                venkK, fown, grad, phi);
+                                                                venkK, fown, grad, phi, flags, lim);
   else
     k_gradient_limiter<4><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
-                                                                venkK, fown, grad, phi);
+                                                                venkK, fown, grad, phi, flags, lim);
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
