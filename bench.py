@@ -46,7 +46,7 @@ def algorithmic_bytes(nc: int, nnzb: int, nst: int, F: int = 3, packed: bool = F
     grad = (nc * 144               # state read
             + nst * 4 + nst * 16   # stencil indices and least-squares coefficient vectors
             + nc * 4               # stencil row pointers
-            + nc * F * 64          # geometry record
+            + nc * (2 * F + 2) * 8 # packed geometry (face midpoint offsets, sqrt of the volume)
             + nc * F * 144)        # face states written
     return asm, grad
 

@@ -118,6 +118,8 @@ struct tfa_mesh {
                                                 // in the off-diagonal array (tfa.h TFA_PACKED_BLOCK)
   tfa::DevBuf<double> cen;                      // [nc][2]
   tfa::DevBuf<double> cgeo;                     // [nc][8 F]
+  tfa::DevBuf<double> ggeo;                     // [nc][2 F + 2]: what the gradient kernel needs of it, packed for 16-byte
+                                                // loads: (dxo, dyo) of each face, then sqrt(Omega), 0
   tfa::DevBuf<int32_t> bfaces, bface_of, bc_tag;  // [nb], [nf], [nb]
 };
 

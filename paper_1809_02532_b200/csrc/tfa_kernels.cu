@@ -54,7 +54,7 @@ constexpr int GP_T = GP_CELLS * (NEQ / 2);   // 288 threads
 template <int NF>
 __global__ void __launch_bounds__(GP_T, NF == 3 ? 4 : 3) k_gradient_limiter(
     int64_t nc, const double* __restrict__ state, const int32_t* __restrict__ st_ptr,
-    const int32_t* __restrict__ st_idx, const double* __restrict__ coef, const double* __restrict__ cgeo,
+    const int32_t* __restrict__ st_idx, const double* __restrict__ coef, const double* __restrict__ ggeo,
     double venkK, double* __restrict__ fown, double* __restrict__ grad_out, double* __restrict__ phi_out,
     int32_t* __restrict__ flags, const __grid_constant__ Limits lim) {
   const int v = 2 * (threadIdx.x % (NEQ / 2));
@@ -97,16 +97,16 @@ __global__ void __launch_bounds__(GP_T, NF == 3 ? 4 : 3) k_gradient_limiter(
   while (q + 8 <= e) batch(std::integral_constant<int, 8>{});
   if (q + 4 <= e) batch(std::integral_constant<int, 4>{});
   for (; q < e; ++q) add(coef2[q], *reinterpret_cast<const double2*>(state + NEQ * (int64_t)st_idx[q] + v));
-  // the cell's own geometry is read here, not before the walk (volatile keeps the compiler from hoisting the loads
-  // and holding 14 more registers across it)
-  const volatile double* g = cgeo + 8 * NF * i;
-  double ox[NF], oy[NF];
+  // the cell's own geometry -- face midpoint offsets and sqrt(Omega), packed for 16-byte loads (NF + 1 of them
+  // instead of 2 NF + 1 eight-byte ones: the loads of the nine lanes of a cell coincide, but each costs the warp one
+  // L1 wavefront per cell it spans) -- is read here, not before the walk (asm volatile keeps the compiler from
+  // hoisting the loads and holding the registers across it)
+  const double* g = ggeo + (2 * NF + 2) * i;
+  double ox[NF], oy[NF], sqrt_vol, unused_;
 #pragma unroll
-  for (int k = 0; k < NF; ++k) {
-    ox[k] = g[8 * k + 3];
-    oy[k] = g[8 * k + 4];
-  }
-  const double sqrt_vol = g[15];
+  for (int k = 0; k < NF; ++k)
+    asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(ox[k]), "=d"(oy[k]) : "l"(g + 2 * k));
+  asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(sqrt_vol), "=d"(unused_) : "l"(g + 2 * NF));
   const double Kh = venkK * sqrt_vol;
   const double eps2 = Kh * Kh * Kh;
   double phi[2], f[NF][2];
@@ -185,10 +185,10 @@ int launch_gradient(const tfa_mesh& m, const double* state, const double* coef, 
   if (m.nc == 0) return 0;
   const Limits lim{m.nc, (int64_t)m.F * m.nc, m.nnzb, 0, m.nb, m.nst};
   if (m.F == 3)
-    k_gradient_limiter<3><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
+    k_gradient_limiter<3><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.ggeo.p,
                                                                 venkK, fown, grad, phi, flags, lim);
   else
-    k_gradient_limiter<4><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.cgeo.p,
+    k_gradient_limiter<4><<<cdiv(m.nc, GP_CELLS), GP_T, 0, st>>>(m.nc, state, m.st_ptr.p, m.st_idx.p, coef, m.ggeo.p,
                                                                 venkK, fown, grad, phi, flags, lim);
   TFA_CUDA(cudaGetLastError());
   return 0;

@@ -376,7 +376,7 @@ __global__ void k_nbr_face(int64_t nc, int F, const int32_t* __restrict__ cell_n
 __global__ void k_cgeo(int64_t nc, int F, const int32_t* __restrict__ cell_nbr, const int32_t* __restrict__ cell_faces,
                        const double* __restrict__ vol, const double* __restrict__ olen,
                        const double* __restrict__ onrm, const double* __restrict__ ooff,
-                       double* __restrict__ cgeo) {
+                       double* __restrict__ cgeo, double* __restrict__ ggeo) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= nc) return;
   double* g = cgeo + 8 * F * i;
@@ -402,6 +402,13 @@ __global__ void k_cgeo(int64_t nc, int F, const int32_t* __restrict__ cell_nbr, 
   }
   g[7] = vol[i];
   g[15] = sqrt(vol[i]);
+  double* gg = ggeo + (2 * F + 2) * i;
+  for (int k = 0; k < F; ++k) {
+    gg[2 * k] = g[8 * k + 3];
+    gg[2 * k + 1] = g[8 * k + 4];
+  }
+  gg[2 * F] = g[15];
+  gg[2 * F + 1] = 0.0;
 }
 
 // ---- boundary faces in ascending face id (L260) ----
@@ -650,6 +657,7 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
     TFA_CUDA(m.face_nodes.alloc(0)); TFA_CUDA(m.face_cells.alloc(0)); TFA_CUDA(m.cell_faces.alloc(0));
     TFA_CUDA(m.cell_nbr.alloc(0)); TFA_CUDA(m.nbrf.alloc(0)); TFA_CUDA(m.st_idx.alloc(0)); TFA_CUDA(m.st_d.alloc(0));
     TFA_CUDA(m.bsr_col.alloc(0)); TFA_CUDA(m.cgeo.alloc(0)); TFA_CUDA(m.blkmap.alloc(0)); TFA_CUDA(m.pblkmap.alloc(0));
+    TFA_CUDA(m.ggeo.alloc(0));
     TFA_CUDA(m.bfaces.alloc(0)); TFA_CUDA(m.bface_of.alloc(0)); TFA_CUDA(m.bc_tag.alloc(0));
     m.uid = next_mesh_uid();
     return 0;
@@ -738,7 +746,9 @@ int build_mesh(tfa_mesh& m, cudaStream_t st) {
     TFA_CUDA(cudaStreamSynchronize(st));
   }
   TFA_CUDA(m.cgeo.alloc(8 * F * nc));
-  k_cgeo<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, F, m.cell_nbr.p, m.cell_faces.p, vol.p, olen.p, onrm.p, ooff.p, m.cgeo.p);
+  TFA_CUDA(m.ggeo.alloc((2 * F + 2) * nc));
+  k_cgeo<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, F, m.cell_nbr.p, m.cell_faces.p, vol.p, olen.p, onrm.p, ooff.p, m.cgeo.p,
+                                       m.ggeo.p);
 
   // boundary faces in ascending face id; faces are numbered by their node pair, so the list -- and the tags the
   // caller attached to it -- do not change when the cells are renumbered

@@ -43,16 +43,16 @@ def test_single_rank_needs_no_process_group():
 
 
 def test_algorithmic_bytes_match_design():
-    """11 596 B per interior cell for k_assemble, about 1020 B for k_gradient_limiter."""
+    """11 596 B per interior cell for k_assemble, about 890 B for k_gradient_limiter."""
     import bench
     nc, nnzb, nst = 1_000_000, 3_997_000, 12_400_000
     asm, grad = bench.algorithmic_bytes(nc, nnzb, nst)
     assert asm == nnzb * 2592 + nc * (3 * 144 + 144 + 432 + 192 + 28)
-    assert grad == nc * (144 + 4 + 192 + 432) + nst * 20
+    assert grad == nc * (144 + 4 + 64 + 432) + nst * 20
     # quadrilateral meshes: 4 face slots (576 B of face states, 256 B of geometry, 16 + 32 B of tables per cell)
     asm4, grad4 = bench.algorithmic_bytes(262144, 5 * 262144, 8 * 262144, F=4)
     assert asm4 == 5 * 262144 * 2592 + 262144 * (3 * 144 + 144 + 576 + 256 + 48)
-    assert grad4 == 262144 * (144 + 4 + 256 + 576) + 8 * 262144 * 20
+    assert grad4 == 262144 * (144 + 4 + 80 + 576) + 8 * 262144 * 20
     # packed Jacobian: full diagonal blocks, 114 entries per off-diagonal block
     asm_p, _ = bench.algorithmic_bytes(nc, nnzb, nst, packed=True)
     assert asm - asm_p == (nnzb - nc) * (2592 - 912)
