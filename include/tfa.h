@@ -211,6 +211,20 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
 int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv, const double* b,
               double* x, int restart, int max_iters, double rtol, double* info, void* stream);
 
+/* ---- one implicit time step (Eq. 12-14): Newton sub-iterations on the BDF2 pseudo-steady residual ----
+ * Repeats  assemble R~(P), dR~/dP  ->  block-Jacobi  ->  GMRES: (dR~/dP) dP = -R~  ->  P += dP   until ||dP||_2 <=
+ * newton_tol * (1 + ||P||_2) (the paper's stopping rule ||dP|| < eps, L128, made relative) or max_newton iterations,
+ * entirely on the device apart from the scalar tests.  state: P^k, on entry the initial guess (usually P^n), on
+ * return P^{n+1}; state_n, state_nm1: P^n, P^{n-1} (must not alias state).  Work arrays, DEVICE pointers owned by the
+ * caller: rhs and dP [n_cells][18], bsr_vals [nnzb][18][18], dinv [n_cells][18][18].  matrix_free != 0 solves with
+ * the matrix-free operator (tfa_gmres_jfnk; the assembled Jacobian then only feeds the preconditioner).
+ * info[0] = Newton iterations done, info[1] = ||dP||_2 / (1 + ||P||_2) of the last one, info[2] = GMRES iterations
+ * in total, info[3] = relative residual of the last linear solve.  Errors of the steps it calls are passed on. */
+int tfa_implicit_step(tfa_ctx* ctx, const tfa_mesh* m, double* state, const double* state_n, const double* state_nm1,
+                      double dt, double* rhs, double* bsr_vals, double* dinv, double* dP, int max_newton,
+                      double newton_tol, int restart, int max_iters, double rtol, int matrix_free, double* info,
+                      void* stream);
+
 /* ---- packed Jacobian (second option) ----
  * The flux Jacobian of a face is block diagonal -- fields 8x8, ions 5x5, electrons 5x5 (only the source couples the
  * groups, on the diagonal block) -- so 210 of the 324 entries of every off-diagonal BSR block are structural zeros:

@@ -80,6 +80,8 @@ SYMBOLS = {
     "tfa_bsr_spmv": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "tfa_block_jacobi": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "tfa_gmres": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
+    "tfa_implicit_step": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp, _vp, _int, _dbl, _int, _int, _dbl, _int,
+                                 C.POINTER(C.c_double), _vp]),
     "tfa_jvp": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _dbl, _vp]),
     "tfa_gmres_jfnk": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
     "tfa_timing_enable": (_int, [_vp, _int]),

@@ -273,6 +273,22 @@ class Context:
                                          int(max_iters), float(rtol), info, _stream()))
         return x, int(info[0]), float(info[1])
 
+    def implicit_step(self, mesh: Mesh, state, state_n, state_nm1, dt, work=None, max_newton=3, newton_tol=0.0,
+                      restart=30, max_iters=300, rtol=1e-8, matrix_free=False):
+        """tfa_implicit_step: Newton sub-iterations of one BDF2 step; `state` (initial guess) is updated in place to
+        P^{n+1}.  Returns (newton_iterations, last relative update, gmres_iterations, last linear residual) and the
+        work dictionary (rhs, vals, dinv, dP), which may be passed in again."""
+        if work is None:
+            f = dict(dtype=torch.float64, device=state.device)
+            work = dict(rhs=torch.empty((mesh.n_cells, NEQ), **f), vals=torch.empty((mesh.nnzb, NEQ, NEQ), **f),
+                        dinv=torch.empty((mesh.n_cells, NEQ, NEQ), **f), dP=torch.empty((mesh.n_cells, NEQ), **f))
+        info = (C.c_double * 4)()
+        _lib.check(_lib.load().tfa_implicit_step(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
+                                                 _dp(work["rhs"]), _dp(work["vals"]), _dp(work["dinv"]), _dp(work["dP"]),
+                                                 int(max_newton), float(newton_tol), int(restart), int(max_iters),
+                                                 float(rtol), int(bool(matrix_free)), info, _stream()))
+        return (int(info[0]), float(info[1]), int(info[2]), float(info[3])), work
+
     def jvp(self, mesh: Mesh, state, v, state_n=None, state_nm1=None, dt=1e-3, eps=0.0, out=None):
         """tfa_jvp: (dR~/dP) v by a forward difference of the residual (matrix-free)."""
         state_n = state if state_n is None else state_n

@@ -463,6 +463,46 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
   return gmres_core(ctx, m, bsr_vals, dinv, nullptr, b, x, restart, max_iters, rtol, info, stream);
 }
 
+// ---- one implicit time step: the Newton sub-iterations of Eq. 14 (L120-128) around the entry points above ----
+int tfa_implicit_step(tfa_ctx* ctx, const tfa_mesh* m, double* state, const double* state_n, const double* state_nm1,
+                      double dt, double* rhs, double* bsr_vals, double* dinv, double* dP, int max_newton,
+                      double newton_tol, int restart, int max_iters, double rtol, int matrix_free, double* info,
+                      void* stream) {
+  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
+  for (int q = 0; q < 4; ++q) info[q] = 0.0;
+  if (m->nc == 0) return 0;
+  if (!state || !state_n || !state_nm1 || !rhs || !bsr_vals || !dinv || !dP) return set_error(TFA_EINVAL, "null argument");
+  if (state == state_n || state == state_nm1) return set_error(TFA_EINVAL, "tfa_implicit_step: state must not alias P^n or P^{n-1}");
+  if (max_newton < 1 || !(newton_tol >= 0.0)) return set_error(TFA_EINVAL, "tfa_implicit_step: max_newton >= 1, newton_tol >= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = (int64_t)NEQ * m->nc;
+  if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
+  double gm[2];
+  for (int it = 0; it < max_newton; ++it) {
+    TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream));
+    TFA_TRY(tfa_block_jacobi(ctx, m, bsr_vals, dinv, stream));
+    TFA_CUDA(cudaMemsetAsync(dP, 0, sizeof(double) * n, st));
+    if (matrix_free)
+      TFA_TRY(tfa_gmres_jfnk(ctx, m, state, state_n, state_nm1, dt, dinv, rhs, dP, restart, max_iters, rtol, gm, stream));
+    else
+      TFA_TRY(tfa_gmres(ctx, m, bsr_vals, dinv, rhs, dP, restart, max_iters, rtol, gm, stream));
+    info[2] += gm[0];
+    info[3] = gm[1];
+    k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, dP, 1.0, state, state);   // P += dP
+    Gm G{m, nullptr, nullptr, nullptr, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, nullptr};
+    TFA_TRY(G.dots(1, dP, n, dP));
+    const double nd = std::sqrt(G.host[0]);
+    TFA_TRY(G.dots(1, state, n, state));
+    const double np = std::sqrt(G.host[0]);
+    info[0] = it + 1;
+    info[1] = nd / (1.0 + np);
+    if (!std::isfinite(nd)) return set_error(TFA_ESINGULAR, "tfa_implicit_step: the Newton update is not finite");
+    if (info[1] <= newton_tol) break;
+  }
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+
 // ---- packed Jacobian (second option; include/tfa.h) ----
 int tfa_packed_spmv(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, const double* x, double* y,
                     void* stream) {

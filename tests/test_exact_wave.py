@@ -374,6 +374,58 @@ def test_rotated_wave_on_the_papers_quadrilateral_mesh_with_the_device_solver(W)
 
 
 @pytest.mark.gpu
+def test_native_implicit_step_equals_the_loop_of_its_parts(W):
+    """tfa_implicit_step (Eq. 12-14 as one call) gives, bit for bit, what the same sequence of tfa_assemble,
+    tfa_block_jacobi, tfa_gmres and the update gives when driven from Python; it stops on the paper's ||dP|| rule;
+    and with the matrix-free operator it lands on the exact wave after one BDF2 step as the frozen-Jacobian loop does."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    c, mass_ratio, dt = 20.0, 25.0, 0.05
+    m = W.quad_mesh(32, 16, 0.0, 2.0 * np.pi, 0.0, np.pi)
+    g = api.Mesh.from_input(m)
+    ctx = api.Context(W.Physics(mass_ratio=mass_ratio, c=c))
+    x = m.centroids()[:, 0]
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Pm, Pn = dev(exact_wave(x, 0.3 - dt, c, mass_ratio)[0]), dev(exact_wave(x, 0.3, c, mass_ratio)[0])
+    # the loop of the parts
+    P = Pn.clone()
+    its = 0
+    for _ in range(4):
+        rhs, vals = ctx.assemble(g, P, Pn, Pm, dt)
+        dP, it, rel = ctx.gmres(g, vals, rhs.reshape(-1).contiguous(), dinv=ctx.block_jacobi(g, vals), restart=30,
+                                max_iters=300, rtol=1e-9)
+        its += it
+        P = P + dP.reshape(-1, 18)
+    # the one call
+    Q = Pn.clone()
+    (nit, upd, gits, rel1), work = ctx.implicit_step(g, Q, Pn, Pm, dt, max_newton=4, newton_tol=0.0, rtol=1e-9)
+    ctx.check()
+    assert nit == 4 and gits == its and torch.equal(Q, P)
+    # the stopping rule: a tolerance between the second and the third update ends it after the third
+    Q2 = Pn.clone()
+    (n1, u1, _, _), _ = ctx.implicit_step(g, Q2, Pn, Pm, dt, work=work, max_newton=1, rtol=1e-9)
+    (n2, u2, _, _), _ = ctx.implicit_step(g, Q2, Pn, Pm, dt, work=work, max_newton=1, rtol=1e-9)
+    (n3, u3, _, _), _ = ctx.implicit_step(g, Q2, Pn, Pm, dt, work=work, max_newton=1, rtol=1e-9)
+    assert u1 > u2 > u3
+    Q3 = Pn.clone()
+    (n, u, _, _), _ = ctx.implicit_step(g, Q3, Pn, Pm, dt, work=work, max_newton=10, newton_tol=0.5 * (u2 + u3), rtol=1e-9)
+    assert n == 3 and u == u3
+    # matrix-free variant: same fixed point (the exact solution at t + dt up to the truncation error)
+    Q4 = Pn.clone()
+    (n4, u4, g4, _), _ = ctx.implicit_step(g, Q4, Pn, Pm, dt, work=work, max_newton=3, rtol=1e-4, max_iters=120,
+                                           matrix_free=True)
+    Pex = exact_wave(x, 0.3 + dt, c, mass_ratio)[0]
+    change = np.abs(Pn.cpu().numpy() - Pex).max(axis=0)
+    for R in (Q, Q4):
+        err = np.abs(R.cpu().numpy() - Pex).max(axis=0)
+        assert (err[[1, 2, 11, 12]] < 0.06 * change[[1, 2, 11, 12]]).all()
+    with pytest.raises(api.TfaError):
+        ctx.implicit_step(g, Pn, Pn, Pm, dt, work=work)          # state must not alias P^n
+    ctx.check()
+
+
+@pytest.mark.gpu
 def test_newton_jfnk_contracts_faster_than_the_frozen_jacobian(W):
     """Matrix-free Newton (the paper's future work, L130) on the same BDF2 step: the operator carries the
     gradient / limiter dependence the assembled Jacobian freezes (S8), so Newton contracts much faster."""
