@@ -219,18 +219,47 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
 // ------------------------------------------------------------------------------------------------
 constexpr int RED_T = 256, RED_B = 592;
 
-// part[b][j] = sum over the CTA's share of V_j . w, j < k  (V_j = V + j * ld)
+// part[b][j] = sum over the CTA's share of V_j . w, j < k  (V_j = V + j * ld).  Eight products per pass over w,
+// 16-byte loads (n and ld are multiples of 18, hence even; the arrays are 16-byte aligned), the eight streams of a
+// thread in flight together.
 __global__ void __launch_bounds__(RED_T) k_dots(int64_t n, int k, const double* __restrict__ V, int64_t ld,
                                                const double* __restrict__ w, double* __restrict__ part) {
   __shared__ double sm[RED_T / 32];
+  const int64_t n2 = n >> 1, ld2 = ld >> 1;
+  const double2* __restrict__ w2 = reinterpret_cast<const double2*>(w);
+  const double2* __restrict__ V2 = reinterpret_cast<const double2*>(V);
+  // caller-owned vectors need not be 16-byte aligned: then one element at a time
+  const bool vec = !((reinterpret_cast<uintptr_t>(V) | reinterpret_cast<uintptr_t>(w)) & 15) && !(n & 1) && !(ld & 1);
   for (int j0 = 0; j0 < k; j0 += 8) {
     double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     const int kj = min(8, k - j0);
-    for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
-      const double we = w[e];
+    const double2* __restrict__ Vb = V2 + (int64_t)j0 * ld2;
+    if (!vec) {
+      for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
+        const double we = w[e];
 #pragma unroll
-      for (int q = 0; q < 8; ++q)
-        if (q < kj) acc[q] = fma(V[(j0 + q) * ld + e], we, acc[q]);
+        for (int q = 0; q < 8; ++q)
+          if (q < kj) acc[q] = fma(V[(j0 + q) * ld + e], we, acc[q]);
+      }
+    } else if (kj == 8) {
+      for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
+        const double2 we = w2[e];
+        double2 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) v[q] = Vb[q * ld2 + e];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = fma(v[q].y, we.y, fma(v[q].x, we.x, acc[q]));
+      }
+    } else {
+      for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
+        const double2 we = w2[e];
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          if (q < kj) {
+            const double2 v = Vb[q * ld2 + e];
+            acc[q] = fma(v.y, we.y, fma(v.x, we.x, acc[q]));
+          }
+      }
     }
     for (int q = 0; q < kj; ++q) {
       double v = acc[q];
@@ -257,16 +286,42 @@ __global__ void __launch_bounds__(32) k_dots_final(int nblocks, const double* __
   for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
   if (threadIdx.x == 0) out[j] = s;
 }
-// w -= sum_j h[j] V_j
+// w -= sum_j h[j] V_j   (16-byte accesses; four basis vectors in flight at a time)
 __global__ void __launch_bounds__(RED_T) k_sub_combination(int64_t n, int k, const double* __restrict__ V, int64_t ld,
                                                           const double* __restrict__ h, double* __restrict__ w) {
   __shared__ double hs[MAXK];
   if (threadIdx.x < k) hs[threadIdx.x] = h[threadIdx.x];
   __syncthreads();
-  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
-    double v = w[e];
-    for (int j = 0; j < k; ++j) v = fma(-hs[j], V[j * ld + e], v);
-    w[e] = v;
+  const int64_t n2 = n >> 1, ld2 = ld >> 1;
+  double2* __restrict__ w2 = reinterpret_cast<double2*>(w);
+  const double2* __restrict__ V2 = reinterpret_cast<const double2*>(V);
+  if (((reinterpret_cast<uintptr_t>(V) | reinterpret_cast<uintptr_t>(w)) & 15) || (n & 1) || (ld & 1)) {
+    for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
+      double v = w[e];
+      for (int j = 0; j < k; ++j) v = fma(-hs[j], V[j * ld + e], v);
+      w[e] = v;
+    }
+    return;
+  }
+  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
+    double2 v = w2[e];
+    int j = 0;
+    for (; j + 4 <= k; j += 4) {
+      double2 t[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) t[q] = V2[(int64_t)(j + q) * ld2 + e];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        v.x = fma(-hs[j + q], t[q].x, v.x);
+        v.y = fma(-hs[j + q], t[q].y, v.y);
+      }
+    }
+    for (; j < k; ++j) {
+      const double2 t = V2[(int64_t)j * ld2 + e];
+      v.x = fma(-hs[j], t.x, v.x);
+      v.y = fma(-hs[j], t.y, v.y);
+    }
+    w2[e] = v;
   }
 }
 // out = a * x + c * y   (y may be null with c = 0)
