@@ -148,8 +148,8 @@ int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const do
     TFA_TRY(launch_gradient(*m, state, ctx->lsq_coef.p, ctx->nu.venkat_K, ctx->fown.p, nullptr, nullptr, ctx->flags.p, st));
   if (ev) TFA_CUDA(cudaEventRecord(ev[1], st));
   if (phases & 2)
-  TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, offd_vals,
-                          ctx->flags.p, ctx->asm_resident_ctas, st));
+    TFA_TRY(launch_assemble(*m, K, state, state_n, state_nm1, dt, ctx->fown.p, ctx->ghost, rhs, bsr_vals, offd_vals,
+                            ctx->flags.p, ctx->asm_resident_ctas, st));
   if (ev) {
     TFA_CUDA(cudaEventRecord(ev[2], st));
     ++ctx->timed;
