@@ -180,6 +180,75 @@ def run_reference(args, wl):
     print(json.dumps(line), flush=True)
 
 
+def run_shards(args, wl):
+    """`--shards N` (one GPU): the sharded assembly of SURVEY 8(f)4 with its N ranks emulated one after another in
+    this process (their kernels never wait on each other; the halos go through the library's pack / unpack kernels
+    with a device buffer standing in for the wire).  Not a scaling measurement -- there is one GPU -- but the cost
+    structure of a rank: owned and ghost cells, halo volumes, and the device time of its kernels for 1/N of the problem."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    torch.cuda.set_device(0)
+    n = args.shards
+    mesh = api.Mesh.from_input(wl.mesh)
+    if wl.reorder == "rcm":
+        mesh.reorder("rcm")
+    P = np.ascontiguousarray(wl.state[mesh.get("perm")])
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    shards = [api.Shard(mesh, n, r) for r in range(n)]
+    torch.cuda.synchronize()
+    t_build = time.time() - t0
+    ctxs = [api.Context(wl.physics) for _ in shards]
+    loc = [torch.from_numpy(P[s.part.local_to_global]).cuda() for s in shards]
+    vals = [torch.empty((s.nnzb_owned, 18, 18), dtype=torch.float64, device="cuda") for s in shards]
+    rhs = [torch.empty((s.part.n_local, 18), dtype=torch.float64, device="cuda") for s in shards]
+    F = mesh.max_faces
+
+    def one_step(timers=None):
+        def lap(key, fn):
+            if timers is None:
+                return fn()
+            a, b = ev(), ev()
+            a.record(); fn(); b.record()
+            timers.setdefault(key, []).append((a, b))
+        lap("halo_state", lambda: api.exchange_in_process(shards, api.HALO_STATE, loc))
+        for r, (s, c) in enumerate(zip(shards, ctxs)):
+            lap(f"gradient_{r}", lambda: c.assemble_gradient(s.mesh, loc[r]))
+        faces = [c.face_states(s.mesh) for s, c in zip(shards, ctxs)]
+        lap("halo_face", lambda: api.exchange_in_process(shards, api.HALO_FACE, faces))
+        for r, (s, c) in enumerate(zip(shards, ctxs)):
+            lap(f"faces_{r}", lambda: c.assemble_faces(s.mesh, loc[r], loc[r], loc[r], wl.dt, rhs=rhs[r], vals=vals[r]))
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    for c in ctxs:
+        c.check()
+    timers = {}
+    for _ in range(args.steps):
+        one_step(timers)
+    torch.cuda.synchronize()
+    ms = {k: float(np.mean([a.elapsed_time(b) for a, b in v])) for k, v in timers.items()}
+    rank_ms = [ms[f"gradient_{r}"] + ms[f"faces_{r}"] for r in range(n)]
+    halo_state = [sum(s.part.count(api.PART_RECV_STATE, q) for q in range(n)) for s in shards]
+    halo_face = [sum(s.part.count(api.PART_RECV_FACE, q) for q in range(n)) for s in shards]
+    line = {"metric": METRIC, "mode": "sharded assembly, ranks emulated on one GPU (no scaling claim)", "unit": UNIT,
+            "n_gpus": 1, "shards": n, "steps": args.steps, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl_description(args.workload, wl), "n_cells": mesh.n_cells, "nnzb": mesh.nnzb},
+            "per_rank": {"owned_cells": [s.part.n_owned for s in shards],
+                         "ghost_cells": [s.part.n_local - s.part.n_owned for s in shards],
+                         "owned_blocks": [s.nnzb_owned for s in shards],
+                         "kernel_ms": rank_ms,
+                         "mcells_per_s": [s.part.n_owned / (t * 1e-3) / 1e6 for s, t in zip(shards, rank_ms)],
+                         "halo_state_bytes_received": [h * 144 for h in halo_state],
+                         "halo_face_bytes_received": [h * F * 144 for h in halo_face]},
+            "slowest_rank_ms": max(rank_ms), "sum_of_ranks_ms": sum(rank_ms),
+            "in_process_exchange_ms": {"state": ms["halo_state"], "face": ms["halo_face"],
+                                       "note": "pack + unpack kernels of all ranks, no wire"},
+            "shard_build_s": t_build}
+    print(json.dumps(line), flush=True)
+
+
 def reduce_max_over_ranks(x: float, world: int, device="cuda") -> float:
     """Replicas only: the one inter-rank step is the max of the device-timed durations."""
     if world <= 1:
@@ -222,6 +291,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--solve", action="store_true", help="also time the linear-solve step (SpMV, block-Jacobi, GMRES)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shards", type=int, default=0,
+                    help="one GPU: emulate the sharded assembly of N ranks in this process and report per-rank costs")
     ap.add_argument("--packed", action="store_true",
                     help="assemble the packed Jacobian (tfa_assemble_packed) instead of the BSR one")
     args = ap.parse_args()
@@ -234,6 +305,8 @@ def main():
     t_gen = time.time() - t_gen
     if args.impl == "reference":
         return run_reference(args, wl)
+    if args.shards > 0:
+        return run_shards(args, wl)
 
     import torch
     import torch.distributed as dist
