@@ -36,8 +36,8 @@
  *                   solution; Harris-sheet total force balance and Ampere's law (GEM set-up)
  * Unpinned (no independent value available):
  *   |A_n| vs ref. [4] of the paper (S3), AUSM+-up constants / a_1/2 choice vs COOLFluiD (S4),
- *   LS weight exponent (S12: any weight is exact on linear fields), the wall rule's choice of which member of
- *   each cleaning pair flips (S24).
+ *   LS weight exponent (S12: any weight is exact on linear fields).  (The wall rule, S24, is this library's own
+ *   definition -- the paper defines no wall -- and is pinned by the properties that define it.)
  */
 #ifndef TFO_H
 #define TFO_H
