@@ -139,7 +139,7 @@ def oracle_sample(wl, n_rows: int, steps: int, warmup: int, threads: int | None 
         oracle.set_num_threads(threads)
     om = oracle.OracleMesh.from_input(wl.mesh)
     state = wl.state
-    if wl.reorder == "rcm":
+    if wl.reorder in ("rcm", "morton"):   # the oracle has no Z-order of its own; its work per cell is the same in any order
         om.reorder("rcm")
         state = np.ascontiguousarray(state[om.get("perm")])
     ph = oracle.physics_c(wl.physics)
@@ -191,8 +191,8 @@ def run_shards(args, wl):
     torch.cuda.set_device(0)
     n = args.shards
     mesh = api.Mesh.from_input(wl.mesh)
-    if wl.reorder == "rcm":
-        mesh.reorder("rcm")
+    if wl.reorder in ("rcm", "morton"):
+        mesh.reorder(wl.reorder)
     P = np.ascontiguousarray(wl.state[mesh.get("perm")])
     ev = lambda: torch.cuda.Event(enable_timing=True)
     t0 = time.time()
@@ -271,6 +271,7 @@ def wl_description(name, wl):
             "c3": "config 3: GEM, 512x256 split quads, periodic-x",
             "c4a": "config 4 run A: GEM, 1M-cell jittered Delaunay, random cell order",
             "c4b": "config 4 run B: GEM, 1M-cell jittered Delaunay, reverse Cuthill-McKee order",
+            "c4m": "config 4's mesh in Z-order (Morton curve through the centroids; not a BASELINE run)",
             "c5": "config 5: GEM, 4M-cell jittered Delaunay, RCM order",
             "q1": "paper mesh (L559, Table 9): double current sheet, 512x512 periodic quadrilaterals",
             "q2": "paper mesh (L433, Table 4): wave, 256x128 periodic quadrilaterals",
@@ -285,7 +286,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4b", choices=["c1", "c2", "c3", "c4a", "c4b", "c5", "q1", "q2", "qm"])
+    ap.add_argument("--workload", default="c4b",
+                    choices=["c1", "c2", "c3", "c4a", "c4b", "c4m", "c5", "q1", "q2", "qm"])
     ap.add_argument("--scale", type=float, default=1.0, help="linear lattice scale (tests only)")
     ap.add_argument("--cpu-rows", type=int, default=200000, help="rows of the oracle's timed sample")
     ap.add_argument("--no-e2e", action="store_true")
@@ -331,8 +333,8 @@ def main():
     e0.record()
     mesh = api.Mesh.from_input(wl.mesh)
     e1.record()
-    if wl.reorder == "rcm":
-        mesh.reorder("rcm")
+    if wl.reorder in ("rcm", "morton"):
+        mesh.reorder(wl.reorder)
     e2.record()
     torch.cuda.synchronize()
     setup_ms = {"mesh_create_ms": e0.elapsed_time(e1), "reorder_ms": e1.elapsed_time(e2), "generate_s": t_gen}

@@ -124,7 +124,11 @@ int tfa_mesh_set_bc(tfa_mesh* m, const int32_t* tags, void* stream);
 /* Renumber the cells for locality and rebuild every derived array under the same rules.
  * kind 0: none; 1: reverse Cuthill-McKee on the face-neighbour graph, computed on the device
  * (S11: start = unvisited cell of minimum (degree, id); neighbours appended by (degree, id));
- * 2: user_perm[new] = old (HOST pointer, must be a bijection).  Permutations compose into PERM. */
+ * 2: user_perm[new] = old (HOST pointer, must be a bijection); 3: Z-order (Morton) curve through the cell centroids
+ * (16 bits per axis over the centroids' bounding box, ties by cell id), computed on the device: consecutive cells form
+ * compact patches, which the gather-bound gradient kernel likes better than RCM's level sets.  The
+ * centroids are the cells' own (unwrapped) ones, so on a periodic mesh the curve does not wrap either.
+ * Permutations compose into PERM. */
 int tfa_mesh_reorder(tfa_mesh* m, int kind, const int32_t* user_perm, void* stream);
 int tfa_mesh_sizes(const tfa_mesh* m, int64_t* n_cells, int64_t* n_faces, int64_t* nnzb,
                    int64_t* n_stencil);

@@ -19,7 +19,7 @@ MESH_ITEMS = dict(face_cells=(0, np.int32), cell_faces=(1, np.int32), stencil_pt
                   perm=(6, np.int32), volume=(7, np.float64), face_normal_len=(8, np.float64),
                   centroid=(9, np.float64), face_nodes=(10, np.int32), cell_nbr=(11, np.int32),
                   bfaces=(12, np.int32), bc_tags=(13, np.int32))
-_REORDER = {"none": 0, "rcm": 1, "user": 2}
+_REORDER = {"none": 0, "rcm": 1, "user": 2, "morton": 3}
 BC_TRANSMISSIVE, BC_GHOST, BC_WALL = 0, 1, 2
 PACKED_BLOCK = 114
 

@@ -527,6 +527,44 @@ __global__ void __launch_bounds__(RCM_T) k_rcm(int32_t nc, int F, const int32_t*
   }
 }
 
+// ---- Z-order (Morton) curve through the cell centroids: an ordering whose consecutive cells form compact patches,
+// so that the cells of one CTA share most of their stencils (tfa_mesh_reorder kind 3) ----
+__device__ __forceinline__ unsigned long long ordered_bits(double x) {   // monotone map double -> uint64
+  const unsigned long long u = (unsigned long long)__double_as_longlong(x);
+  return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double from_ordered_bits(unsigned long long u) {
+  return __longlong_as_double((long long)((u >> 63) ? (u & 0x7fffffffffffffffull) : ~u));
+}
+__global__ void k_bbox(int64_t nc, const double* __restrict__ cen, unsigned long long* __restrict__ box) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  atomicMin(box + 0, ordered_bits(cen[2 * i]));
+  atomicMax(box + 1, ordered_bits(cen[2 * i]));
+  atomicMin(box + 2, ordered_bits(cen[2 * i + 1]));
+  atomicMax(box + 3, ordered_bits(cen[2 * i + 1]));
+}
+__device__ __forceinline__ unsigned spread16(unsigned v) {   // abcd -> 0a0b0c0d
+  v = (v | (v << 8)) & 0x00ff00ffu;
+  v = (v | (v << 4)) & 0x0f0f0f0fu;
+  v = (v | (v << 2)) & 0x33333333u;
+  v = (v | (v << 1)) & 0x55555555u;
+  return v;
+}
+__global__ void k_morton_keys(int64_t nc, const double* __restrict__ cen, const unsigned long long* __restrict__ box,
+                              uint64_t* __restrict__ keys, int32_t* __restrict__ vals) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nc) return;
+  const double x0 = from_ordered_bits(box[0]), x1 = from_ordered_bits(box[1]);
+  const double y0 = from_ordered_bits(box[2]), y1 = from_ordered_bits(box[3]);
+  const double sx = x1 > x0 ? 65535.0 / (x1 - x0) : 0.0, sy = y1 > y0 ? 65535.0 / (y1 - y0) : 0.0;
+  const unsigned qx = (unsigned)min(65535.0, max(0.0, (cen[2 * i] - x0) * sx));
+  const unsigned qy = (unsigned)min(65535.0, max(0.0, (cen[2 * i + 1] - y0) * sy));
+  // ties (cells in one quantisation box) are broken by the cell id: the order is unique
+  keys[i] = ((uint64_t)(spread16(qx) | (spread16(qy) << 1)) << 32) | (uint64_t)(uint32_t)i;
+  vals[i] = (int32_t)i;
+}
+
 __global__ void k_reverse(int32_t n, const int32_t* __restrict__ in, int32_t* __restrict__ out) {
   int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = in[n - 1 - i];
@@ -898,6 +936,21 @@ int tfa_mesh_reorder(tfa_mesh* m, int kind, const int32_t* user_perm, void* stre
     k_rcm<<<1, RCM_T, 0, st>>>((int32_t)nc, F, m->cell_nbr.p, order.p, pos.p, parent.p);
     k_reverse<<<cdiv(nc, TPB), TPB, 0, st>>>((int32_t)nc, order.p, p.p);
     TFA_CUDA(cudaGetLastError());
+    TFA_CUDA(cudaStreamSynchronize(st));
+  } else if (kind == 3) {
+    DevBuf<unsigned long long> box;
+    DevBuf<uint64_t> keys, keys_s;
+    DevBuf<int32_t> ids;
+    TFA_CUDA(box.alloc(4)); TFA_CUDA(keys.alloc(nc)); TFA_CUDA(keys_s.alloc(nc)); TFA_CUDA(ids.alloc(nc));
+    const unsigned long long init[4] = {~0ull, 0ull, ~0ull, 0ull};
+    TFA_CUDA(cudaMemcpyAsync(box.p, init, sizeof(init), cudaMemcpyHostToDevice, st));
+    k_bbox<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m->cen.p, box.p);
+    k_morton_keys<<<cdiv(nc, TPB), TPB, 0, st>>>(nc, m->cen.p, box.p, keys.p, ids.p);
+    size_t tmp_bytes = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys.p, keys_s.p, ids.p, p.p, (int)nc, 0, 64, st);
+    DevBuf<char> tmp;
+    TFA_CUDA(tmp.alloc((int64_t)tmp_bytes));
+    TFA_CUDA(cub::DeviceRadixSort::SortPairs(tmp.p, tmp_bytes, keys.p, keys_s.p, ids.p, p.p, (int)nc, 0, 64, st));
     TFA_CUDA(cudaStreamSynchronize(st));
   } else if (kind == 2) {
     if (!user_perm) return set_error(TFA_EINVAL, "user permutation missing");

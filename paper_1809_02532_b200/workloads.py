@@ -354,11 +354,11 @@ def make_workload(name: str, scale: float = 1.0) -> Workload:
         nx, ny = max(4, int(round(512 * scale))), max(4, int(round(256 * scale)))
         m = split_quad_mesh(nx, ny, *GEM_DOMAIN, periodic_x=True, periodic_y=False)
         return Workload(name, m, gem_state(m.centroids()), ph, 1e-3, 10)
-    if name in ("c4a", "c4b"):
+    if name in ("c4a", "c4b", "c4m"):   # c4m: config 4's mesh in Z-order (not a BASELINE run; a third ordering)
         npx, npy = int(round(1000 * scale)) + 1, int(round(500 * scale)) + 1
         m = delaunay_mesh(npx, npy, *GEM_DOMAIN, jitter=0.3, seed=2, shuffle_cells=True)
         return Workload(name, m, gem_state(m.centroids()), ph, 1e-3, 10,
-                        reorder="rcm" if name == "c4b" else "none", seed=2)
+                        reorder={"c4a": "none", "c4b": "rcm", "c4m": "morton"}[name], seed=2)
     if name == "c5":
         npx, npy = int(round(2000 * scale)) + 1, int(round(1000 * scale)) + 1
         m = delaunay_mesh(npx, npy, *GEM_DOMAIN, jitter=0.3, seed=3, shuffle_cells=False)

@@ -100,6 +100,40 @@ def test_rcm_disconnected_components(api, orc, W):
         np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
 
 
+@pytest.mark.parametrize("name", ["c1", "delaunay"])
+def test_morton_order(api, orc, W, name):
+    """tfa_mesh_reorder kind 3 (Z-order through the centroids, include/tfa.h).  The curve is the library's own choice, so
+    what is checked is what is unique: the permutation is a bijection that sorts the cells by the interleaved 16-bit
+    centroid coordinates written out here with numpy (ties by cell id), and every table after it equals the
+    oracle's after the same permutation given as a user one.  Patches of 32 consecutive cells are compact: they
+    touch fewer distinct stencil rows than in RCM order."""
+    mi = small_meshes(W)[name]
+    g = api.Mesh.from_input(mi)
+    cen = g.get("centroid")
+    g.reorder("morton")
+    perm = g.get("perm")
+    assert sorted(perm.tolist()) == list(range(g.n_cells))
+    lo, hi = cen.min(axis=0), cen.max(axis=0)
+    q = np.clip(np.floor((cen - lo) * (65535.0 / (hi - lo))), 0, 65535).astype(np.uint64)
+    code = np.zeros(g.n_cells, dtype=np.uint64)
+    for b in range(16):
+        code |= ((q[:, 0] >> np.uint64(b)) & np.uint64(1)) << np.uint64(2 * b)
+        code |= ((q[:, 1] >> np.uint64(b)) & np.uint64(1)) << np.uint64(2 * b + 1)
+    np.testing.assert_array_equal(perm, np.lexsort((np.arange(g.n_cells), code)))
+    o = orc.OracleMesh.from_input(mi)
+    o.reorder("user", perm.astype(np.int32))
+    for item in INT_ITEMS:
+        np.testing.assert_array_equal(g.get(item), o.get(item), err_msg=item)
+
+    def rows_per_patch(mesh):
+        sp, sc = mesh.get("stencil_ptr"), mesh.get("stencil_idx")
+        return np.mean([len(np.unique(sc[sp[a]:sp[min(a + 32, mesh.n_cells)]]))
+                        for a in range(0, mesh.n_cells, 32)])
+    r = api.Mesh.from_input(mi)
+    r.reorder("rcm")
+    assert rows_per_patch(g) < rows_per_patch(r)
+
+
 def test_mesh_errors_and_degenerate_sizes(api, W):
     mi = W.split_quad_mesh(3, 3, periodic_x=False, periodic_y=False)
     bad = mi.cell_nodes.copy()
