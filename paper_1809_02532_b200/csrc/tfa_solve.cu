@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "tfa_common.cuh"
+#include "tfa_tma.cuh"
 
 namespace tfa {
 int assemble_impl(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
@@ -129,88 +130,146 @@ __global__ void k_row_of_block(int64_t nc, const int32_t* __restrict__ rowptr, i
 }
 
 // ------------------------------------------------------------------------------------------------
-// Inverse of each diagonal block: one warp per cell, Gauss-Jordan with partial pivoting.  Lane r keeps row r in
-// registers; rows are never moved (the pivot of step k is the largest |a[r][k]| among the rows not yet used,
-// p_k); the pivot row goes through a double-buffered 18-double row of shared memory, one __syncwarp per step.  With P the permutation (PA)[k] = A[p_k], the in-place result S = (PA)^-1 sits as row k in lane p_k and
-// A^-1[k][p_c] = S[k][c]; it is put in order in shared memory and written out coalesced.
-// (First version: the block in shared memory, every lane sweeping 11 elements per step; 3 loads and a store
-// per element made it shared-memory-bandwidth bound, 9.8 ms at 1M cells.)
+// Inverse of each diagonal block: Gauss-Jordan with partial pivoting, FIVE blocks per warp.  A group of six lanes
+// owns one block, lane r of the group keeping rows 3r..3r+2 in registers (54 doubles); rows are never moved: the
+// pivot of step k is the largest |a[R][k]| among the rows not yet used, p_k, found with two group-masked warp
+// reductions, and its row reaches the other five lanes by shuffles from the owning lane.  Every value a lane
+// receives feeds three FMAs, and one shuffle instruction serves five blocks: 7 shared-memory-crossbar wavefronts
+// and 11 FP64 instructions per block and step, against 36 and 18 for the one-warp-per-block version before it
+// (3.4 ms at 1M cells, its shared-memory data pipe 67 % busy: profiles/r1_ncu_full_block_jacobi_c4b.md).
+// The blocks come in by TMA (one bulk load of 2592 B each) and go out the same way.  With P the permutation
+// (PA)[k] = A[p_k], the in-place result S = (PA)^-1 sits as row k in the lane that owned p_k and
+// A^-1[k][p_c] = S[k][c]; it is put in order in the shared-memory buffer the block arrived in.
 // ------------------------------------------------------------------------------------------------
-constexpr int BJ_WARPS = 8;
+constexpr int BJ_WARPS = 4, BJ_G = 5, BJ_L = 6, BJ_R = 3;
+// 1/d for a normal d: the hardware's 20-bit seed and two Newton steps (the pivot is never zero, subnormal or not
+// finite: those end the inversion before this is reached)
+__device__ __forceinline__ double bj_rcp(double d) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+  double e = fma(-d, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-d, y, 1.0);
+  return fma(y, e, y);
+}
+constexpr size_t BJ_SMEM = sizeof(double) * BJ_WARPS * BJ_G * BLK + sizeof(uint64_t) * BJ_WARPS;
 __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ blkmap, int BS,
                                                                const double* __restrict__ vals,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
-  __shared__ __align__(16) double rowbuf[BJ_WARPS][2][NEQ];
-  __shared__ __align__(16) double outb[BJ_WARPS][BLK];
+  extern __shared__ __align__(128) unsigned char bj_raw[];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int64_t i = blockIdx.x * (int64_t)BJ_WARPS + w;
-  if (i >= nc) return;
-  // the diagonal block of row i (every row of the mesh's pattern has one); blkmap == NULL: vals is the packed
-  // Jacobian's array of diagonal blocks
-  const int64_t bd = blkmap ? (int64_t)blkmap[(int64_t)BS * i] : i;
-  const bool has = lane < NEQ;
-  double a[NEQ];
-#pragma unroll
-  for (int c = 0; c < NEQ; ++c) a[c] = 0.0;
-  if (has) {
-    const double2* __restrict__ src = reinterpret_cast<const double2*>(vals + bd * BLK + lane * NEQ);
-#pragma unroll
-    for (int c = 0; c < NEQ; c += 2) {
-      const double2 t = src[c / 2];
-      a[c] = t.x;
-      a[c + 1] = t.y;
-    }
-  }
-  bool used = !has, singular = false;
-  int myk = 0;
-  int pk[NEQ];
-#pragma unroll
-  for (int k = 0; k < NEQ; ++k) pk[k] = 0;
-#pragma unroll
-  for (int k = 0; k < NEQ; ++k) {
-    // pivot: the largest |a[r][k]| over the rows not used yet, compared on the high word (sign, exponent, 20
-    // mantissa bits: any entry within 2^-20 of the largest serves partial pivoting equally well) with one warp
-    // reduction; ties go to the smallest r.  NaN / Inf sort above every finite number and end the inversion.
-    const unsigned key = used ? 0u : (unsigned)(__double2hiint(a[k]) & 0x7fffffff);
-    const unsigned mx = __reduce_max_sync(0xffffffffu, key);
-    if (mx == 0u || mx >= 0x7ff00000u) singular = true;   // warp-uniform: zero / subnormal / not finite
-    if (!singular) {
-      const int arg = __ffs(__ballot_sync(0xffffffffu, key == mx)) - 1;
-      pk[k] = arg;
-      double2* __restrict__ rb = reinterpret_cast<double2*>(rowbuf[w][k & 1]);
-      const bool mine = lane == arg;
-      if (mine) {
-#pragma unroll
-        for (int c = 0; c < NEQ; c += 2) rb[c / 2] = make_double2(a[c], a[c + 1]);
-        used = true;
-        myk = k;
-      }
-      __syncwarp();
-      // one code path for all rows: a[c] <- m t[c] + z with (m, z) = (1/t[k], 0) on the pivot row (its own row
-      // is t) and (-a[k]/t[k], a[c]) elsewhere; column k becomes the inverse's: 1/t[k] and -a[k]/t[k]
-      const double ip = 1.0 / rowbuf[w][k & 1][k];
-      const double m = mine ? ip : -(a[k] * ip);
-#pragma unroll
-      for (int c = 0; c < NEQ; c += 2) {
-        const double2 t = rb[c / 2];
-        a[c] = c == k ? m : fma(m, t.x, mine ? 0.0 : a[c]);
-        a[c + 1] = c + 1 == k ? m : fma(m, t.y, mine ? 0.0 : a[c + 1]);
-      }
-    }
-  }
-  if (singular) {
-    if (lane == 0) atomicAdd(flags + 1, 1);
-    for (int e = lane; e < BLK; e += 32) dinv[i * BLK + e] = 0.0;
-    return;
-  }
-  if (has) {
-#pragma unroll
-    for (int c = 0; c < NEQ; ++c) outb[w][myk * NEQ + pk[c]] = a[c];
+  double(*buf)[BLK] = reinterpret_cast<double(*)[BLK]>(bj_raw) + w * BJ_G;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(bj_raw + sizeof(double) * BJ_WARPS * BJ_G * BLK) + w;
+  const int64_t i0 = (blockIdx.x * (int64_t)BJ_WARPS + w) * BJ_G;
+  // no early return: a warp past the end runs with nb = 0 (the compiler must see all 32 lanes reach the shuffles)
+  const int nb = (int)max((int64_t)0, min((int64_t)BJ_G, nc - i0));
+  if (lane == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_arrive_expect_tx(bar, (uint32_t)(nb * BLK * sizeof(double)));
   }
   __syncwarp();
-  const double2* __restrict__ ob2 = reinterpret_cast<const double2*>(outb[w]);
-  double2* __restrict__ dst = reinterpret_cast<double2*>(dinv + i * BLK);
-  for (int e = lane; e < BLK / 2; e += 32) dst[e] = ob2[e];
+  // the diagonal block of row i (every row of the mesh's pattern has one); blkmap == NULL: vals is the packed
+  // Jacobian's array of diagonal blocks
+  if (lane < nb) {
+    const int64_t i = i0 + lane, bd = blkmap ? (int64_t)blkmap[(int64_t)BS * i] : i;
+    bulk_load(buf[lane], vals + bd * BLK, (uint32_t)(BLK * sizeof(double)), bar);
+  }
+  const int g = lane / BJ_L, r = lane - BJ_L * g;
+  const bool have = g < nb;                                     // lanes 30, 31 and the groups past the end idle
+  const int gl0 = BJ_L * g;                                     // the group's first lane; its rotations by 1 and 2
+  const int rot1 = g < BJ_G ? gl0 + (r + 1) % BJ_L : lane, rot2 = g < BJ_G ? gl0 + (r + 2) % BJ_L : lane;
+  double a[BJ_R][NEQ];
+  mbar_wait(bar, 0);
+#pragma unroll
+  for (int s = 0; s < BJ_R; ++s)
+#pragma unroll
+    for (int c = 0; c < NEQ; c += 2) {
+      const double2 t = have ? *reinterpret_cast<const double2*>(&buf[g][(BJ_R * r + s) * NEQ + c]) : make_double2(0.0, 0.0);
+      a[s][c] = t.x;
+      a[s][c + 1] = t.y;
+    }
+  bool used[BJ_R] = {false, false, false}, singular = false;
+  int myk[BJ_R] = {0, 0, 0};
+  double scale[BJ_R] = {1.0, 1.0, 1.0};
+  unsigned pk[3] = {0u, 0u, 0u};   // p_k, five bits each, six to a word
+#pragma unroll
+  for (int k = 0; k < NEQ; ++k) {
+    // pivot: the largest |a[R][k]| over the rows not used yet, compared on the high word without its last five
+    // bits (exponent and 15 mantissa bits: any entry within 2^-15 of the largest serves partial pivoting equally
+    // well); those five bits carry 31 - R, so that ties go to the smallest R and one maximum over the group's
+    // six lanes (three rotations by shuffle; a masked __reduce_max_sync runs once per group, six times slower)
+    // gives the row as well.  NaN / Inf sort above every finite number and end the inversion.
+    unsigned lkey = 0u;
+#pragma unroll
+    for (int s = 0; s < BJ_R; ++s) {
+      const unsigned key = ((unsigned)__double2hiint(a[s][k]) & 0x7fffffe0u) | (unsigned)(31 - BJ_R * r - s);
+      lkey = max(lkey, used[s] ? 0u : key);
+    }
+    lkey = max(lkey, __shfl_sync(0xffffffffu, lkey, rot1));
+    lkey = max(lkey, __shfl_sync(0xffffffffu, lkey, rot2));
+    const unsigned mx = max(lkey, __shfl_sync(0xffffffffu, lkey, rot2));
+    if (mx < 32u || mx >= 0x7ff00000u) singular = true;   // group-uniform: zero / subnormal / not finite
+    const int win = min(31 - (int)(mx & 31u), NEQ - 1);
+    const int owner = gl0 + win / BJ_R, slot = win - BJ_R * (win / BJ_R);
+    pk[k / 6] |= (unsigned)win << (5 * (k % 6));
+    // rows other than the pivot row: a[c] <- a[c] + m t[c] with m = -a[k]/t[k], and column k becomes the inverse's,
+    // m.  The pivot row is NOT divided by its pivot now: every later step acts linearly on it, so the factor
+    // 1/t[k] is kept in `scale` and applied once at the end (its column k holds 1 until then).
+    const bool s1 = slot == 1, s2 = slot == 2;
+    const double ip = bj_rcp(__shfl_sync(0xffffffffu, s2 ? a[2][k] : (s1 ? a[1][k] : a[0][k]), owner));
+    double m[BJ_R];
+#pragma unroll
+    for (int s = 0; s < BJ_R; ++s) {
+      const bool mine = BJ_R * r + s == win;
+      m[s] = mine ? 0.0 : -(a[s][k] * ip);
+      if (mine) {
+        used[s] = true;
+        myk[s] = k;
+        scale[s] = ip;
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < NEQ; ++c) {
+      if (c == k) continue;
+      const double t = __shfl_sync(0xffffffffu, s2 ? a[2][c] : (s1 ? a[1][c] : a[0][c]), owner);
+#pragma unroll
+      for (int s = 0; s < BJ_R; ++s) a[s][c] = fma(m[s], t, a[s][c]);
+    }
+#pragma unroll
+    for (int s = 0; s < BJ_R; ++s) a[s][k] = (used[s] && myk[s] == k) ? 1.0 : m[s];
+  }
+  __syncwarp();
+  if (have) {
+#pragma unroll
+    for (int s = 0; s < BJ_R; ++s)
+#pragma unroll
+      for (int c = 0; c < NEQ; ++c)
+        buf[g][myk[s] * NEQ + (int)((pk[c / 6] >> (5 * (c % 6))) & 31u)] = scale[s] * a[s][c];
+    if (singular) {   // the block's inverse is reported as zeros, and counted
+      for (int e = r; e < BLK; e += BJ_L) buf[g][e] = 0.0;
+      if (r == 0) atomicAdd(flags + 1, 1);
+    }
+  }
+  fence_async_smem();
+  __syncwarp();
+  if (lane < nb) {
+    bulk_store(dinv + (i0 + lane) * BLK, buf[lane], (uint32_t)(BLK * sizeof(double)));
+    bulk_commit();
+    bulk_wait_read();
+  }
+}
+static int launch_block_jacobi(int64_t nc, const int32_t* blkmap, int BS, const double* vals, double* dinv,
+                               int32_t* flags, cudaStream_t st) {
+  if ((reinterpret_cast<uintptr_t>(vals) | reinterpret_cast<uintptr_t>(dinv)) & 15)
+    return set_error(TFA_EINVAL, "tfa_block_jacobi: the block arrays must be 16-byte aligned");
+  static bool attr_set = false;   // the attribute belongs to the function; setting it twice is harmless
+  if (!attr_set) {
+    TFA_CUDA(cudaFuncSetAttribute(k_block_jacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BJ_SMEM));
+    attr_set = true;
+  }
+  k_block_jacobi<<<cdiv(nc, BJ_WARPS * BJ_G), 32 * BJ_WARPS, BJ_SMEM, st>>>(nc, blkmap, BS, vals, dinv, flags);
+  return 0;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -502,8 +561,7 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, m->blkmap.p, blk_stride(m->F), bsr_vals, dinv,
-                                                                  ctx->flags.p);
+  TFA_TRY(launch_block_jacobi(m->nc, m->blkmap.p, blk_stride(m->F), bsr_vals, dinv, ctx->flags.p, st));
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
@@ -596,7 +654,7 @@ int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  k_block_jacobi<<<cdiv(m->nc, BJ_WARPS), 32 * BJ_WARPS, 0, st>>>(m->nc, nullptr, 0, diag_vals, dinv, ctx->flags.p);
+  TFA_TRY(launch_block_jacobi(m->nc, nullptr, 0, diag_vals, dinv, ctx->flags.p, st));
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
