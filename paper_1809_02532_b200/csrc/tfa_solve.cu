@@ -132,10 +132,10 @@ __global__ void k_row_of_block(int64_t nc, const int32_t* __restrict__ rowptr, i
 // ------------------------------------------------------------------------------------------------
 // Inverse of each diagonal block: Gauss-Jordan with partial pivoting, FIVE blocks per warp.  A group of six lanes
 // owns one block, lane r of the group keeping rows 3r..3r+2 in registers (54 doubles); rows are never moved: the
-// pivot of step k is the largest |a[R][k]| among the rows not yet used, p_k, found with two group-masked warp
-// reductions, and its row reaches the other five lanes by shuffles from the owning lane.  Every value a lane
-// receives feeds three FMAs, and one shuffle instruction serves five blocks: 7 shared-memory-crossbar wavefronts
-// and 11 FP64 instructions per block and step, against 36 and 18 for the one-warp-per-block version before it
+// pivot of step k is the largest |a[R][k]| among the rows not yet used, p_k, found by three shuffle rotations
+// inside the group, and its row reaches the group through 144 bytes of shared memory.  Every value a lane
+// receives feeds three FMAs, and one broadcast load serves five blocks: 11 shared-memory wavefronts and 11 FP64
+// instructions per block and step, against 36 and 18 for the one-warp-per-block version before it
 // (3.4 ms at 1M cells, its shared-memory data pipe 67 % busy: profiles/r1_ncu_full_block_jacobi_c4b.md).
 // The blocks come in by TMA (one bulk load of 2592 B each) and go out the same way.  With P the permutation
 // (PA)[k] = A[p_k], the in-place result S = (PA)^-1 sits as row k in the lane that owned p_k and
@@ -144,6 +144,10 @@ __global__ void k_row_of_block(int64_t nc, const int32_t* __restrict__ rowptr, i
 constexpr int BJ_WARPS = 4, BJ_G = 5, BJ_L = 6, BJ_R = 3;
 // 1/d for a normal d: the hardware's 20-bit seed and two Newton steps (the pivot is never zero, subnormal or not
 // finite: those end the inversion before this is reached)
+__device__ __forceinline__ void bj_put_row(double2* __restrict__ dst, const double (&row)[NEQ]) {
+#pragma unroll
+  for (int c = 0; c < NEQ; c += 2) dst[c / 2] = make_double2(row[c], row[c + 1]);
+}
 __device__ __forceinline__ double bj_rcp(double d) {
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
@@ -152,14 +156,16 @@ __device__ __forceinline__ double bj_rcp(double d) {
   e = fma(-d, y, 1.0);
   return fma(y, e, y);
 }
-constexpr size_t BJ_SMEM = sizeof(double) * BJ_WARPS * BJ_G * BLK + sizeof(uint64_t) * BJ_WARPS;
+constexpr size_t BJ_SMEM = sizeof(double) * BJ_WARPS * (BJ_G * BLK + 2 * BJ_G * NEQ) + sizeof(uint64_t) * BJ_WARPS;
 __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ blkmap, int BS,
                                                                const double* __restrict__ vals,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
   extern __shared__ __align__(128) unsigned char bj_raw[];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   double(*buf)[BLK] = reinterpret_cast<double(*)[BLK]>(bj_raw) + w * BJ_G;
-  uint64_t* bar = reinterpret_cast<uint64_t*>(bj_raw + sizeof(double) * BJ_WARPS * BJ_G * BLK) + w;
+  // pivot rows: [2][BJ_G][18] doubles per warp (144 bytes apart: the five owners' 16-byte stores fall in distinct banks)
+  double* const prows = reinterpret_cast<double*>(bj_raw) + BJ_WARPS * BJ_G * BLK + w * 2 * BJ_G * NEQ;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(bj_raw + sizeof(double) * BJ_WARPS * (BJ_G * BLK + 2 * BJ_G * NEQ)) + w;
   const int64_t i0 = (blockIdx.x * (int64_t)BJ_WARPS + w) * BJ_G;
   // no early return: a warp past the end runs with nb = 0 (the compiler must see all 32 lanes reach the shuffles)
   const int nb = (int)max((int64_t)0, min((int64_t)BJ_G, nc - i0));
@@ -177,6 +183,7 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
   }
   const int g = lane / BJ_L, r = lane - BJ_L * g;
   const bool have = g < nb;                                     // lanes 30, 31 and the groups past the end idle
+  const int gb = min(g, BJ_G - 1);                              // lanes 30, 31 read (never write) the last buffer
   const int gl0 = BJ_L * g;                                     // the group's first lane; its rotations by 1 and 2
   const int rot1 = g < BJ_G ? gl0 + (r + 1) % BJ_L : lane, rot2 = g < BJ_G ? gl0 + (r + 2) % BJ_L : lane;
   double a[BJ_R][NEQ];
@@ -216,8 +223,18 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
     // rows other than the pivot row: a[c] <- a[c] + m t[c] with m = -a[k]/t[k], and column k becomes the inverse's,
     // m.  The pivot row is NOT divided by its pivot now: every later step acts linearly on it, so the factor
     // 1/t[k] is kept in `scale` and applied once at the end (its column k holds 1 until then).
-    const bool s1 = slot == 1, s2 = slot == 2;
-    const double ip = bj_rcp(__shfl_sync(0xffffffffu, s2 ? a[2][k] : (s1 ? a[1][k] : a[0][k]), owner));
+    // the pivot row goes through 144 bytes of shared memory, double-buffered: its owner stores whichever of its
+    // three rows it is -- the only place the dynamic row slot costs anything -- and the six lanes read it back as
+    // broadcasts, one __syncwarp per step
+    double2* __restrict__ prow = reinterpret_cast<double2*>(prows + ((k & 1) * BJ_G + gb) * NEQ);
+    if (have && lane == owner) {
+      if (slot == 0) bj_put_row(prow, a[0]);
+      else if (slot == 1) bj_put_row(prow, a[1]);
+      else bj_put_row(prow, a[2]);
+    }
+    __syncwarp();
+    const double2 tkk = prow[k / 2];
+    const double ip = bj_rcp(k & 1 ? tkk.y : tkk.x);
     double m[BJ_R];
 #pragma unroll
     for (int s = 0; s < BJ_R; ++s) {
@@ -230,11 +247,13 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
       }
     }
 #pragma unroll
-    for (int c = 0; c < NEQ; ++c) {
-      if (c == k) continue;
-      const double t = __shfl_sync(0xffffffffu, s2 ? a[2][c] : (s1 ? a[1][c] : a[0][c]), owner);
+    for (int c = 0; c < NEQ; c += 2) {
+      const double2 t = prow[c / 2];
 #pragma unroll
-      for (int s = 0; s < BJ_R; ++s) a[s][c] = fma(m[s], t, a[s][c]);
+      for (int s = 0; s < BJ_R; ++s) {
+        if (c != k) a[s][c] = fma(m[s], t.x, a[s][c]);
+        if (c + 1 != k) a[s][c + 1] = fma(m[s], t.y, a[s][c + 1]);
+      }
     }
 #pragma unroll
     for (int s = 0; s < BJ_R; ++s) a[s][k] = (used[s] && myk[s] == k) ? 1.0 : m[s];
