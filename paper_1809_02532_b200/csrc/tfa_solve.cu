@@ -297,34 +297,37 @@ static int launch_block_jacobi(int64_t nc, const int32_t* blkmap, int BS, const 
 // ------------------------------------------------------------------------------------------------
 constexpr int RED_T = 256, RED_B = 592;
 
-// part[b][j] = sum over the CTA's share of V_j . w, j < k  (V_j = V + j * ld).  Eight products per pass over w,
+// part[b][j] = sum over the CTA's share of V_j . w, j < k  (V_j = V + j * ld); with `self`, entry k is w . w (the
+// norm the Gram-Schmidt pass starts from, taken in the same pass over w).  Eight products per pass over w,
 // 16-byte loads (n and ld are multiples of 18, hence even; the arrays are 16-byte aligned), the eight streams of a
 // thread in flight together.
 __global__ void __launch_bounds__(RED_T) k_dots(int64_t n, int k, const double* __restrict__ V, int64_t ld,
-                                               const double* __restrict__ w, double* __restrict__ part) {
+                                               const double* __restrict__ w, double* __restrict__ part, bool self) {
   __shared__ double sm[RED_T / 32];
-  const int64_t n2 = n >> 1, ld2 = ld >> 1;
+  const int64_t n2 = n >> 1;
   const double2* __restrict__ w2 = reinterpret_cast<const double2*>(w);
-  const double2* __restrict__ V2 = reinterpret_cast<const double2*>(V);
   // caller-owned vectors need not be 16-byte aligned: then one element at a time
   const bool vec = !((reinterpret_cast<uintptr_t>(V) | reinterpret_cast<uintptr_t>(w)) & 15) && !(n & 1) && !(ld & 1);
-  for (int j0 = 0; j0 < k; j0 += 8) {
+  const int kk = k + (self ? 1 : 0);
+  for (int j0 = 0; j0 < kk; j0 += 8) {
     double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    const int kj = min(8, k - j0);
-    const double2* __restrict__ Vb = V2 + (int64_t)j0 * ld2;
+    const int kj = min(8, kk - j0);
+    const double* vp[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) vp[q] = j0 + q < k ? V + (int64_t)(j0 + q) * ld : w;
     if (!vec) {
       for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
         const double we = w[e];
 #pragma unroll
         for (int q = 0; q < 8; ++q)
-          if (q < kj) acc[q] = fma(V[(j0 + q) * ld + e], we, acc[q]);
+          if (q < kj) acc[q] = fma(vp[q][e], we, acc[q]);
       }
     } else if (kj == 8) {
       for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
         const double2 we = w2[e];
         double2 v[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) v[q] = Vb[q * ld2 + e];
+        for (int q = 0; q < 8; ++q) v[q] = reinterpret_cast<const double2*>(vp[q])[e];
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[q] = fma(v[q].y, we.y, fma(v[q].x, we.x, acc[q]));
       }
@@ -334,7 +337,7 @@ __global__ void __launch_bounds__(RED_T) k_dots(int64_t n, int k, const double* 
 #pragma unroll
         for (int q = 0; q < 8; ++q)
           if (q < kj) {
-            const double2 v = Vb[q * ld2 + e];
+            const double2 v = reinterpret_cast<const double2*>(vp[q])[e];
             acc[q] = fma(v.y, we.y, fma(v.x, we.x, acc[q]));
           }
       }
@@ -364,42 +367,58 @@ __global__ void __launch_bounds__(32) k_dots_final(int nblocks, const double* __
   for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
   if (threadIdx.x == 0) out[j] = s;
 }
-// w -= sum_j h[j] V_j   (16-byte accesses; four basis vectors in flight at a time)
+// w -= sum_j h[j] V_j   (16-byte accesses; four basis vectors in flight at a time).  With `part` the CTA's share of
+// the NEW w . w goes to part[b][0] (the norm after the Gram-Schmidt pass, from the values just computed).
 __global__ void __launch_bounds__(RED_T) k_sub_combination(int64_t n, int k, const double* __restrict__ V, int64_t ld,
-                                                          const double* __restrict__ h, double* __restrict__ w) {
+                                                          const double* __restrict__ h, double* __restrict__ w,
+                                                          double* __restrict__ part) {
   __shared__ double hs[MAXK];
+  __shared__ double sm[RED_T / 32];
   if (threadIdx.x < k) hs[threadIdx.x] = h[threadIdx.x];
   __syncthreads();
   const int64_t n2 = n >> 1, ld2 = ld >> 1;
   double2* __restrict__ w2 = reinterpret_cast<double2*>(w);
   const double2* __restrict__ V2 = reinterpret_cast<const double2*>(V);
+  double nrm = 0.0;
   if (((reinterpret_cast<uintptr_t>(V) | reinterpret_cast<uintptr_t>(w)) & 15) || (n & 1) || (ld & 1)) {
     for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n; e += (int64_t)RED_T * gridDim.x) {
       double v = w[e];
       for (int j = 0; j < k; ++j) v = fma(-hs[j], V[j * ld + e], v);
       w[e] = v;
+      nrm = fma(v, v, nrm);
     }
-    return;
-  }
-  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
-    double2 v = w2[e];
-    int j = 0;
-    for (; j + 4 <= k; j += 4) {
-      double2 t[4];
+  } else {
+    for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
+      double2 v = w2[e];
+      int j = 0;
+      for (; j + 4 <= k; j += 4) {
+        double2 t[4];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) t[q] = V2[(int64_t)(j + q) * ld2 + e];
+        for (int q = 0; q < 4; ++q) t[q] = V2[(int64_t)(j + q) * ld2 + e];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        v.x = fma(-hs[j + q], t[q].x, v.x);
-        v.y = fma(-hs[j + q], t[q].y, v.y);
+        for (int q = 0; q < 4; ++q) {
+          v.x = fma(-hs[j + q], t[q].x, v.x);
+          v.y = fma(-hs[j + q], t[q].y, v.y);
+        }
       }
+      for (; j < k; ++j) {
+        const double2 t = V2[(int64_t)j * ld2 + e];
+        v.x = fma(-hs[j], t.x, v.x);
+        v.y = fma(-hs[j], t.y, v.y);
+      }
+      w2[e] = v;
+      nrm = fma(v.y, v.y, fma(v.x, v.x, nrm));
     }
-    for (; j < k; ++j) {
-      const double2 t = V2[(int64_t)j * ld2 + e];
-      v.x = fma(-hs[j], t.x, v.x);
-      v.y = fma(-hs[j], t.y, v.y);
-    }
-    w2[e] = v;
+  }
+  if (!part) return;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = nrm;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int q = 0; q < RED_T / 32; ++q) t += sm[q];
+    part[(int64_t)blockIdx.x * MAXK] = t;
   }
 }
 // out = a * x + c * y   (y may be null with c = 0)
@@ -438,7 +457,7 @@ struct Gm {
   }
   // host[j] = V_j . w for j < k (synchronises)
   int dots(int k, const double* V, int64_t ld, const double* w) {
-    k_dots<<<RED_B, RED_T, 0, st>>>(n, k, V, ld, w, part);
+    k_dots<<<RED_B, RED_T, 0, st>>>(n, k, V, ld, w, part, false);
     k_dots_final<<<k, 32, 0, st>>>(RED_B, part, out);
     TFA_CUDA(cudaMemcpyAsync(host, out, sizeof(double) * k, cudaMemcpyDeviceToHost, st));
     TFA_CUDA(cudaStreamSynchronize(st));
@@ -494,22 +513,26 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
     for (; k < mk && iters < max_iters; ++k, ++iters) {
       G.precond(V + (int64_t)k * n, z);
       TFA_TRY(G.spmv(z, w));
-      // classical Gram-Schmidt (all projections from one pass over the basis), repeated when it cancelled
-      // more than a factor sqrt(2) of the vector (the Daniel-Gragg-Kaufman-Stewart test): "twice is enough"
+      // classical Gram-Schmidt (all projections from one pass over the basis), repeated when it cancelled more
+      // than a factor 10 of the vector (the Daniel-Gragg-Kaufman-Stewart test with eta = 0.1: the loss of
+      // orthogonality of a single pass grows like eps / eta^2, and on the preconditioned systems of the method a
+      // pass keeps 0.3-0.6 of the norm).  One pass = two kernels and ONE synchronisation: the projections stay on
+      // the device between them, the norm before comes out of the first (entry k + 1), the norm after out of the
+      // second (entry k + 2).
       double* h = &H[(size_t)k * (mk + 1)];
       for (int j = 0; j <= k + 1; ++j) h[j] = 0.0;
-      TFA_TRY(G.dots(1, w, n, w));
-      double before = std::sqrt(G.host[0]), hk1 = 0.0;
+      double hk1 = 0.0;
       for (int pass = 0; pass < 2; ++pass) {
-        TFA_TRY(G.dots(k + 1, V, n, w));
+        k_dots<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, w, G.part, true);
+        k_dots_final<<<k + 2, 32, 0, st>>>(RED_B, G.part, G.out);
+        k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, G.out, w, G.part);
+        k_dots_final<<<1, 32, 0, st>>>(RED_B, G.part, G.out + k + 2);
+        TFA_CUDA(cudaMemcpyAsync(G.host, G.out, sizeof(double) * (k + 3), cudaMemcpyDeviceToHost, st));
+        TFA_CUDA(cudaStreamSynchronize(st));
         for (int j = 0; j <= k; ++j) h[j] += G.host[j];
-        TFA_CUDA(cudaMemcpyAsync(G.out, G.host, sizeof(double) * (k + 1), cudaMemcpyHostToDevice, st));
-        k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, G.out, w);
-        TFA_CUDA(cudaStreamSynchronize(st));   // G.host is reused by the next reduction
-        TFA_TRY(G.dots(1, w, n, w));
-        hk1 = std::sqrt(G.host[0]);
-        if (hk1 > 0.7071067811865476 * before) break;
-        before = hk1;
+        const double before = std::sqrt(G.host[k + 1]);
+        hk1 = std::sqrt(G.host[k + 2]);
+        if (!(hk1 <= 0.1 * before)) break;   // also leaves on NaN
       }
       h[k + 1] = hk1;
       if (!std::isfinite(hk1)) return set_error(TFA_ESINGULAR, "tfa_gmres: a Krylov vector is not finite");
@@ -546,7 +569,7 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
       for (int j = 0; j < k; ++j) G.host[j] = -yv[j];
       TFA_CUDA(cudaMemcpyAsync(G.out, G.host, sizeof(double) * k, cudaMemcpyHostToDevice, st));
       TFA_CUDA(cudaMemsetAsync(w, 0, sizeof(double) * n, st));
-      k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k, V, n, G.out, w);   // w = sum_j y_j V_j
+      k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k, V, n, G.out, w, nullptr);   // w = sum_j y_j V_j
       TFA_CUDA(cudaStreamSynchronize(st));
       G.precond(w, z);
       k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, z, 1.0, x, x);
