@@ -199,13 +199,14 @@ int tfa_probe_math(const double* x, double* sqrt_out, double* rcp_out, int64_t n
  * matrix arguments are DEVICE pointers owned by the caller; x, y, b have 18 * n_cells entries. ---- */
 /* y = A x for A = bsr_vals in the mesh's BSR pattern. */
 int tfa_bsr_spmv(const tfa_mesh* m, const double* bsr_vals, const double* x, double* y, void* stream);
-/* dinv [n_cells][18][18] = inverses of the diagonal blocks (Gauss-Jordan with partial pivoting, one warp per
- * block; the pivot is the largest remaining entry of the column up to 2^-20 relative).  A singular block (pivot 0,
- * subnormal or not finite) gets a zero inverse and is reported by tfa_check as TFA_ESINGULAR. */
+/* dinv [n_cells][18][18] = inverses of the diagonal blocks (Gauss-Jordan with partial pivoting, five blocks per
+ * warp; the pivot is the largest remaining entry of the column up to 2^-15 relative, ties to the smallest row).  A
+ * singular block (pivot 0, subnormal or not finite) gets a zero inverse and is reported by tfa_check as
+ * TFA_ESINGULAR.  bsr_vals and dinv must be 16-byte aligned (the blocks move by TMA bulk copies), else TFA_EINVAL. */
 int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, double* dinv, void* stream);
 /* Solve A x = b by right-preconditioned GMRES(restart): A M^-1 u = b, x = x0 + M^-1 u, M^-1 = dinv (block
  * diagonal; NULL = no preconditioner).  x holds the initial guess on entry and the solution on return.
- * Orthogonalisation: classical Gram-Schmidt, repeated once when it cancelled more than a factor sqrt(2); the small Hessenberg problem is solved on the host
+ * Orthogonalisation: classical Gram-Schmidt, repeated once when it cancelled more than a factor 10; the small Hessenberg problem is solved on the host
  * with Givens rotations (each iteration synchronises the stream).  Stops when the true residual norm
  * ||b - A x|| <= rtol * ||b|| (checked at every restart; the recurrence's estimate ends a cycle) or after
  * max_iters iterations.  info[0] = iterations done, info[1] = ||b - A x|| / ||b|| on return.
