@@ -153,6 +153,49 @@ def test_block_jacobi_needs_its_pivoting(system):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("shape", [None, (1, 1), (1, 2), (1, 3), (2, 5), (3, 7), (10, 10)])
+def test_block_jacobi_group_tails(W, shape):
+    """The kernel works on five blocks per warp (six lanes each, lanes 30 and 31 idle) and twenty per CTA: cell
+    counts of 1, 2, 4, 6, 20, 42 and 200 leave groups, warps and CTAs partly empty.  Random diagonal blocks with one
+    singular block among them (zero inverse + count, its neighbours in the same warp untouched); numpy's inverse
+    is the check."""
+    import torch
+    from paper_1809_02532_b200 import api, build
+    build.build()
+    if shape is None:
+        g = api.Mesh(np.array([[0.0, 0], [1, 0], [0, 1]]), np.array([[0, 1, 2]], dtype=np.int32))
+    else:
+        g = api.Mesh.from_input(W.split_quad_mesh(*shape, periodic_x=False, periodic_y=False))
+    n = g.n_cells
+    rng = np.random.default_rng(n)
+    blocks = rng.standard_normal((n, 18, 18)) + 3.0 * np.eye(18)
+    bad = n // 2 if n > 1 else None
+    if bad is not None:
+        blocks[bad, :, 5] = 0.0                       # a zero column: singular
+    ctx = api.Context(W.Physics())
+    dinv = ctx.block_jacobi_packed(g, torch.from_numpy(blocks).cuda()).cpu().numpy()
+    good = np.ones(n, dtype=bool)
+    if bad is not None:
+        good[bad] = False
+        assert not dinv[bad].any()
+        with pytest.raises(api.TfaError) as e:
+            ctx.check()
+        assert e.value.code == -6
+    else:
+        ctx.check()
+    ref = np.linalg.inv(blocks[good])
+    cond = np.linalg.cond(blocks[good], 1)
+    assert (np.abs(dinv[good] - ref).max(axis=(1, 2)) <= 1e-13 * cond * np.abs(ref).max(axis=(1, 2))).all()
+    # the same blocks through the BSR entry point (diagonal block found through the block map)
+    rp, col = g.get("bsr_rowptr"), g.get("bsr_col")
+    vals = torch.zeros((g.nnzb, 18, 18), dtype=torch.float64, device="cuda")
+    diag = np.array([rp[i] + int(np.nonzero(col[rp[i]:rp[i + 1]] == i)[0][0]) for i in range(n)])
+    vals[torch.from_numpy(diag).cuda()] = torch.from_numpy(blocks).cuda()
+    ctx2 = api.Context(W.Physics())
+    assert np.array_equal(ctx2.block_jacobi(g, vals).cpu().numpy(), dinv)
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("precond", [True, False])
 def test_gmres_parity(system, precond):
     import torch
