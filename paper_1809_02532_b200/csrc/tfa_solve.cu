@@ -139,11 +139,7 @@ static int launch_packed_spmv(const tfa_mesh* m, const double* dvals, const doub
                               cudaStream_t st) {
   if ((reinterpret_cast<uintptr_t>(dvals) | reinterpret_cast<uintptr_t>(ovals) | reinterpret_cast<uintptr_t>(x)) & 15)
     return set_error(TFA_EINVAL, "tfa_packed_spmv: the packed arrays and x must be 16-byte aligned");
-  static bool attr_set = false;
-  if (!attr_set) {
-    TFA_CUDA(cudaFuncSetAttribute(k_packed_spmv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)packed_spmv_smem(4)));
-    attr_set = true;
-  }
+  TFA_CUDA(cudaFuncSetAttribute(k_packed_spmv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)packed_spmv_smem(4)));
   k_packed_spmv<<<cdiv(m->nc, SV_CELLS), SV_T, packed_spmv_smem(m->F), st>>>(
       m->nc, blk_stride(m->F), m->bsr_rowptr.p, m->bsr_col.p, m->blkmap.p, dvals, ovals, x, y);
   return 0;
@@ -327,11 +323,8 @@ static int launch_block_jacobi(int64_t nc, const int32_t* blkmap, int BS, const 
                                int32_t* flags, cudaStream_t st) {
   if ((reinterpret_cast<uintptr_t>(vals) | reinterpret_cast<uintptr_t>(dinv)) & 15)
     return set_error(TFA_EINVAL, "tfa_block_jacobi: the block arrays must be 16-byte aligned");
-  static bool attr_set = false;   // the attribute belongs to the function; setting it twice is harmless
-  if (!attr_set) {
-    TFA_CUDA(cudaFuncSetAttribute(k_block_jacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BJ_SMEM));
-    attr_set = true;
-  }
+  // per launch: the attribute belongs to the function on the CURRENT device, and the call is cheap
+  TFA_CUDA(cudaFuncSetAttribute(k_block_jacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BJ_SMEM));
   k_block_jacobi<<<cdiv(nc, BJ_WARPS * BJ_G), 32 * BJ_WARPS, BJ_SMEM, st>>>(nc, blkmap, BS, vals, dinv, flags);
   return 0;
 }
