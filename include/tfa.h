@@ -243,7 +243,8 @@ int tfa_implicit_step(tfa_ctx* ctx, const tfa_mesh* m, double* state, const doub
  * tfa_assemble_packed = tfa_assemble writing that form (same arithmetic, same rhs, bit-identical entries; 5328
  * instead of 10368 bytes of Jacobian per triangle); tfa_packed_to_bsr expands it into the mesh's BSR value array;
  * tfa_packed_spmv, tfa_block_jacobi_packed and tfa_gmres_packed are the linear-solve entry points on it.  Not
- * available on a shard's mesh.  All pointers DEVICE pointers. */
+ * available on a shard's mesh.  All pointers DEVICE pointers; the packed arrays, x and dinv must be 16-byte aligned
+ * (the blocks move by TMA bulk copies and 16-byte loads; TFA_EINVAL otherwise). */
 int tfa_assemble_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                         const double* state_nm1, double dt, double* rhs, double* diag_vals, double* offd_vals,
                         void* stream);
