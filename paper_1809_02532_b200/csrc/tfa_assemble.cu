@@ -588,6 +588,13 @@ __global__ void __launch_bounds__(AsmCfg<T>::NT, T >= 10 ? 2 : 4) k_assemble(
     }
   }
   __syncthreads();   // the prologue's neighbour table (plain stores) is visible
+  // packed output: the AUSM warpgroup takes 8 registers per thread from the Maxwell one (136 / 120, no spills in
+  // either role); measured 1.91 against 1.96 ms at c4b.  The BSR kernel, bound by its store stream, does not move
+  // (2.18 against 2.17 ms) and keeps the even split; 152 / 104 and 168 / 88 spill in the Maxwell role and lose.
+  if constexpr (PK && C::AW == 4 && C::MW == 4) {
+    if (warp >= C::AW) asm volatile("setmaxnreg.dec.sync.aligned.u32 120;");
+    else asm volatile("setmaxnreg.inc.sync.aligned.u32 136;");
+  }
   if (warp >= C::AW)
     role_loop<T, NM, NF, PK, 2>(S, JAC, nc, K, state, state_n, state_nm1, inv2dt, fown, cgeo, nbrf, blkmap, ghost, rhs,
                                 vals, vals_o, flags, lim);
