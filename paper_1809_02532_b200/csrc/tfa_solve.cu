@@ -199,7 +199,7 @@ __device__ __forceinline__ double bj_rcp(double d) {
 }
 constexpr size_t BJ_SMEM = sizeof(double) * BJ_WARPS * (BJ_G * BLK + 2 * BJ_G * NEQ) + sizeof(uint64_t) * BJ_WARPS;
 __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, const int32_t* __restrict__ blkmap, int BS,
-                                                               const double* __restrict__ vals,
+                                                               const double* __restrict__ vals, int64_t nblk,
                                                                double* __restrict__ dinv, int32_t* __restrict__ flags) {
   extern __shared__ __align__(128) unsigned char bj_raw[];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -220,6 +220,7 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
   // Jacobian's array of diagonal blocks
   if (lane < nb) {
     const int64_t i = i0 + lane, bd = blkmap ? (int64_t)blkmap[(int64_t)BS * i] : i;
+    TFA_BOUND(flags, bd >= 0 && bd < nblk);
     bulk_load(buf[lane], vals + bd * BLK, (uint32_t)(BLK * sizeof(double)), bar);
   }
   const int g = lane / BJ_L, r = lane - BJ_L * g;
@@ -319,13 +320,13 @@ __global__ void __launch_bounds__(32 * BJ_WARPS, 3) k_block_jacobi(int64_t nc, c
     bulk_wait_read();
   }
 }
-static int launch_block_jacobi(int64_t nc, const int32_t* blkmap, int BS, const double* vals, double* dinv,
-                               int32_t* flags, cudaStream_t st) {
+static int launch_block_jacobi(int64_t nc, const int32_t* blkmap, int BS, const double* vals, int64_t nblk,
+                               double* dinv, int32_t* flags, cudaStream_t st) {
   if ((reinterpret_cast<uintptr_t>(vals) | reinterpret_cast<uintptr_t>(dinv)) & 15)
     return set_error(TFA_EINVAL, "tfa_block_jacobi: the block arrays must be 16-byte aligned");
   // per launch: the attribute belongs to the function on the CURRENT device, and the call is cheap
   TFA_CUDA(cudaFuncSetAttribute(k_block_jacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BJ_SMEM));
-  k_block_jacobi<<<cdiv(nc, BJ_WARPS * BJ_G), 32 * BJ_WARPS, BJ_SMEM, st>>>(nc, blkmap, BS, vals, dinv, flags);
+  k_block_jacobi<<<cdiv(nc, BJ_WARPS * BJ_G), 32 * BJ_WARPS, BJ_SMEM, st>>>(nc, blkmap, BS, vals, nblk, dinv, flags);
   return 0;
 }
 
@@ -640,7 +641,7 @@ int tfa_block_jacobi(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, do
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  TFA_TRY(launch_block_jacobi(m->nc, m->blkmap.p, blk_stride(m->F), bsr_vals, dinv, ctx->flags.p, st));
+  TFA_TRY(launch_block_jacobi(m->nc, m->blkmap.p, blk_stride(m->F), bsr_vals, m->nnzb, dinv, ctx->flags.p, st));
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
@@ -731,7 +732,7 @@ int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_
     TFA_CUDA(ctx->flags.alloc(4));
     TFA_CUDA(cudaMemsetAsync(ctx->flags.p, 0, 16, st));
   }
-  TFA_TRY(launch_block_jacobi(m->nc, nullptr, 0, diag_vals, dinv, ctx->flags.p, st));
+  TFA_TRY(launch_block_jacobi(m->nc, nullptr, 0, diag_vals, m->nc, dinv, ctx->flags.p, st));
   TFA_CUDA(cudaGetLastError());
   return 0;
 }
