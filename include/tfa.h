@@ -179,6 +179,21 @@ int tfa_assemble_gradient(tfa_ctx* ctx, const tfa_mesh* m, const double* state, 
 int tfa_assemble_faces(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                        const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream);
 double* tfa_face_states(tfa_ctx* ctx);
+/* Step a2 without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): face_states [n_cells][F][18] (DEVICE pointer, caller-owned) = the
+ * reconstructed face states tfa_assemble_gradient leaves in the context, bit for bit, from state [n_cells][18]
+ * (DEVICE pointer).  The least-squares coefficients, the only scratch of the step, live in a static device array of
+ * the library -- 32 MiB on every GPU that loads it, held until the process exits -- that holds
+ * TFA_STATIC_MAX_STENCIL stencil entries (STENCIL_PTR[n_cells]: about 170 000 triangles or 260 000 Cartesian
+ * quadrilaterals); a mesh with more returns TFA_EINVAL.  The call allocates and frees nothing, on the device or
+ * through a library, and does not synchronise; the first call on a device looks the array's address up (make it
+ * before a capture starts).  The array is shared by all calls, contexts and streams: every call rewrites the part
+ * it reads (nothing needs clearing), so calls in stream order are independent of each other, but two calls that
+ * OVERLAP on the GPU (different streams or threads) race on it.  Reads the context's numerics only (weight power,
+ * Venkatakrishnan K) and leaves the context's own workspace alone. */
+#define TFA_STATIC_MAX_STENCIL 2097152
+int tfa_face_states_static(const tfa_ctx* ctx, const tfa_mesh* m, const double* state, double* face_states,
+                           void* stream);
 /* Synchronise and report: 0, or TFA_ENONPHYS if any assembly since the last check met a face
  * state with rho <= 0 or T <= 0 (S16), or TFA_ECUDA for a sticky CUDA error. */
 int tfa_check(tfa_ctx* ctx, void* stream);

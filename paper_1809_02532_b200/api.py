@@ -22,6 +22,7 @@ MESH_ITEMS = dict(face_cells=(0, np.int32), cell_faces=(1, np.int32), stencil_pt
 _REORDER = {"none": 0, "rcm": 1, "user": 2, "morton": 3}
 BC_TRANSMISSIVE, BC_GHOST, BC_WALL = 0, 1, 2
 PACKED_BLOCK = 114
+STATIC_MAX_STENCIL = 2097152   # tfa.h TFA_STATIC_MAX_STENCIL
 
 
 def _stream() -> int:
@@ -231,6 +232,14 @@ class Context:
         iface = {"shape": (n,), "typestr": "<f8", "data": (int(ptr), False), "version": 3, "strides": None}
         holder = type("_FaceStates", (), {"__cuda_array_interface__": iface})()
         return torch.as_tensor(holder, device="cuda").view(mesh.n_cells, mesh.max_faces, NEQ)
+
+    def face_states_static(self, mesh: Mesh, state, out=None) -> torch.Tensor:
+        """tfa_face_states_static: step a2 into the caller's [n_cells][F][18] buffer with the scratch in the library's
+        static device array (no allocation in the call when `out` is given; STATIC_MAX_STENCIL entries at most)."""
+        if out is None:
+            out = torch.empty((mesh.n_cells, mesh.max_faces, NEQ), dtype=torch.float64, device=state.device)
+        _lib.check(_lib.load().tfa_face_states_static(self._h, mesh._h, _dp(state), _dp(out), _stream()))
+        return out
 
     def assemble_faces(self, mesh: Mesh, state, state_n=None, state_nm1=None, dt=1e-3, rhs=None, vals=None):
         """tfa_assemble_faces: steps a3..a7 on the context's face states.  vals must be given (its size is the

@@ -18,7 +18,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libtfa.so")
-SOURCES = ["tfa_mesh.cu", "tfa_kernels.cu", "tfa_assemble.cu", "tfa_solve.cu", "tfa_api.cu", "tfa_shard.cu"]
+SOURCES = ["tfa_mesh.cu", "tfa_kernels.cu", "tfa_assemble.cu", "tfa_solve.cu", "tfa_api.cu", "tfa_shard.cu",
+           "tfa_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + os.environ.get("TFA_NVCC_EXTRA", "").split()
 
