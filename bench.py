@@ -499,8 +499,35 @@ def main():
             torch.cuda.synchronize()
             gp_s = time.perf_counter() - tt
         ctx.check()
+        # mixed precision: Krylov cycles on FP32 copies of the packed matrix and of the inverses, restarts in FP64
+        tt = time.perf_counter()
+        d32, o32 = api.packed_to_f32(mesh, pk_d, pk_o)
+        dinv32 = api.to_f32(dinv_p)
+        torch.cuda.synchronize()
+        conv_s = time.perf_counter() - tt
+        mixed = {}
+        for tol in (1e-6, 1e-10):
+            for _ in range(2):
+                torch.cuda.synchronize()
+                tt = time.perf_counter()
+                xm, itm, relm = ctx.gmres_packed_f32(mesh, pk_d, pk_o, d32, o32, bvec, dinv32=dinv32, restart=30,
+                                                     max_iters=300, rtol=tol)
+                torch.cuda.synchronize()
+                gm32_s = time.perf_counter() - tt
+            mixed["rtol_%g" % tol] = {"iterations": itm, "relative_residual": relm, "seconds": gm32_s}
+        for _ in range(2):
+            torch.cuda.synchronize()
+            tt = time.perf_counter()
+            xp10, itp10, relp10 = ctx.gmres_packed(mesh, pk_d, pk_o, bvec, dinv=dinv_p, restart=30, max_iters=300,
+                                                   rtol=1e-10)
+            torch.cuda.synchronize()
+            gp10_s = time.perf_counter() - tt
+        mixed["fp64_rtol_1e-10"] = {"iterations": itp10, "relative_residual": relp10, "seconds": gp10_s}
+        mixed["convert_seconds"] = conv_s
+        mixed["max_diff_to_fp64_solution"] = float((xm - xp10).abs().max() / xp10.abs().max())
+        ctx.check()
         pspmv_bytes = nc * 2592 + (nnzb - nc) * 912 + 2 * n * 8 + nnzb * 4 + nc * 4
-        del pk_d, pk_o, dinv_p, xp
+        del pk_d, pk_o, dinv_p, xp, d32, o32, dinv32, xm, xp10
         spmv_bytes = nnzb * 2592 + 2 * n * 8 + nnzb * 4 + nc * 4
         solve = {"spmv_ms": spmv_ms, "spmv_algorithmic_bytes": spmv_bytes,
                  "spmv_gbs": spmv_bytes / (spmv_ms * 1e-3) / 1e9, "block_jacobi_ms": bj_ms,
@@ -509,7 +536,8 @@ def main():
                            "preconditioner": "block-Jacobi (18x18 diagonal blocks)"},
                  "packed": {"spmv_ms": pspmv_ms, "spmv_algorithmic_bytes": pspmv_bytes,
                             "spmv_gbs": pspmv_bytes / (pspmv_ms * 1e-3) / 1e9,
-                            "gmres": {"iterations": itp, "relative_residual": relp, "seconds": gp_s}},
+                            "gmres": {"iterations": itp, "relative_residual": relp, "seconds": gp_s},
+                            "gmres_f32_cycles": mixed},
                  "gmres_jfnk": {"restart": 30, "rtol": 1e-6, "iterations": itj, "relative_residual": relj,
                                 "seconds": gj_s, "operator": "tfa_jvp (matrix-free), same preconditioner"}}
         del xv, yv, dinv, xs, xj

@@ -268,6 +268,21 @@ int tfa_packed_to_bsr(const tfa_mesh* m, const double* diag_vals, const double* 
 int tfa_packed_spmv(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, const double* x, double* y,
                     void* stream);
 int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, double* dinv, void* stream);
+/* Mixed-precision solve on the packed Jacobian: the Krylov cycles of GMRES(restart) run on an FP32 copy of the matrix
+ * (and, when dinv32 is given, of the block-Jacobi inverses; NULL = no preconditioner) with FP64 vectors and FP64
+ * accumulation; the residual b - A x at every restart, and the one reported in info[1], is computed with the FP64
+ * matrix, and a cycle ends once it has reduced its own residual by 1e-5 (iterative refinement with GMRES as the
+ * inner solver: the FP32 copy perturbs the operator by 6e-8 relative, which a restart corrects).  Same stopping
+ * rule, same error codes as tfa_gmres_packed.  The copies are the caller's: tfa_packed_to_f32 fills
+ * diag32 [n_cells][18][18] and offd32 [nnzb - n_cells][TFA_PACKED_BLOCK_F32] (114 entries + 2 of padding: blocks
+ * 464 bytes apart), tfa_to_f32 converts any array (the inverses dinv -> dinv32).  DEVICE pointers, 16-byte aligned. */
+#define TFA_PACKED_BLOCK_F32 116
+int tfa_to_f32(const double* src, float* dst, int64_t n, void* stream);
+int tfa_packed_to_f32(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, float* diag32, float* offd32,
+                      void* stream);
+int tfa_gmres_packed_f32(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, const double* offd_vals,
+                         const float* diag32, const float* offd32, const float* dinv32, const double* b, double* x,
+                         int restart, int max_iters, double rtol, double* info, void* stream);
 int tfa_gmres_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, const double* offd_vals,
                      const double* dinv, const double* b, double* x, int restart, int max_iters, double rtol,
                      double* info, void* stream);

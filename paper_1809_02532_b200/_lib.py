@@ -57,6 +57,9 @@ SYMBOLS = {
     "tfa_packed_spmv": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "tfa_block_jacobi_packed": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "tfa_gmres_packed": (_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _int, _int, _dbl, C.POINTER(C.c_double), _vp]),
+    "tfa_to_f32": (_int, [_vp, _vp, _i64, _vp]),
+    "tfa_packed_to_f32": (_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "tfa_gmres_packed_f32": (_int, [_vp] * 9 + [_int, _int, _dbl, C.POINTER(C.c_double), _vp]),
     "tfa_assemble_gradient": (_int, [_vp, _vp, _vp, _vp]),
     "tfa_assemble_faces": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "tfa_face_states": (_vp, [_vp]),

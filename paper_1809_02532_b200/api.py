@@ -41,6 +41,14 @@ def _dp(t: torch.Tensor | None):
     return C.c_void_p(t.data_ptr())
 
 
+def _fp(t: torch.Tensor | None):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise ValueError("expected a contiguous float32 CUDA tensor")
+    return C.c_void_p(t.data_ptr())
+
+
 def default_physics(src=None) -> Physics:
     p = Physics()
     _lib.load().tfa_default_physics(C.byref(p))
@@ -217,6 +225,17 @@ class Context:
         info = (C.c_double * 2)()
         _lib.check(_lib.load().tfa_gmres_packed(self._h, mesh._h, _dp(diag), _dp(offd), _dp(dinv), _dp(b), _dp(x),
                                                 int(restart), int(max_iters), float(rtol), info, _stream()))
+        return x, int(info[0]), float(info[1])
+
+    def gmres_packed_f32(self, mesh: Mesh, diag, offd, diag32, offd32, b, x=None, dinv32=None, restart=30,
+                         max_iters=300, rtol=1e-8):
+        """tfa_gmres_packed_f32: Krylov cycles on the FP32 copies (packed_to_f32, to_f32), restarts in FP64."""
+        if x is None:
+            x = torch.zeros_like(b)
+        info = (C.c_double * 2)()
+        _lib.check(_lib.load().tfa_gmres_packed_f32(self._h, mesh._h, _dp(diag), _dp(offd), _fp(diag32), _fp(offd32),
+                                                    _fp(dinv32), _dp(b), _dp(x), int(restart), int(max_iters),
+                                                    float(rtol), info, _stream()))
         return x, int(info[0]), float(info[1])
 
     def assemble_gradient(self, mesh: Mesh, state):
@@ -539,6 +558,25 @@ def packed_spmv(mesh: Mesh, diag, offd, x, y=None):
         y = torch.empty_like(x)
     _lib.check(_lib.load().tfa_packed_spmv(mesh._h, _dp(diag), _dp(offd), _dp(x), _dp(y), _stream()))
     return y
+
+
+PACKED_BLOCK_F32 = 116
+
+
+def to_f32(src, dst=None):
+    """tfa_to_f32: an FP32 copy of an FP64 device array."""
+    if dst is None:
+        dst = torch.empty(src.shape, dtype=torch.float32, device=src.device)
+    _lib.check(_lib.load().tfa_to_f32(_dp(src), _fp(dst), src.numel(), _stream()))
+    return dst
+
+
+def packed_to_f32(mesh: Mesh, diag, offd):
+    """tfa_packed_to_f32: FP32 copies of the packed Jacobian for gmres_packed_f32 (off-diagonal blocks 116 apart)."""
+    diag32 = torch.empty((mesh.n_cells, NEQ, NEQ), dtype=torch.float32, device=diag.device)
+    offd32 = torch.empty((mesh.nnzb - mesh.n_cells, PACKED_BLOCK_F32), dtype=torch.float32, device=diag.device)
+    _lib.check(_lib.load().tfa_packed_to_f32(mesh._h, _dp(diag), _dp(offd), _fp(diag32), _fp(offd32), _stream()))
+    return diag32, offd32
 
 
 def packed_to_bsr(mesh: Mesh, diag, offd, vals=None):

@@ -145,6 +145,119 @@ static int launch_packed_spmv(const tfa_mesh* m, const double* dvals, const doub
   return 0;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Mixed precision (tfa_gmres_packed_f32): the packed Jacobian and the block-diagonal preconditioner stored in FP32,
+// vectors and accumulation in FP64.  Off-diagonal blocks sit TFA_PACKED_BLOCK_F32 = 116 floats apart (464 bytes: a
+// 16-byte multiple, so that a row's blocks can come in by TMA and the field rows be read with 16-byte loads).
+// ------------------------------------------------------------------------------------------------
+constexpr int PKF = TFA_PACKED_BLOCK_F32;
+__global__ void k_to_f32(int64_t n, const double* __restrict__ src, float* __restrict__ dst) {
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)blockDim.x * gridDim.x)
+    dst[e] = (float)src[e];
+}
+__global__ void k_offd_to_f32(int64_t nblk, const double* __restrict__ src, float* __restrict__ dst) {
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < nblk * PKF; t += (int64_t)blockDim.x * gridDim.x) {
+    const int64_t b = t / PKF;
+    const int e = (int)(t - b * PKF);
+    dst[t] = e < TFA_PACKED_BLOCK ? (float)src[b * TFA_PACKED_BLOCK + e] : 0.0f;
+  }
+}
+__global__ void __launch_bounds__(SV_T) k_packed_spmv_f32(int64_t nc, int BS, const int32_t* __restrict__ rowptr,
+                                                         const int32_t* __restrict__ col,
+                                                         const int32_t* __restrict__ blkmap,
+                                                         const float* __restrict__ dvals, const float* __restrict__ ovals,
+                                                         const double* __restrict__ x, double* __restrict__ y) {
+  extern __shared__ __align__(128) unsigned char ps_raw[];
+  float* const sm = reinterpret_cast<float*>(ps_raw + 16);
+  uint64_t* const bar = reinterpret_cast<uint64_t*>(ps_raw);
+  const int r = threadIdx.x % NEQ;
+  const int64_t i0 = blockIdx.x * (int64_t)SV_CELLS, i = i0 + threadIdx.x / NEQ;
+  const int64_t iend = min(i0 + SV_CELLS, nc);
+  const int64_t s0 = rowptr[i0] - i0;   // the CTA's first off-diagonal slot
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_arrive_expect_tx(bar, (uint32_t)((rowptr[iend] - iend - s0) * (PKF * sizeof(float))));
+  }
+  __syncthreads();
+  const bool live = i < nc;
+  int64_t b0 = 0, b1 = 0;
+  if (live) {
+    b0 = rowptr[i];
+    b1 = rowptr[i + 1];
+    if (r == 0 && b1 - b0 > 1)
+      bulk_load(sm + (b0 - i - s0) * PKF, ovals + (b0 - i) * PKF, (uint32_t)((b1 - b0 - 1) * (PKF * sizeof(float))), bar);
+  }
+  double acc = 0.0;
+  if (live) {
+    const float2* __restrict__ a = reinterpret_cast<const float2*>(dvals + i * BLK + r * NEQ);
+    const double2* __restrict__ xv = reinterpret_cast<const double2*>(x + NEQ * i);
+#pragma unroll
+    for (int c = 0; c < NEQ / 2; ++c) {
+      const float2 av = a[c];
+      const double2 xx = xv[c];
+      acc = fma((double)av.x, xx.x, acc);
+      acc = fma((double)av.y, xx.y, acc);
+    }
+  }
+  mbar_wait(bar, 0);
+  if (!live) return;
+  int base, n, c0, cs, cT;
+  packed_row(r, base, n, c0, cs, cT);
+  const int64_t bd = blkmap[(int64_t)BS * i];
+  const float* __restrict__ a = sm + (b0 - i - s0) * PKF + base;
+  for (int64_t b = b0; b < b1; ++b) {
+    if (b == bd) continue;
+    const double* __restrict__ xj = x + NEQ * (int64_t)col[b];
+    if (n == 8) {
+      const float4* __restrict__ a4 = reinterpret_cast<const float4*>(a);
+      const double2* __restrict__ x2 = reinterpret_cast<const double2*>(xj);
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const float4 av = a4[c];
+        const double2 xa = x2[2 * c], xb = x2[2 * c + 1];
+        acc = fma((double)av.y, xa.y, fma((double)av.x, xa.x, acc));
+        acc = fma((double)av.w, xb.y, fma((double)av.z, xb.x, acc));
+      }
+    } else {
+      acc = fma((double)a[0], xj[c0], acc);
+      acc = fma((double)a[1], xj[cs], acc);
+      acc = fma((double)a[2], xj[cs + 1], acc);
+      acc = fma((double)a[3], xj[cs + 2], acc);
+      acc = fma((double)a[4], xj[cT], acc);
+    }
+    a += PKF;
+  }
+  y[NEQ * i + r] = acc;
+}
+// z = D v with D = [nc][18][18] in FP32 (the preconditioner's application in the mixed-precision solve)
+__global__ void __launch_bounds__(SV_T) k_diag_spmv_f32(int64_t nc, const float* __restrict__ dv,
+                                                       const double* __restrict__ x, double* __restrict__ y) {
+  const int r = threadIdx.x % NEQ;
+  const int64_t i = blockIdx.x * (int64_t)SV_CELLS + threadIdx.x / NEQ;
+  if (i >= nc) return;
+  const float2* __restrict__ a = reinterpret_cast<const float2*>(dv + i * BLK + r * NEQ);
+  const double2* __restrict__ xv = reinterpret_cast<const double2*>(x + NEQ * i);
+  double acc = 0.0;
+#pragma unroll
+  for (int c = 0; c < NEQ / 2; ++c) {
+    const float2 av = a[c];
+    const double2 xx = xv[c];
+    acc = fma((double)av.x, xx.x, acc);
+    acc = fma((double)av.y, xx.y, acc);
+  }
+  y[NEQ * i + r] = acc;
+}
+static int launch_packed_spmv_f32(const tfa_mesh* m, const float* dvals, const float* ovals, const double* x, double* y,
+                                  cudaStream_t st) {
+  if ((reinterpret_cast<uintptr_t>(dvals) | reinterpret_cast<uintptr_t>(ovals) | reinterpret_cast<uintptr_t>(x)) & 15)
+    return set_error(TFA_EINVAL, "tfa_gmres_packed_f32: the FP32 arrays and x must be 16-byte aligned");
+  const size_t smem = 16 + sizeof(float) * SV_CELLS * m->F * PKF;
+  k_packed_spmv_f32<<<cdiv(m->nc, SV_CELLS), SV_T, smem, st>>>(m->nc, blk_stride(m->F), m->bsr_rowptr.p, m->bsr_col.p,
+                                                              m->blkmap.p, dvals, ovals, x, y);
+  return 0;
+}
+
 // packed -> BSR: thread (block b, entry e) of the mesh's pattern
 __global__ void k_packed_to_bsr(int64_t nc, int64_t nnzb, int BS, const int32_t* __restrict__ rowptr,
                                 const int32_t* __restrict__ blkmap, const int32_t* __restrict__ row_of_block,
@@ -479,7 +592,12 @@ struct Gm {
   double *part, *out;   // reduction scratch (device)
   double host[MAXK];
   std::function<int(const double*, double*)> op;   // y = A x when the matrix is not assembled (JFNK)
+  // mixed precision: the operator of the Krylov cycle (FP32 matrix) -- the residual at a restart still uses spmv --
+  // and the preconditioner's application (FP32 blocks)
+  std::function<int(const double*, double*)> op_inner;
+  std::function<void(const double*, double*)> pre;
 
+  int spmv_inner(const double* x, double* y) const { return op_inner ? op_inner(x, y) : spmv(x, y); }
   int spmv(const double* x, double* y) const {
     if (op) return op(x, y);
     if (vals_o)
@@ -490,7 +608,8 @@ struct Gm {
   }
   // z = M^-1 v (block-diagonal product), or a copy without preconditioner
   void precond(const double* v, double* z) const {
-    if (dinv) k_bsr_spmv<true><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, nullptr, nullptr, dinv, v, z);
+    if (pre) pre(v, z);
+    else if (dinv) k_bsr_spmv<true><<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, nullptr, nullptr, dinv, v, z);
     else k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, v, 0.0, nullptr, z);
   }
   // host[j] = V_j . w for j < k (synchronises)
@@ -510,7 +629,9 @@ using namespace tfa;
 
 static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const double* dinv,
                       std::function<int(const double*, double*)> op, const double* b, double* x, int restart,
-                      int max_iters, double rtol, double* info, void* stream, const double* offd_vals = nullptr) {
+                      int max_iters, double rtol, double* info, void* stream, const double* offd_vals = nullptr,
+                      std::function<int(const double*, double*)> op_inner = nullptr,
+                      std::function<void(const double*, double*)> pre = nullptr, double inner_floor = 0.0) {
   if (restart < 1 || restart > MAXK - 2 || max_iters < 0 || !(rtol >= 0.0))
     return set_error(TFA_EINVAL, "tfa_gmres: restart must be in 1..62, max_iters >= 0, rtol >= 0");
   cudaStream_t st = (cudaStream_t)stream;
@@ -521,7 +642,7 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
   double* V = ctx->krylov.p;              // V_0 .. V_mk
   double* w = V + (int64_t)(mk + 1) * n;  // work vector
   double* z = w + n;                      // preconditioned vector
-  Gm G{m, bsr_vals, dinv, offd_vals, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, op};
+  Gm G{m, bsr_vals, dinv, offd_vals, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, op, op_inner, pre};
 
   TFA_TRY(G.dots(1, b, n, b));
   const double bnorm = std::sqrt(G.host[0]);
@@ -550,7 +671,7 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
     int k = 0;
     for (; k < mk && iters < max_iters; ++k, ++iters) {
       G.precond(V + (int64_t)k * n, z);
-      TFA_TRY(G.spmv(z, w));
+      TFA_TRY(G.spmv_inner(z, w));
       // classical Gram-Schmidt (all projections from one pass over the basis), repeated when it cancelled more
       // than a factor 10 of the vector (the Daniel-Gragg-Kaufman-Stewart test with eta = 0.1: the loss of
       // orthogonality of a single pass grows like eps / eta^2, and on the preconditioned systems of the method a
@@ -591,7 +712,9 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
       h[k + 1] = 0.0;
       g[k + 1] = -sn[k] * g[k];
       g[k] = cs[k] * g[k];
-      if (std::fabs(g[k + 1]) <= rtol * bnorm || hk1 == 0.0) {
+      // (mixed precision: a cycle ends once it has reduced ITS residual by inner_floor -- below that the FP32
+      // operator's rounding, not the Krylov space, limits the true residual, which the restart recomputes in FP64)
+      if (std::fabs(g[k + 1]) <= rtol * bnorm || hk1 == 0.0 || std::fabs(g[k + 1]) <= inner_floor * beta) {
         ++k;
         ++iters;
         break;
@@ -747,6 +870,45 @@ int tfa_gmres_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, c
   if (!diag_vals || !b || !x || (!offd_vals && m->nnzb > m->nc)) return set_error(TFA_EINVAL, "null argument");
   return gmres_core(ctx, m, diag_vals, dinv, nullptr, b, x, restart, max_iters, rtol, info, stream,
                     offd_vals ? offd_vals : diag_vals);
+}
+
+// ---- mixed precision on the packed Jacobian (include/tfa.h) ----
+int tfa_to_f32(const double* src, float* dst, int64_t n, void* stream) {
+  if (n < 0 || (n > 0 && (!src || !dst))) return set_error(TFA_EINVAL, "bad argument");
+  if (n == 0) return 0;
+  k_to_f32<<<1184, 256, 0, (cudaStream_t)stream>>>(n, src, dst);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+int tfa_packed_to_f32(const tfa_mesh* m, const double* diag_vals, const double* offd_vals, float* diag32, float* offd32,
+                      void* stream) {
+  if (!m) return set_error(TFA_EINVAL, "null argument");
+  if (m->nc == 0) return 0;
+  const int64_t no = m->nnzb - m->nc;
+  if (!diag_vals || !diag32 || (no > 0 && (!offd_vals || !offd32))) return set_error(TFA_EINVAL, "null argument");
+  k_to_f32<<<1184, 256, 0, (cudaStream_t)stream>>>(m->nc * (int64_t)BLK, diag_vals, diag32);
+  if (no > 0) k_offd_to_f32<<<1184, 256, 0, (cudaStream_t)stream>>>(no, offd_vals, offd32);
+  TFA_CUDA(cudaGetLastError());
+  return 0;
+}
+int tfa_gmres_packed_f32(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, const double* offd_vals,
+                         const float* diag32, const float* offd32, const float* dinv32, const double* b, double* x,
+                         int restart, int max_iters, double rtol, double* info, void* stream) {
+  if (!ctx || !m || !info) return set_error(TFA_EINVAL, "null argument");
+  info[0] = 0.0;
+  info[1] = 0.0;
+  if (m->nc == 0) return 0;
+  const bool offd = m->nnzb > m->nc;
+  if (!diag_vals || !diag32 || !b || !x || (offd && (!offd_vals || !offd32))) return set_error(TFA_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  auto inner = [=](const double* xin, double* yout) -> int {
+    return launch_packed_spmv_f32(m, diag32, offd ? offd32 : diag32, xin, yout, st);
+  };
+  std::function<void(const double*, double*)> pre;
+  if (dinv32)
+    pre = [=](const double* v, double* z) { k_diag_spmv_f32<<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, dinv32, v, z); };
+  return gmres_core(ctx, m, diag_vals, nullptr, nullptr, b, x, restart, max_iters, rtol, info, stream,
+                    offd ? offd_vals : diag_vals, inner, pre, 1e-5);
 }
 
 // ---- matrix-free operator (the paper's future work, L130) ----

@@ -112,6 +112,21 @@ def test_packed_assembly_parity_and_solve(api, orc, W, case):
     xb, itb, relb = ctx.gmres(g, vals_b, b, dinv=dinv_b, restart=30, max_iters=200, rtol=1e-10)
     assert relp <= 1e-10 and abs(itp - itb) <= 1
     assert float((xp - xb).abs().max()) <= 1e-7 * float(xb.abs().max())
+    # mixed precision (tfa_gmres_packed_f32): Krylov cycles on FP32 copies, restarts and the reported residual in
+    # FP64 -- the same tolerance is reached, and the residual it reports is the true FP64 one
+    d32, o32 = api.packed_to_f32(g, diag, offd)
+    assert o32.shape[1] == 116 and float(o32[:, 114:].abs().max()) == 0.0
+    assert torch.equal(d32, diag.to(torch.float32)) and torch.equal(o32[:, :114], offd.to(torch.float32))
+    dinv32 = api.to_f32(dinv_p)
+    for tol in (1e-6, 1e-10):
+        xm, itm, relm = ctx.gmres_packed_f32(g, diag, offd, d32, o32, b, dinv32=dinv32, restart=30, max_iters=200, rtol=tol)
+        true_rel = float((b - api.bsr_spmv(g, vals_b, xm)).norm() / b.norm())
+        assert relm <= tol and abs(true_rel - relm) <= 1e-3 * relm + 1e-15, (tol, relm, true_rel)
+        x64, it64, _ = ctx.gmres_packed(g, diag, offd, b, dinv=dinv_p, restart=30, max_iters=200, rtol=tol)
+        assert itm <= it64 + max(3, it64 // 5), (tol, itm, it64)
+    assert float((xm - xb).abs().max()) <= 1e-7 * float(xb.abs().max())
+    xu, itu, relu = ctx.gmres_packed_f32(g, diag, offd, d32, o32, b, restart=30, max_iters=600, rtol=1e-6)   # no preconditioner
+    assert relu <= 1e-6
     ctx.check()
 
 
