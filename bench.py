@@ -528,6 +528,22 @@ def main():
         ctx.check()
         pspmv_bytes = nc * 2592 + (nnzb - nc) * 912 + 2 * n * 8 + nnzb * 4 + nc * 4
         del pk_d, pk_o, dinv_p, xp, d32, o32, dinv32, xm, xp10
+        # one Newton sub-iteration of Eq. 14 as one call (tfa_implicit_step): assembled BSR path against mode 2
+        work = dict(rhs=torch.empty((nc, 18), dtype=torch.float64, device="cuda"), vals=vals, dinv=dinv,
+                    dP=torch.empty((nc, 18), dtype=torch.float64, device="cuda"))
+        newton = {}
+        for mode, key in ((False, "bsr_fp64"), ("packed_f32", "packed_f32_cycles")):
+            for _ in range(2):
+                S = P.clone()
+                torch.cuda.synchronize()
+                tt = time.perf_counter()
+                (nit, upd, gits, lrel), _ = ctx.implicit_step(mesh, S, Pn, Pnm1, wl.dt, work=work, max_newton=1,
+                                                              rtol=1e-6, matrix_free=mode)
+                torch.cuda.synchronize()
+                nw_s = time.perf_counter() - tt
+            newton[key] = {"seconds": nw_s, "gmres_iterations": gits, "linear_residual": lrel, "update": upd}
+        ctx.check()
+        del work, S
         spmv_bytes = nnzb * 2592 + 2 * n * 8 + nnzb * 4 + nc * 4
         solve = {"spmv_ms": spmv_ms, "spmv_algorithmic_bytes": spmv_bytes,
                  "spmv_gbs": spmv_bytes / (spmv_ms * 1e-3) / 1e9, "block_jacobi_ms": bj_ms,
@@ -538,6 +554,7 @@ def main():
                             "spmv_gbs": pspmv_bytes / (pspmv_ms * 1e-3) / 1e9,
                             "gmres": {"iterations": itp, "relative_residual": relp, "seconds": gp_s},
                             "gmres_f32_cycles": mixed},
+                 "newton_iteration": newton,
                  "gmres_jfnk": {"restart": 30, "rtol": 1e-6, "iterations": itj, "relative_residual": relj,
                                 "seconds": gj_s, "operator": "tfa_jvp (matrix-free), same preconditioner"}}
         del xv, yv, dinv, xs, xj

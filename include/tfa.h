@@ -238,6 +238,9 @@ int tfa_gmres(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, const dou
  * return P^{n+1}; state_n, state_nm1: P^n, P^{n-1} (must not alias state).  Work arrays, DEVICE pointers owned by the
  * caller: rhs and dP [n_cells][18], bsr_vals [nnzb][18][18], dinv [n_cells][18][18].  matrix_free != 0 solves with
  * the matrix-free operator (tfa_gmres_jfnk; the assembled Jacobian then only feeds the preconditioner).
+ * matrix_free == 2 is the fastest assembled variant: packed Jacobian (tfa_assemble_packed; bsr_vals is then only
+ * storage and holds the packed form on return: diagonal blocks first, off-diagonal blocks behind them) and the
+ * mixed-precision solve tfa_gmres_packed_f32, whose FP32 copies live in the context; not on a shard's mesh.
  * info[0] = Newton iterations done, info[1] = ||dP||_2 / (1 + ||P||_2) of the last one, info[2] = GMRES iterations
  * in total, info[3] = relative residual of the last linear solve.  Errors of the steps it calls are passed on. */
 int tfa_implicit_step(tfa_ctx* ctx, const tfa_mesh* m, double* state, const double* state_n, const double* state_nm1,

@@ -305,7 +305,8 @@ class Context:
                       restart=30, max_iters=300, rtol=1e-8, matrix_free=False):
         """tfa_implicit_step: Newton sub-iterations of one BDF2 step; `state` (initial guess) is updated in place to
         P^{n+1}.  Returns (newton_iterations, last relative update, gmres_iterations, last linear residual) and the
-        work dictionary (rhs, vals, dinv, dP), which may be passed in again."""
+        work dictionary (rhs, vals, dinv, dP), which may be passed in again.  matrix_free: False (assembled BSR
+        matrix), True (tfa_gmres_jfnk) or "packed_f32" (mode 2: packed Jacobian + mixed-precision solve)."""
         if work is None:
             f = dict(dtype=torch.float64, device=state.device)
             work = dict(rhs=torch.empty((mesh.n_cells, NEQ), **f), vals=torch.empty((mesh.nnzb, NEQ, NEQ), **f),
@@ -314,7 +315,8 @@ class Context:
         _lib.check(_lib.load().tfa_implicit_step(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1), float(dt),
                                                  _dp(work["rhs"]), _dp(work["vals"]), _dp(work["dinv"]), _dp(work["dP"]),
                                                  int(max_newton), float(newton_tol), int(restart), int(max_iters),
-                                                 float(rtol), int(bool(matrix_free)), info, _stream()))
+                                                 float(rtol), 2 if matrix_free == "packed_f32" else int(bool(matrix_free)), info,
+                                                 _stream()))
         return (int(info[0]), float(info[1]), int(info[2]), float(info[3])), work
 
     def jvp(self, mesh: Mesh, state, v, state_n=None, state_nm1=None, dt=1e-3, eps=0.0, out=None):

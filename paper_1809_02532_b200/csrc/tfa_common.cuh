@@ -138,6 +138,8 @@ struct tfa_ctx {
   tfa::DevBuf<double> krylov, red;
   // matrix-free operator: perturbed state and its residual; the base residual
   tfa::DevBuf<double> jfnk, jfnk0;
+  // FP32 copies of the packed Jacobian and of the block-Jacobi inverses (tfa_implicit_step, mode 2)
+  tfa::DevBuf<float> mixed;
   // device staging buffers of tfa_assemble_host
   tfa::DevBuf<double> stage_state[3], stage_rhs, stage_vals;
   int launches = 0;

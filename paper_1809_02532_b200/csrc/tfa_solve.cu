@@ -794,11 +794,32 @@ int tfa_implicit_step(tfa_ctx* ctx, const tfa_mesh* m, double* state, const doub
   const int64_t n = (int64_t)NEQ * m->nc;
   if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
   double gm[2];
+  if (matrix_free < 0 || matrix_free > 2) return set_error(TFA_EINVAL, "tfa_implicit_step: mode must be 0, 1 or 2");
+  // mode 2: packed Jacobian inside the caller's value array (it always fits), FP32 copies in the context
+  const int64_t n_offd = m->nnzb - m->nc;
+  double *pk_d = bsr_vals, *pk_o = bsr_vals + m->nc * (int64_t)BLK;
+  float *d32 = nullptr, *o32 = nullptr, *i32 = nullptr;
+  if (matrix_free == 2) {
+    const int64_t need = 2 * m->nc * (int64_t)BLK + n_offd * PKF;
+    if (ctx->mixed.n < need) TFA_CUDA(ctx->mixed.alloc(need));
+    d32 = ctx->mixed.p;
+    o32 = d32 + m->nc * (int64_t)BLK;
+    i32 = o32 + n_offd * PKF;
+  }
   for (int it = 0; it < max_newton; ++it) {
-    TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream));
-    TFA_TRY(tfa_block_jacobi(ctx, m, bsr_vals, dinv, stream));
+    if (matrix_free == 2) {
+      TFA_TRY(tfa_assemble_packed(ctx, m, state, state_n, state_nm1, dt, rhs, pk_d, pk_o, stream));
+      TFA_TRY(tfa_block_jacobi_packed(ctx, m, pk_d, dinv, stream));
+      TFA_TRY(tfa_packed_to_f32(m, pk_d, pk_o, d32, o32, stream));
+      TFA_TRY(tfa_to_f32(dinv, i32, m->nc * (int64_t)BLK, stream));
+    } else {
+      TFA_TRY(tfa_assemble(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream));
+      TFA_TRY(tfa_block_jacobi(ctx, m, bsr_vals, dinv, stream));
+    }
     TFA_CUDA(cudaMemsetAsync(dP, 0, sizeof(double) * n, st));
-    if (matrix_free)
+    if (matrix_free == 2)
+      TFA_TRY(tfa_gmres_packed_f32(ctx, m, pk_d, pk_o, d32, o32, i32, rhs, dP, restart, max_iters, rtol, gm, stream));
+    else if (matrix_free)
       TFA_TRY(tfa_gmres_jfnk(ctx, m, state, state_n, state_nm1, dt, dinv, rhs, dP, restart, max_iters, rtol, gm, stream));
     else
       TFA_TRY(tfa_gmres(ctx, m, bsr_vals, dinv, rhs, dP, restart, max_iters, rtol, gm, stream));

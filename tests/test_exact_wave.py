@@ -420,6 +420,22 @@ def test_native_implicit_step_equals_the_loop_of_its_parts(W):
     for R in (Q, Q4):
         err = np.abs(R.cpu().numpy() - Pex).max(axis=0)
         assert (err[[1, 2, 11, 12]] < 0.06 * change[[1, 2, 11, 12]]).all()
+    # mode 2 (packed Jacobian, GMRES cycles in FP32, restarts in FP64): the same Newton iterates up to the linear
+    # solves' tolerance -- every update solves the same system to rtol = 1e-9
+    Q5 = Pn.clone()
+    (n5, u5, g5, rel5), _ = ctx.implicit_step(g, Q5, Pn, Pm, dt, work=work, max_newton=4, rtol=1e-9,
+                                              matrix_free="packed_f32")
+    ctx.check()
+    assert n5 == 4 and rel5 <= 1e-9 and g5 <= gits + max(4, gits // 5), (g5, gits)
+    upd = float((Q - Pn).abs().max())
+    assert float((Q5 - Q).abs().max()) <= 1e-6 * upd
+    # on return the value array holds the packed form of the last assembly (here: at P^n, one Newton iteration)
+    Q6 = Pn.clone()
+    ctx.implicit_step(g, Q6, Pn, Pm, dt, work=work, max_newton=1, rtol=1e-9, matrix_free="packed_f32")
+    _, diag6, offd6 = ctx.assemble_packed(g, Pn, Pn, Pm, dt)
+    flat = work["vals"].view(-1)
+    assert torch.equal(flat[:diag6.numel()], diag6.view(-1))
+    assert torch.equal(flat[diag6.numel():diag6.numel() + offd6.numel()], offd6.view(-1))
     with pytest.raises(api.TfaError):
         ctx.implicit_step(g, Pn, Pn, Pm, dt, work=work)          # state must not alias P^n
     ctx.check()
