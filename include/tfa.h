@@ -272,8 +272,9 @@ int tfa_packed_spmv(const tfa_mesh* m, const double* diag_vals, const double* of
                     void* stream);
 int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_vals, double* dinv, void* stream);
 /* Mixed-precision solve on the packed Jacobian: the Krylov cycles of GMRES(restart) run on an FP32 copy of the matrix
- * (and, when dinv32 is given, of the block-Jacobi inverses; NULL = no preconditioner) with FP64 vectors and FP64
- * accumulation; the residual b - A x at every restart, and the one reported in info[1], is computed with the FP64
+ * (and, when dinv32 is given, of the block-Jacobi inverses; NULL = no preconditioner) and keep their basis vectors
+ * in FP32 (each is rounded once, when it is normalised; the projections, the work vector, the sums and the Hessenberg
+ * problem are FP64); the residual b - A x at every restart, and the one reported in info[1], is computed with the FP64
  * matrix, and a cycle ends once it has reduced its own residual by 1e-5 (iterative refinement with GMRES as the
  * inner solver: the FP32 copy perturbs the operator by 6e-8 relative, which a restart corrects).  Same stopping
  * rule, same error codes as tfa_gmres_packed.  The copies are the caller's: tfa_packed_to_f32 fills

@@ -1,6 +1,7 @@
 // tfa_solve.cu — the linear solve of Eq. 14 (L123) on the assembled BSR system: BSR
 // matrix-vector product, block-Jacobi preconditioner, restarted GMRES (the paper's solver configuration,
 // L28, L392).  Kernels are HBM-bound streams; the Hessenberg least-squares problem lives on the host.
+#include <algorithm>
 #include <cmath>
 #include <functional>
 #include <vector>
@@ -573,6 +574,121 @@ __global__ void __launch_bounds__(RED_T) k_sub_combination(int64_t n, int k, con
     part[(int64_t)blockIdx.x * MAXK] = t;
   }
 }
+// ---- the same three kernels for a Krylov basis stored in FP32 (mixed-precision solve; w, the sums and the
+// coefficients stay FP64).  Basis vectors are ld floats apart, ld a multiple of 4: 16-byte loads of four entries;
+// n = 18 n_cells is even but need not be a multiple of 4: the last pair is handled by one thread. ----
+__device__ __forceinline__ void block_sum_to(double v, double* sm, double* dst) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int q = 0; q < RED_T / 32; ++q) t += sm[q];
+    *dst = t;
+  }
+  __syncthreads();
+}
+// v = fl32(a x): the new basis vector, and the same values in FP64 (what the preconditioner reads next)
+__global__ void __launch_bounds__(RED_T) k_scale_f32(int64_t n, double a, const double* __restrict__ x,
+                                                    float* __restrict__ v32, double* __restrict__ v64) {
+  const int64_t n2 = n >> 1;
+  const double2* __restrict__ x2 = reinterpret_cast<const double2*>(x);
+  float2* __restrict__ o32 = reinterpret_cast<float2*>(v32);
+  double2* __restrict__ o64 = reinterpret_cast<double2*>(v64);
+  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n2; e += (int64_t)RED_T * gridDim.x) {
+    const double2 t = x2[e];
+    const float2 f = make_float2((float)(a * t.x), (float)(a * t.y));
+    o32[e] = f;
+    o64[e] = make_double2((double)f.x, (double)f.y);
+  }
+}
+// part[b][j] = V_j . w for j < k, part[b][k] = w . w
+__global__ void __launch_bounds__(RED_T) k_dots_f32(int64_t n, int k, const float* __restrict__ V, int64_t ld,
+                                                   const double* __restrict__ w, double* __restrict__ part) {
+  __shared__ double sm[RED_T / 32];
+  const int64_t n4 = n >> 2, ld4 = ld >> 2;
+  const double2* __restrict__ w2 = reinterpret_cast<const double2*>(w);
+  const float4* __restrict__ V4 = reinterpret_cast<const float4*>(V);
+  const bool tail = (n & 3) && blockIdx.x == 0 && threadIdx.x == 0;   // elements 4 n4, 4 n4 + 1
+  for (int j0 = 0; j0 < k || j0 == 0; j0 += 8) {
+    double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, self = 0.0;
+    const int kj = min(8, k - j0);
+    const float4* __restrict__ Vb = V4 + (int64_t)j0 * ld4;
+    for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n4; e += (int64_t)RED_T * gridDim.x) {
+      const double2 wa = w2[2 * e], wb = w2[2 * e + 1];
+      float4 v[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        if (q < kj) v[q] = Vb[q * ld4 + e];
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        if (q < kj)
+          acc[q] = fma((double)v[q].w, wb.y, fma((double)v[q].z, wb.x, fma((double)v[q].y, wa.y, fma((double)v[q].x, wa.x, acc[q]))));
+      if (j0 == 0) self = fma(wb.y, wb.y, fma(wb.x, wb.x, fma(wa.y, wa.y, fma(wa.x, wa.x, self))));
+    }
+    if (tail) {
+      const double2 wa = w2[2 * n4];
+      for (int q = 0; q < kj; ++q) {
+        const float* vq = V + (int64_t)(j0 + q) * ld + 4 * n4;
+        acc[q] = fma((double)vq[1], wa.y, fma((double)vq[0], wa.x, acc[q]));
+      }
+      if (j0 == 0) self = fma(wa.y, wa.y, fma(wa.x, wa.x, self));
+    }
+    for (int q = 0; q < kj; ++q) block_sum_to(acc[q], sm, part + (int64_t)blockIdx.x * MAXK + j0 + q);
+    if (j0 == 0) block_sum_to(self, sm, part + (int64_t)blockIdx.x * MAXK + k);
+  }
+}
+// w -= sum_j h[j] V_j; with `part`, part[b][0] = the CTA's share of the new w . w
+__global__ void __launch_bounds__(RED_T) k_sub_combination_f32(int64_t n, int k, const float* __restrict__ V, int64_t ld,
+                                                              const double* __restrict__ h, double* __restrict__ w,
+                                                              double* __restrict__ part) {
+  __shared__ double hs[MAXK];
+  __shared__ double sm[RED_T / 32];
+  if (threadIdx.x < k) hs[threadIdx.x] = h[threadIdx.x];
+  __syncthreads();
+  const int64_t n4 = n >> 2, ld4 = ld >> 2;
+  double2* __restrict__ w2 = reinterpret_cast<double2*>(w);
+  const float4* __restrict__ V4 = reinterpret_cast<const float4*>(V);
+  double nrm = 0.0;
+  for (int64_t e = blockIdx.x * (int64_t)RED_T + threadIdx.x; e < n4; e += (int64_t)RED_T * gridDim.x) {
+    double2 a = w2[2 * e], b = w2[2 * e + 1];
+    int j = 0;
+    for (; j + 4 <= k; j += 4) {
+      float4 t[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) t[q] = V4[(int64_t)(j + q) * ld4 + e];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        a.x = fma(-hs[j + q], (double)t[q].x, a.x);
+        a.y = fma(-hs[j + q], (double)t[q].y, a.y);
+        b.x = fma(-hs[j + q], (double)t[q].z, b.x);
+        b.y = fma(-hs[j + q], (double)t[q].w, b.y);
+      }
+    }
+    for (; j < k; ++j) {
+      const float4 t = V4[(int64_t)j * ld4 + e];
+      a.x = fma(-hs[j], (double)t.x, a.x);
+      a.y = fma(-hs[j], (double)t.y, a.y);
+      b.x = fma(-hs[j], (double)t.z, b.x);
+      b.y = fma(-hs[j], (double)t.w, b.y);
+    }
+    w2[2 * e] = a;
+    w2[2 * e + 1] = b;
+    nrm = fma(b.y, b.y, fma(b.x, b.x, fma(a.y, a.y, fma(a.x, a.x, nrm))));
+  }
+  if ((n & 3) && blockIdx.x == 0 && threadIdx.x == 0) {
+    double2 a = w2[2 * n4];
+    for (int j = 0; j < k; ++j) {
+      const float* vq = V + (int64_t)j * ld + 4 * n4;
+      a.x = fma(-hs[j], (double)vq[0], a.x);
+      a.y = fma(-hs[j], (double)vq[1], a.y);
+    }
+    w2[2 * n4] = a;
+    nrm = fma(a.y, a.y, fma(a.x, a.x, nrm));
+  }
+  if (part) block_sum_to(nrm, sm, part + (int64_t)blockIdx.x * MAXK);
+}
 // out = a * x + c * y   (y may be null with c = 0)
 __global__ void __launch_bounds__(RED_T) k_axpby(int64_t n, double a, const double* __restrict__ x, double c,
                                                 const double* __restrict__ y, double* __restrict__ out) {
@@ -631,17 +747,29 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
                       std::function<int(const double*, double*)> op, const double* b, double* x, int restart,
                       int max_iters, double rtol, double* info, void* stream, const double* offd_vals = nullptr,
                       std::function<int(const double*, double*)> op_inner = nullptr,
-                      std::function<void(const double*, double*)> pre = nullptr, double inner_floor = 0.0) {
+                      std::function<void(const double*, double*)> pre = nullptr, double inner_floor = 0.0,
+                      bool basis32 = false) {
   if (restart < 1 || restart > MAXK - 2 || max_iters < 0 || !(rtol >= 0.0))
     return set_error(TFA_EINVAL, "tfa_gmres: restart must be in 1..62, max_iters >= 0, rtol >= 0");
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = (int64_t)NEQ * m->nc;
   const int mk = restart;
-  if (ctx->krylov.n < (int64_t)(mk + 3) * n) TFA_CUDA(ctx->krylov.alloc((int64_t)(mk + 3) * n));
+  const int64_t ld32 = (n + 3) & ~(int64_t)3;   // FP32 basis: vectors this many floats apart
+  const int64_t off32 = (((int64_t)(mk + 1) * ld32 + 1) / 2 + 1) & ~(int64_t)1;   // its size in doubles, even
+  const int64_t need = std::max((int64_t)(mk + 3) * n, basis32 ? off32 + 3 * n : (int64_t)0);
+  if (ctx->krylov.n < need) TFA_CUDA(ctx->krylov.alloc(need));
   if (ctx->red.n < (int64_t)RED_B * MAXK + MAXK) TFA_CUDA(ctx->red.alloc((int64_t)RED_B * MAXK + MAXK));
   double* V = ctx->krylov.p;              // V_0 .. V_mk
   double* w = V + (int64_t)(mk + 1) * n;  // work vector
   double* z = w + n;                      // preconditioned vector
+  // mixed precision: the basis in FP32 (vectors ld32 floats apart), the newest basis vector also in FP64 (vcur)
+  float* V32 = reinterpret_cast<float*>(ctx->krylov.p);
+  double* vcur = nullptr;
+  if (basis32) {
+    w = ctx->krylov.p + off32;
+    z = w + n;
+    vcur = z + n;
+  }
   Gm G{m, bsr_vals, dinv, offd_vals, n, st, ctx->red.p, ctx->red.p + (int64_t)RED_B * MAXK, {}, op, op_inner, pre};
 
   TFA_TRY(G.dots(1, b, n, b));
@@ -665,12 +793,13 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
     // a non-finite residual (NaN / Inf in the matrix, the preconditioner or b): x holds the last iterate
     if (!std::isfinite(beta)) return set_error(TFA_ESINGULAR, "tfa_gmres: the residual norm is not finite");
     if (rel <= rtol || iters >= max_iters) break;
-    k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / beta, w, 0.0, nullptr, V);
+    if (basis32) k_scale_f32<<<RED_B, RED_T, 0, st>>>(n, 1.0 / beta, w, V32, vcur);
+    else k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / beta, w, 0.0, nullptr, V);
     std::fill(g.begin(), g.end(), 0.0);
     g[0] = beta;
     int k = 0;
     for (; k < mk && iters < max_iters; ++k, ++iters) {
-      G.precond(V + (int64_t)k * n, z);
+      G.precond(basis32 ? vcur : V + (int64_t)k * n, z);
       TFA_TRY(G.spmv_inner(z, w));
       // classical Gram-Schmidt (all projections from one pass over the basis), repeated when it cancelled more
       // than a factor 10 of the vector (the Daniel-Gragg-Kaufman-Stewart test with eta = 0.1: the loss of
@@ -682,9 +811,11 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
       for (int j = 0; j <= k + 1; ++j) h[j] = 0.0;
       double hk1 = 0.0;
       for (int pass = 0; pass < 2; ++pass) {
-        k_dots<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, w, G.part, true);
+        if (basis32) k_dots_f32<<<RED_B, RED_T, 0, st>>>(n, k + 1, V32, ld32, w, G.part);
+        else k_dots<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, w, G.part, true);
         k_dots_final<<<k + 2, 32, 0, st>>>(RED_B, G.part, G.out);
-        k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, G.out, w, G.part);
+        if (basis32) k_sub_combination_f32<<<RED_B, RED_T, 0, st>>>(n, k + 1, V32, ld32, G.out, w, G.part);
+        else k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k + 1, V, n, G.out, w, G.part);
         k_dots_final<<<1, 32, 0, st>>>(RED_B, G.part, G.out + k + 2);
         TFA_CUDA(cudaMemcpyAsync(G.host, G.out, sizeof(double) * (k + 3), cudaMemcpyDeviceToHost, st));
         TFA_CUDA(cudaStreamSynchronize(st));
@@ -695,7 +826,10 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
       }
       h[k + 1] = hk1;
       if (!std::isfinite(hk1)) return set_error(TFA_ESINGULAR, "tfa_gmres: a Krylov vector is not finite");
-      if (hk1 > 0.0) k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / hk1, w, 0.0, nullptr, V + (int64_t)(k + 1) * n);
+      if (hk1 > 0.0) {
+        if (basis32) k_scale_f32<<<RED_B, RED_T, 0, st>>>(n, 1.0 / hk1, w, V32 + (int64_t)(k + 1) * ld32, vcur);
+        else k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0 / hk1, w, 0.0, nullptr, V + (int64_t)(k + 1) * n);
+      }
       // Givens rotations on column k of the Hessenberg matrix
       for (int j = 0; j < k; ++j) {
         const double t = cs[j] * h[j] + sn[j] * h[j + 1];
@@ -730,7 +864,8 @@ static int gmres_core(tfa_ctx* ctx, const tfa_mesh* m, const double* bsr_vals, c
       for (int j = 0; j < k; ++j) G.host[j] = -yv[j];
       TFA_CUDA(cudaMemcpyAsync(G.out, G.host, sizeof(double) * k, cudaMemcpyHostToDevice, st));
       TFA_CUDA(cudaMemsetAsync(w, 0, sizeof(double) * n, st));
-      k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k, V, n, G.out, w, nullptr);   // w = sum_j y_j V_j
+      if (basis32) k_sub_combination_f32<<<RED_B, RED_T, 0, st>>>(n, k, V32, ld32, G.out, w, nullptr);
+      else k_sub_combination<<<RED_B, RED_T, 0, st>>>(n, k, V, n, G.out, w, nullptr);   // w = sum_j y_j V_j
       TFA_CUDA(cudaStreamSynchronize(st));
       G.precond(w, z);
       k_axpby<<<RED_B, RED_T, 0, st>>>(n, 1.0, z, 1.0, x, x);
@@ -929,7 +1064,7 @@ int tfa_gmres_packed_f32(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_val
   if (dinv32)
     pre = [=](const double* v, double* z) { k_diag_spmv_f32<<<cdiv(m->nc, SV_CELLS), SV_T, 0, st>>>(m->nc, dinv32, v, z); };
   return gmres_core(ctx, m, diag_vals, nullptr, nullptr, b, x, restart, max_iters, rtol, info, stream,
-                    offd ? offd_vals : diag_vals, inner, pre, 1e-5);
+                    offd ? offd_vals : diag_vals, inner, pre, 1e-5, true);
 }
 
 // ---- matrix-free operator (the paper's future work, L130) ----
