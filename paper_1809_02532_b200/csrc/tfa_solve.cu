@@ -163,22 +163,28 @@ __global__ void k_offd_to_f32(int64_t nblk, const double* __restrict__ src, floa
     dst[t] = e < TFA_PACKED_BLOCK ? (float)src[b * TFA_PACKED_BLOCK + e] : 0.0f;
   }
 }
-__global__ void __launch_bounds__(SV_T) k_packed_spmv_f32(int64_t nc, int BS, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(SV_T) k_packed_spmv_f32(int64_t nc, int BS, int maxrow,
+                                                         const int32_t* __restrict__ rowptr,
                                                          const int32_t* __restrict__ col,
                                                          const int32_t* __restrict__ blkmap,
                                                          const float* __restrict__ dvals, const float* __restrict__ ovals,
                                                          const double* __restrict__ x, double* __restrict__ y) {
+  // shared memory: mbarrier | x rows of every block of the CTA's rows (diagonal ones included), 18 doubles each |
+  // the off-diagonal blocks (FP32, PKF apart)
   extern __shared__ __align__(128) unsigned char ps_raw[];
-  float* const sm = reinterpret_cast<float*>(ps_raw + 16);
   uint64_t* const bar = reinterpret_cast<uint64_t*>(ps_raw);
+  double* const xs = reinterpret_cast<double*>(ps_raw + 16);
+  const int maxblk = SV_CELLS * maxrow;   // maxrow = F + 1 blocks per row at most
+  float* const sm = reinterpret_cast<float*>(ps_raw + 16 + sizeof(double) * NEQ * maxblk);
   const int r = threadIdx.x % NEQ;
   const int64_t i0 = blockIdx.x * (int64_t)SV_CELLS, i = i0 + threadIdx.x / NEQ;
   const int64_t iend = min(i0 + SV_CELLS, nc);
-  const int64_t s0 = rowptr[i0] - i0;   // the CTA's first off-diagonal slot
+  const int64_t B0 = rowptr[i0], B1 = rowptr[iend];
+  const int64_t s0 = B0 - i0;   // the CTA's first off-diagonal slot
   if (threadIdx.x == 0) {
     mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    mbar_arrive_expect_tx(bar, (uint32_t)((rowptr[iend] - iend - s0) * (PKF * sizeof(float))));
+    mbar_arrive_expect_tx(bar, (uint32_t)((B1 - iend - s0) * (PKF * sizeof(float))));
   }
   __syncthreads();
   const bool live = i < nc;
@@ -189,10 +195,24 @@ __global__ void __launch_bounds__(SV_T) k_packed_spmv_f32(int64_t nc, int BS, co
     if (r == 0 && b1 - b0 > 1)
       bulk_load(sm + (b0 - i - s0) * PKF, ovals + (b0 - i) * PKF, (uint32_t)((b1 - b0 - 1) * (PKF * sizeof(float))), bar);
   }
+  // the x rows the CTA multiplies with, gathered once (16-byte pieces, nine per row) instead of once per thread
+  {
+    const int npieces = (int)(B1 - B0) * (NEQ / 2);
+    double2* __restrict__ xs2 = reinterpret_cast<double2*>(xs);
+    const double2* __restrict__ x2 = reinterpret_cast<const double2*>(x);
+    for (int q = threadIdx.x; q < npieces; q += SV_T) {
+      const int blk = q / (NEQ / 2), piece = q - blk * (NEQ / 2);
+      xs2[q] = x2[(int64_t)col[B0 + blk] * (NEQ / 2) + piece];
+    }
+  }
   double acc = 0.0;
+  int base, n, c0, cs, cT;
+  packed_row(r, base, n, c0, cs, cT);
+  __syncthreads();
   if (live) {
+    const int64_t bd = blkmap[(int64_t)BS * i];
     const float2* __restrict__ a = reinterpret_cast<const float2*>(dvals + i * BLK + r * NEQ);
-    const double2* __restrict__ xv = reinterpret_cast<const double2*>(x + NEQ * i);
+    const double2* __restrict__ xv = reinterpret_cast<const double2*>(xs + NEQ * (bd - B0));
 #pragma unroll
     for (int c = 0; c < NEQ / 2; ++c) {
       const float2 av = a[c];
@@ -203,13 +223,11 @@ __global__ void __launch_bounds__(SV_T) k_packed_spmv_f32(int64_t nc, int BS, co
   }
   mbar_wait(bar, 0);
   if (!live) return;
-  int base, n, c0, cs, cT;
-  packed_row(r, base, n, c0, cs, cT);
   const int64_t bd = blkmap[(int64_t)BS * i];
   const float* __restrict__ a = sm + (b0 - i - s0) * PKF + base;
   for (int64_t b = b0; b < b1; ++b) {
     if (b == bd) continue;
-    const double* __restrict__ xj = x + NEQ * (int64_t)col[b];
+    const double* __restrict__ xj = xs + NEQ * (b - B0);
     if (n == 8) {
       const float4* __restrict__ a4 = reinterpret_cast<const float4*>(a);
       const double2* __restrict__ x2 = reinterpret_cast<const double2*>(xj);
@@ -253,8 +271,8 @@ static int launch_packed_spmv_f32(const tfa_mesh* m, const float* dvals, const f
                                   cudaStream_t st) {
   if ((reinterpret_cast<uintptr_t>(dvals) | reinterpret_cast<uintptr_t>(ovals) | reinterpret_cast<uintptr_t>(x)) & 15)
     return set_error(TFA_EINVAL, "tfa_gmres_packed_f32: the FP32 arrays and x must be 16-byte aligned");
-  const size_t smem = 16 + sizeof(float) * SV_CELLS * m->F * PKF;
-  k_packed_spmv_f32<<<cdiv(m->nc, SV_CELLS), SV_T, smem, st>>>(m->nc, blk_stride(m->F), m->bsr_rowptr.p, m->bsr_col.p,
+  const size_t smem = 16 + sizeof(double) * NEQ * SV_CELLS * (m->F + 1) + sizeof(float) * SV_CELLS * m->F * PKF;
+  k_packed_spmv_f32<<<cdiv(m->nc, SV_CELLS), SV_T, smem, st>>>(m->nc, blk_stride(m->F), m->F + 1, m->bsr_rowptr.p, m->bsr_col.p,
                                                               m->blkmap.p, dvals, ovals, x, y);
   return 0;
 }
