@@ -179,6 +179,13 @@ int tfa_assemble_gradient(tfa_ctx* ctx, const tfa_mesh* m, const double* state, 
 int tfa_assemble_faces(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                        const double* state_nm1, double dt, double* rhs, double* bsr_vals, void* stream);
 double* tfa_face_states(tfa_ctx* ctx);
+/* tfa_assemble_faces writing the packed Jacobian (tfa_assemble_packed, below).  On a shard's mesh: diag_vals
+ * [n_owned][18][18] indexed by the owned cell (local id - first_owned_local), offd_vals [nnzb_owned - n_owned][114]:
+ * the owned rows' off-diagonal blocks in pattern order -- the same values, bit for bit, as the corresponding pieces
+ * of the single-GPU packed arrays (half the Jacobian memory per rank). */
+int tfa_assemble_faces_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                              const double* state_nm1, double dt, double* rhs, double* diag_vals, double* offd_vals,
+                              void* stream);
 /* Step a2 without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
  * serving loops, harnesses that forbid it): face_states [n_cells][F][18] (DEVICE pointer, caller-owned) = the
  * reconstructed face states tfa_assemble_gradient leaves in the context, bit for bit, from state [n_cells][18]
@@ -260,8 +267,8 @@ int tfa_implicit_step(tfa_ctx* ctx, const tfa_mesh* m, double* state, const doub
  *                                      17), each row-major.
  * tfa_assemble_packed = tfa_assemble writing that form (same arithmetic, same rhs, bit-identical entries; 5328
  * instead of 10368 bytes of Jacobian per triangle); tfa_packed_to_bsr expands it into the mesh's BSR value array;
- * tfa_packed_spmv, tfa_block_jacobi_packed and tfa_gmres_packed are the linear-solve entry points on it.  Not
- * available on a shard's mesh.  All pointers DEVICE pointers; the packed arrays, x and dinv must be 16-byte aligned
+ * tfa_packed_spmv, tfa_block_jacobi_packed and tfa_gmres_packed are the linear-solve entry points on it (single
+ * mesh only; a shard assembles the packed form with tfa_assemble_faces_packed, tfa_assemble_packed refuses its mesh).  All pointers DEVICE pointers; the packed arrays, x and dinv must be 16-byte aligned
  * (the blocks move by TMA bulk copies and 16-byte loads; TFA_EINVAL otherwise). */
 int tfa_assemble_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
                         const double* state_nm1, double dt, double* rhs, double* diag_vals, double* offd_vals,

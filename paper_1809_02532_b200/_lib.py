@@ -63,6 +63,7 @@ SYMBOLS = {
     "tfa_assemble_gradient": (_int, [_vp, _vp, _vp, _vp]),
     "tfa_assemble_faces": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "tfa_face_states": (_vp, [_vp]),
+    "tfa_assemble_faces_packed": (_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp, _vp]),
     "tfa_face_states_static": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "tfa_partition_create": (_int, [C.POINTER(_vp), _i64, _int, _vp, _vp, _vp, _int, _int]),
     "tfa_partition_destroy": (None, [_vp]),

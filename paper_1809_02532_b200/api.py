@@ -271,6 +271,16 @@ class Context:
                                                   _dp(rhs), _dp(vals), _stream()))
         return rhs, vals
 
+    def assemble_faces_packed(self, mesh: Mesh, state, state_n, state_nm1, dt, rhs, diag, offd):
+        """tfa_assemble_faces_packed: steps a3..a7 on the context's face states, packed output (diag, offd given)."""
+        state_n = state if state_n is None else state_n
+        state_nm1 = state if state_nm1 is None else state_nm1
+        if rhs is None:
+            rhs = torch.empty((mesh.n_cells, NEQ), dtype=torch.float64, device=state.device)
+        _lib.check(_lib.load().tfa_assemble_faces_packed(self._h, mesh._h, _dp(state), _dp(state_n), _dp(state_nm1),
+                                                         float(dt), _dp(rhs), _dp(diag), _dp(offd), _stream()))
+        return rhs, diag, offd
+
     def assemble_host(self, mesh: Mesh, state, state_n, state_nm1, dt, rhs, vals):
         """tfa_assemble_host on HOST buffers (numpy arrays or CPU tensors, ideally pinned)."""
         def hp(x):
@@ -506,6 +516,21 @@ class Shard:
         ctx.assemble_gradient(self.mesh, state)
         exchange(HALO_FACE, ctx.face_states(self.mesh))
         return ctx.assemble_faces(self.mesh, state, state_n, state_nm1, dt, rhs, vals)
+
+    def assemble_packed(self, ctx: Context, state, state_n=None, state_nm1=None, dt=1e-3, rhs=None, diag=None, offd=None,
+                        exchange=None):
+        """The same sharded assembly with the packed Jacobian of the owned rows: diag [n_owned][18][18],
+        offd [nnzb_owned - n_owned][114] (tfa_assemble_faces_packed)."""
+        exchange = exchange or self.exchange
+        f = dict(dtype=torch.float64, device=state.device)
+        if diag is None:
+            diag = torch.empty((self.part.n_owned, NEQ, NEQ), **f)
+        if offd is None:
+            offd = torch.empty((self.nnzb_owned - self.part.n_owned, PACKED_BLOCK), **f)
+        exchange(HALO_STATE, state)
+        ctx.assemble_gradient(self.mesh, state)
+        exchange(HALO_FACE, ctx.face_states(self.mesh))
+        return ctx.assemble_faces_packed(self.mesh, state, state_n, state_nm1, dt, rhs, diag, offd)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -193,6 +193,16 @@ int tfa_assemble_faces(tfa_ctx* ctx, const tfa_mesh* m, const double* state, con
   return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, bsr_vals, stream, false, 2);
 }
 
+int tfa_assemble_faces_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,
+                              const double* state_nm1, double dt, double* rhs, double* diag_vals, double* offd_vals,
+                              void* stream) {
+  if (ctx && m && ctx->ws_uid != m->uid)
+    return set_error(TFA_EINVAL, "tfa_assemble_faces_packed: no face states of this mesh (call tfa_assemble_gradient first)");
+  if (m && m->nc > 0 && !diag_vals) return set_error(TFA_EINVAL, "null argument");
+  return assemble_impl(ctx, m, state, state_n, state_nm1, dt, rhs, diag_vals, stream, false, 2,
+                       offd_vals ? offd_vals : diag_vals);
+}
+
 double* tfa_face_states(tfa_ctx* ctx) { return ctx ? ctx->fown.p : nullptr; }
 
 int tfa_assemble_host(tfa_ctx* ctx, const tfa_mesh* m, const double* state, const double* state_n,

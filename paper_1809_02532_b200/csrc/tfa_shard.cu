@@ -196,16 +196,22 @@ constexpr int TPB = 256;
 // first owned row's first block.
 __global__ void k_shard_tables(int64_t nl, int F, int BS, int64_t o0, int64_t o1, int32_t off,
                                const int32_t* __restrict__ cell_nbr, int32_t* __restrict__ nbrf,
-                               int32_t* __restrict__ blkmap) {
+                               int32_t* __restrict__ blkmap, int32_t* __restrict__ pblkmap) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= nl) return;
   const bool own = i >= o0 && i < o1;
   int32_t* b = blkmap + BS * i;
+  int32_t* pb = pblkmap + BS * i;
   b[0] = own ? b[0] - off : -1;
+  // packed form of the owned rows: diagonal blocks indexed by the owned cell, off-diagonal blocks in the order of
+  // the owned rows' pattern with the diagonal ones taken out (columns ascend in local id, so the mirror block
+  // (j, i) lies behind row j's diagonal block exactly when i > j)
+  pb[0] = own ? (int32_t)(i - o0) : -1;
   for (int k = 0; k < F; ++k) {
     const int64_t j = cell_nbr[F * i + k];
     const bool to_owned = j >= o0 && j < o1;
     b[1 + k] = (to_owned && b[1 + k] >= 0) ? b[1 + k] - off : -1;
+    pb[1 + k] = b[1 + k] >= 0 ? b[1 + k] - (int32_t)(j - o0) - (i > j ? 1 : 0) : -1;
     if (!own && !to_owned) nbrf[F * i + k] = -1;
   }
 }
@@ -304,7 +310,7 @@ int tfa_shard_create(tfa_shard** out, const tfa_mesh* g, int n_ranks, int rank, 
     s->nnzb_owned = nl ? rp[o1] - rp[o0] : 0;
     if (nl) {
       k_shard_tables<<<cdiv(nl, TPB), TPB, 0, st>>>(nl, F, BS, o0, o1, (int32_t)s->block_offset, m.cell_nbr.p, m.nbrf.p,
-                                                   m.blkmap.p);
+                                                   m.blkmap.p, m.pblkmap.p);
       TFA_CUDA(cudaGetLastError());
     }
     for (int kind = 0; kind < 2; ++kind) {

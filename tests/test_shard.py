@@ -139,7 +139,7 @@ def test_halo_exchange_two_gloo_processes():
 # ------------------------------------------------------------------------------------------
 # GPU: the sharded assembly, ranks emulated one after another in one process on one GPU
 # ------------------------------------------------------------------------------------------
-def sharded_assembly(api, gmesh, n_ranks, P, Pn, Pnm1, dt, ghost=None, numerics=None):
+def sharded_assembly(api, gmesh, n_ranks, P, Pn, Pnm1, dt, ghost=None, numerics=None, packed=None):
     """Assemble with n_ranks shards of `gmesh` living in this process; the halos travel through the library's pack
     and unpack kernels (api.exchange_in_process).  Returns per rank (shard, rhs, vals) and the local states."""
     import torch
@@ -172,6 +172,13 @@ def sharded_assembly(api, gmesh, n_ranks, P, Pn, Pnm1, dt, ghost=None, numerics=
         vals = torch.full((s.nnzb_owned, 18, 18), nan, dtype=torch.float64, device="cuda")
         rhs, _ = c.assemble_faces(s.mesh, st, sn, sm, dt, vals=vals)
         c.check()
+        if packed is not None:   # the packed Jacobian of the owned rows, from the same face states
+            n = s.part.n_owned
+            pd = torch.full((n, 18, 18), nan, dtype=torch.float64, device="cuda")
+            po = torch.full((s.nnzb_owned - n, 114), nan, dtype=torch.float64, device="cuda")
+            rhs_p, _, _ = c.assemble_faces_packed(s.mesh, st, sn, sm, dt, None, pd, po)
+            c.check()
+            packed.append((rhs_p, pd, po))
         out.append((s, rhs, vals))
     return out, loc
 
@@ -203,7 +210,16 @@ def test_sharded_assembly_equals_the_single_gpu_assembly_bit_for_bit(orc, W, kin
     rhs_g, vals_g = ctx.assemble(g, dev(P), dev(Pn), dev(Pnm1), 1e-3)
     ctx.check()
     rp_g, col_g = g.get("bsr_rowptr"), g.get("bsr_col")
-    out, _ = sharded_assembly(api, g, n_ranks, P, Pn, Pnm1, 1e-3, ghost)
+    packed = []
+    out, _ = sharded_assembly(api, g, n_ranks, P, Pn, Pnm1, 1e-3, ghost, packed=packed)
+    # the packed output of a shard (tfa_assemble_faces_packed): the rank's pieces of the single-GPU packed arrays
+    _, diag_g, offd_g = ctx.assemble_packed(g, dev(P), dev(Pn), dev(Pnm1), 1e-3)
+    for (s, rhs, vals), (rhs_p, pd, po) in zip(out, packed):
+        o0, n, c0 = s.part.first_owned_local, s.part.n_owned, s.part.first_owned_global
+        assert not bool(torch.isnan(pd).any()) and not bool(torch.isnan(po).any())
+        assert torch.equal(rhs_p[o0:o0 + n], rhs[o0:o0 + n])
+        assert torch.equal(pd, diag_g[c0:c0 + n])
+        assert torch.equal(po, offd_g[int(rp_g[c0]) - c0:int(rp_g[c0 + n]) - (c0 + n)])
     rows_seen = 0
     for s, rhs, vals in out:
         assert not bool(torch.isnan(vals).any()), "an owned block was not written"
