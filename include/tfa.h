@@ -284,7 +284,8 @@ int tfa_block_jacobi_packed(tfa_ctx* ctx, const tfa_mesh* m, const double* diag_
  * problem are FP64); the residual b - A x at every restart, and the one reported in info[1], is computed with the FP64
  * matrix, and a cycle ends once it has reduced its own residual by 1e-5 (iterative refinement with GMRES as the
  * inner solver: the FP32 copy perturbs the operator by 6e-8 relative, which a restart corrects).  Same stopping
- * rule, same error codes as tfa_gmres_packed.  The copies are the caller's: tfa_packed_to_f32 fills
+ * rule, same error codes as tfa_gmres_packed (matrix entries beyond the FP32 range become infinite in the copy and
+ * end the solve with TFA_ESINGULAR).  The copies are the caller's: tfa_packed_to_f32 fills
  * diag32 [n_cells][18][18] and offd32 [nnzb - n_cells][TFA_PACKED_BLOCK_F32] (114 entries + 2 of padding: blocks
  * 464 bytes apart), tfa_to_f32 converts any array (the inverses dinv -> dinv32).  DEVICE pointers, 16-byte aligned. */
 #define TFA_PACKED_BLOCK_F32 116
